@@ -1,0 +1,201 @@
+"""ctypes front end of oracle/oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may import
+this module.  It imports nothing from the CUDA path; inputs are plain numpy arrays
+(normally those written by paper_2203_14354_b200.synth, which holds no method arithmetic).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "oracle.cpp"
+_LIB = _HERE / "liboracle.so"
+
+FATE_NAMES = ("detected", "bulk_absorbed", "surface_absorbed", "escaped", "truncated", "nan_abort")
+FATE_DETECTED, FATE_BULK_ABSORBED, FATE_SURFACE_ABSORBED, FATE_ESCAPED, FATE_TRUNCATED, FATE_NAN_ABORT = range(6)
+H_RAYLEIGH, H_REFLECT_DIFFUSE, H_REFLECT_SPECULAR, H_SURFACE_TRANSMIT = 0x10, 0x20, 0x40, 0x80
+H_FRESNEL_REFLECT, H_FRESNEL_REFRACT, H_TIR = 0x100, 0x200, 0x400
+
+
+def build(force: bool = False) -> Path:
+    """Compile oracle.cpp with g++ (no CUDA, no external libraries)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-pthread", "-ffp-contract=off",
+                               str(_SRC), "-o", str(tmp)])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(str(build()))
+        vp, i32, i64, u32, u64, f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_double
+        L.orc_create.restype = vp
+        L.orc_destroy.argtypes = [vp]
+        L.orc_hardware_threads.restype = C.c_int
+        L.orc_set_materials.argtypes = [vp, C.c_int, C.c_int, f64, f64, vp, vp, vp]
+        L.orc_set_surfaces.argtypes = [vp, C.c_int, C.c_int, f64, f64, vp, vp, vp, vp]
+        L.orc_set_geometry.argtypes = [vp, i64, vp, i64, vp, vp, vp, vp, vp]
+        L.orc_build_bvh.argtypes = [vp]
+        L.orc_first_hit.argtypes = [vp, i64] + [vp] * 7 + [C.c_int, vp, vp, C.c_int]
+        L.orc_propagate.argtypes = ([vp, i64] + [vp] * 11 + [u64, u64, i32, C.c_int] + [vp] * 8 +
+                                    [i64, vp, i64, f64, f64, vp, vp, vp, C.c_int])
+        L.orc_philox4x32_10.argtypes = [vp, vp, vp]
+        L.orc_uniforms.argtypes = [u64, u64, u32, u32, vp]
+        L.orc_rayleigh.argtypes = [vp, vp, u64, u64, u32]
+        L.orc_rayleigh.restype = C.c_int
+        L.orc_lambert.argtypes = [vp, vp, vp, u64, u64, u32]
+        L.orc_specular.argtypes = [vp, vp, vp]
+        L.orc_fresnel.argtypes = [f64, f64, vp, vp, vp, f64, vp]
+        L.orc_fresnel.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _f32(a):
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def hardware_threads() -> int:
+    return int(lib().orc_hardware_threads())
+
+
+class Oracle:
+    """One scene (geometry + optical tables) in the double-precision CPU tracker."""
+
+    def __init__(self, geometry=None, optics=None, bvh: bool | None = None):
+        self.L = lib()
+        self.h = C.c_void_p(self.L.orc_create())
+        self.use_bvh = False
+        self.n_chan = 0
+        if optics is not None:
+            self.set_optics(optics)
+        if geometry is not None:
+            self.set_geometry(geometry)
+            if bvh is None:
+                bvh = geometry.n_tri > 5000
+            if bvh:
+                self.build_bvh()
+
+    def __del__(self):
+        try:
+            self.L.orc_destroy(self.h)
+        except Exception:
+            pass
+
+    def set_optics(self, o):
+        self.L.orc_set_materials(self.h, o.refr_index.shape[0], o.n_lambda, o.lambda0, o.dlambda,
+                                 _p(_f32(o.refr_index)), _p(_f32(o.abs_len)), _p(_f32(o.scat_len)))
+        self.L.orc_set_surfaces(self.h, o.detect.shape[0], o.n_lambda, o.lambda0, o.dlambda, _p(_f32(o.detect)),
+                                _p(_f32(o.reflect_diffuse)), _p(_f32(o.reflect_specular)), _p(_f32(o.transmit)))
+
+    def set_geometry(self, g):
+        self.n_chan = int(g.n_channels)
+        self.L.orc_set_geometry(self.h, g.n_vert, _p(_f32(g.xyz)), g.n_tri, _p(_i32(g.idx)), _p(_i32(g.mat_inner)),
+                                _p(_i32(g.mat_outer)), _p(_i32(g.surface)), _p(_i32(g.channel)))
+        self.use_bvh = False
+
+    def build_bvh(self) -> int:
+        n = self.L.orc_build_bvh(self.h)
+        self.use_bvh = True
+        return n
+
+    def first_hit(self, origin, direction, exclude=None, use_bvh: bool | None = None, nthreads: int | None = None):
+        """origin, direction: [3,n] float32.  Returns (tri int32[n], dist float64[n])."""
+        o, d = _f32(origin), _f32(direction)
+        n = o.shape[1]
+        tri = np.empty(n, np.int32)
+        dist = np.empty(n, np.float64)
+        ex = None if exclude is None else _i32(exclude)
+        ub = self.use_bvh if use_bvh is None else use_bvh
+        self.L.orc_first_hit(self.h, n, _p(o[0]), _p(o[1]), _p(o[2]), _p(d[0]), _p(d[1]), _p(d[2]), _p(ex), int(ub),
+                             _p(tri), _p(dist), nthreads or hardware_threads())
+        return tri, dist
+
+    def propagate(self, ph, seed: int, max_steps: int, n_bins: int = 0, t_min: float = 0.0, dt: float = 1.0,
+                  use_bvh: bool | None = None, nthreads: int | None = None, full: bool = True) -> dict:
+        """ph: synth.Photons.  Returns dict of per-photon arrays and histograms (numpy)."""
+        n = ph.n
+        pos, k, e = _f32(ph.pos), _f32(ph.dir), _f32(ph.pol)
+        wl, t0 = _f32(ph.wavelength), _f32(ph.t0)
+        out = dict(flags=np.zeros(n, np.uint32), channel=np.full(n, -1, np.int32), t=np.zeros(n, np.float64),
+                   steps=np.zeros(n, np.uint32), last_tri=np.full(n, -1, np.int32))
+        if full:
+            out.update(pos=np.zeros((3, n)), dir=np.zeros((3, n)), pol=np.zeros((3, n)))
+        out.update(chan_count=np.zeros(self.n_chan, np.uint64), time_hist=np.zeros(n_bins, np.uint64),
+                   fate_count=np.zeros(8, np.uint64), total_steps=np.zeros(1, np.uint64))
+        ub = self.use_bvh if use_bvh is None else use_bvh
+        self.L.orc_propagate(self.h, n, _p(pos[0]), _p(pos[1]), _p(pos[2]), _p(k[0]), _p(k[1]), _p(k[2]),
+                             _p(e[0]), _p(e[1]), _p(e[2]), _p(wl), _p(t0), int(ph.id_base), int(seed), int(max_steps),
+                             int(ub), _p(out["flags"]), _p(out["channel"]), _p(out["t"]), _p(out["steps"]),
+                             _p(out["last_tri"]), _p(out.get("pos")), _p(out.get("dir")), _p(out.get("pol")),
+                             self.n_chan, _p(out["chan_count"]), n_bins, float(t_min), float(dt), _p(out["time_hist"]),
+                             _p(out["fate_count"]), _p(out["total_steps"]), nthreads or hardware_threads())
+        out["fate"] = out["flags"] & 0xF
+        return out
+
+
+# ---- single pieces (for the pins)
+def philox4x32_10(ctr, key):
+    c = np.asarray(ctr, np.uint32)
+    k = np.asarray(key, np.uint32)
+    o = np.zeros(4, np.uint32)
+    lib().orc_philox4x32_10(_p(c), _p(k), _p(o))
+    return o
+
+
+def uniforms(seed, photon, step, block):
+    o = np.zeros(4)
+    lib().orc_uniforms(seed, photon, step, block, _p(o))
+    return o
+
+
+def rayleigh(k, e, seed, pid, step=0):
+    k = np.array(k, np.float64)
+    e = np.array(e, np.float64)
+    it = lib().orc_rayleigh(_p(k), _p(e), seed, pid, step)
+    return k, e, it
+
+
+def lambert(nhat, seed, pid, step=0):
+    n = np.array(nhat, np.float64)
+    k = np.zeros(3)
+    e = np.zeros(3)
+    lib().orc_lambert(_p(n), _p(k), _p(e), seed, pid, step)
+    return k, e
+
+
+def specular(nhat, k, e):
+    n = np.array(nhat, np.float64)
+    k = np.array(k, np.float64)
+    e = np.array(e, np.float64)
+    lib().orc_specular(_p(n), _p(k), _p(e))
+    return k, e
+
+
+def fresnel(n1, n2, nhat, k, e, u):
+    n = np.array(nhat, np.float64)
+    k = np.array(k, np.float64)
+    e = np.array(e, np.float64)
+    R = C.c_double(0.0)
+    oc = lib().orc_fresnel(float(n1), float(n2), _p(n), _p(k), _p(e), float(u), C.byref(R))
+    return oc, R.value, k, e
