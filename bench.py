@@ -1,0 +1,300 @@
+#!/usr/bin/env python
+"""bench.py -- photons propagated / s on the DARWIN-scale TPC (BASELINE.json configs[2]) on N B200s.
+
+A "step" is one pass of the whole hot path (photon claim -> Philox -> BVH first hit -> bulk / surface physics ->
+fates and per-PMT / arrival-time reductions) over one batch of 1e7 synthetic photons resident in HBM.
+    python bench.py --gpus N --steps K --warmup W            # this library (one rank per GPU under torchrun)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on a bounded sample (rank 0 only)
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "photons propagated/sec on 1 B200 (DARWIN-scale TPC); % of propagation roofline"
+UNIT = "photons/s"
+# Algorithmic work per photon-step at C2: the ideal path of an 8-wide BVH
+# over T = 113 280 triangles with 4-triangle leaves = ceil(log8(T/4)) = 5 nodes x 125 lane-instructions
+# + 4 triangles x 45 + 250 for the physics of the step = 1055 lane-instructions; 5 x 80 B + 4 x 48 B = 592 B.
+ALG_LANE_INSTR_PER_STEP = 5 * 125 + 4 * 45 + 250
+ALG_BYTES_PER_STEP = 5 * 80 + 4 * 48
+ALG_STATE_BYTES_PER_PHOTON = 52 + 32
+SM_COUNT, LANES_PER_SM = 148, 128
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return dict(hbm_gbs=float(d.get("hbm_gbs", 6650.0)), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons during the timed region (pynvml; nvidia-smi as a fallback)."""
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._proc = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            names = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+                     0x80: "hw_power_brake_slowdown"}
+
+            def loop():
+                while not self._stop.is_set():
+                    try:
+                        self.samples.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                        r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                        for bit, nm in names.items():
+                            if r & bit:
+                                self.reasons.add(nm)
+                    except Exception:
+                        pass
+                    time.sleep(self.period)
+            self._thr = threading.Thread(target=loop, daemon=True)
+            self._thr.start()
+        except Exception:
+            q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                 "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+            try:
+                self._proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                               "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            except Exception:
+                self._proc = None
+        return self
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thr:
+            self._thr.join(timeout=1.0)
+        if self._proc:
+            self._proc.terminate()
+            try:
+                out, _ = self._proc.communicate(timeout=2.0)
+            except Exception:
+                out = ""
+            for line in out.splitlines():
+                f = [x.strip() for x in line.split(",")]
+                if len(f) >= 6:
+                    try:
+                        self.samples.append(float(f[0]))
+                        self.max_mhz = float(f[1])
+                    except ValueError:
+                        continue
+                    for nm, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[2:6]):
+                        if v.lower().startswith("active"):
+                            self.reasons.add(nm)
+        med = float(np.median(self.samples)) if self.samples else None
+        return dict(sm_mhz=med, sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons), samples=len(self.samples))
+
+
+def workload(args):
+    from paper_2203_14354_b200 import synth
+    c = synth.config(args.config)
+    n = args.photons or c.n_photons
+    return c, n
+
+
+def cpu_baseline(c, n_sample, id_base=0, threads=None):
+    """The oracle, as it stands, on the first n_sample photons of the workload's batch."""
+    from oracle import oracle as orc
+    o = orc.Oracle(c.geometry, c.optics, bvh=True)
+    cores = threads or orc.hardware_threads()
+    ph = c.make_photons(n_sample, id_base)
+    t0 = time.perf_counter()
+    out = o.propagate(ph, c.seed, c.max_steps, n_bins=2000, dt=1.0, full=False, nthreads=cores)
+    dt = time.perf_counter() - t0
+    return dict(value=n_sample / dt, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"first {n_sample} photons of the {c.name} batch, all {cores} host threads, {dt:.2f} s",
+                photon_steps_per_s=float(out["total_steps"][0]) / dt, seconds=dt,
+                detected_fraction=float(out["fate_count"][0]) / n_sample), o
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores; each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    c, n_full = workload(args)
+    n_sample = args.ref_sample
+    from oracle import oracle as orc
+    o = orc.Oracle(c.geometry, c.optics, bvh=True)
+    cores = orc.hardware_threads()
+    times, steps_total = [], 0
+    for it in range(args.warmup + args.steps):
+        ph = c.make_photons(n_sample, it * n_sample)
+        t0 = time.perf_counter()
+        out = o.propagate(ph, c.seed, c.max_steps, n_bins=2000, dt=1.0, full=False, nthreads=cores)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+            steps_total += int(out["total_steps"][0])
+    total = sum(times)
+    value = n_sample * args.steps / total
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=1e3 * total / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", config=dict(workload=c.name, photons_per_step=n_sample, full_batch=n_full, max_steps=c.max_steps,
+                                              triangles=c.geometry.n_tri),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle",
+                                  sample=f"{n_sample} photons of the {c.name} batch per step, {cores} host threads"),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                photon_steps_per_s=steps_total / total, gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: DARWIN-scale TPC)")
+    ap.add_argument("--photons", type=int, default=0, help="photons per step per GPU (default: the config's batch)")
+    ap.add_argument("--ref-sample", type=int, default=100_000, help="photons per step of the oracle (--impl reference / cpu_baseline)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2203_14354_b200 import binding as dw
+    from paper_2203_14354_b200 import dist as dwdist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU path")
+    rank, world, local = dwdist.init_from_env()
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    c, n = workload(args)
+    ctx = dw.Context(local)
+    ctx.set_optics(c.optics)
+    ctx.set_geometry(c.geometry)
+    stats = ctx.build_bvh()
+    id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
+    ph = c.make_photons(n, id_base)
+    d_ph = dw.DevicePhotons(ph, dev)
+    out = dw.DeviceResults(n, ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), dev)   # 32 B / photon
+    hist = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0, dev)
+    stream = torch.cuda.current_stream()
+    flags = dw.PROP_UNBOUNDED_QUERY if args.literal else 0
+
+    def step():
+        ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream)
+        if world > 1:
+            dwdist.merge_hists(hist)        # the only exchange: tens of kB of integer histograms
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    hist.zero_()
+    dwdist.barrier()
+    torch.cuda.synchronize()
+    launches0 = ctx.last_launch()["n_launches"]
+    sampler = ClockSampler(local).start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record(stream)
+    for i in range(args.steps):
+        step()
+        ev[i + 1].record(stream)
+    torch.cuda.synchronize()
+    dwdist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    per_step_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[-1])
+    total_ms = dwdist.max_over_ranks(total_ms)
+    launches = ctx.last_launch()["n_launches"] - launches0
+    h = hist.numpy()                                # this rank's reductions over the K timed steps
+    local_steps = int(h["total_steps"][0])
+    total_steps = dwdist.sum_over_ranks(local_steps)
+    fate = h["fate_count"].astype(np.int64)
+    n_all = n * world
+    value = n_all * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the host-buffer entry (pinned host memory, H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        hp = dw.HostPhotons(ph)
+        hout = dw.HostResults(n, ("flags", "channel", "t"))
+        hh = dw.HostHists(ctx.n_chan, 2000, 0.0, 1.0)
+        ctx.propagate_host(hp, c.seed, c.max_steps, hout, hh, flags=flags)      # warm-up (allocates staging)
+        dwdist.barrier()
+        t0 = time.perf_counter()
+        reps = max(1, min(args.steps, 3))
+        for _ in range(reps):
+            ctx.propagate_host(hp, c.seed, c.max_steps, hout, hh, flags=flags)
+        torch.cuda.synchronize()
+        dt = dwdist.max_over_ranks(time.perf_counter() - t0)
+        e2e = dict(value=n_all * reps / dt, unit=UNIT, h2d_bytes_per_step=int(hp.nbytes), d2h_bytes_per_step=int(hout.nbytes + hh.nbytes),
+                   ms_per_step=1e3 * dt / reps, api="dw_propagate_host (pinned host buffers, chunked copies overlapped with propagation)")
+
+    if rank != 0:
+        dwdist.finalize()
+        return 0
+
+    peaks = measured_peaks()
+    kernel_ms = float(np.mean(per_step_ms))
+    steps_per_launch = local_steps / args.steps
+    peak_lane = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6          # lane-instructions / s
+    achieved_lane = steps_per_launch * ALG_LANE_INSTR_PER_STEP / (kernel_ms * 1e-3)
+    alg_bytes = steps_per_launch * ALG_BYTES_PER_STEP + n * ALG_STATE_BYTES_PER_PHOTON
+    roofline = dict(bound="alu", achieved=achieved_lane / 1e12, peak=peak_lane / 1e12, unit="Tlane-instr/s",
+                    frac=achieved_lane / peak_lane, traffic=None, kernel="propagate_kernel", kernel_ms=kernel_ms,
+                    algorithmic_lane_instr_per_photon_step=ALG_LANE_INSTR_PER_STEP,
+                    algorithmic_bytes_per_launch=alg_bytes,
+                    memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
+                    peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)")
+    traffic_file = ROOT / "profiles" / "traffic.json"
+    if traffic_file.exists():
+        try:
+            roofline["traffic"] = json.loads(traffic_file.read_text()).get(f"C{args.config}")
+        except Exception:
+            pass
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu, _ = cpu_baseline(c, args.ref_sample)
+
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                data="synthetic",
+                config=dict(workload=c.name, photons_per_step_per_gpu=n, triangles=c.geometry.n_tri, max_steps=c.max_steps,
+                            seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
+                            mode="literal" if args.literal else "bounded rays", bvh_nodes=stats["n_nodes"],
+                            bvh_build_ms=stats["build_ms"], launch=ctx.last_launch()),
+                photon_steps_per_s=total_steps / (total_ms * 1e-3),
+                steps_per_photon=total_steps / (n_all * args.steps),
+                fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
+                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu)
+    print(json.dumps(line))
+    dwdist.finalize()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

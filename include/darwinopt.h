@@ -1,0 +1,200 @@
+/* darwinopt.h -- C ABI of libdarwinopt.so: B200-native photon propagation through a triangle-mesh
+ * detector, the hot path of "GPU-based optical simulation of the DARWIN detector" (arXiv 2203.14354).
+ *
+ * Citations: P:<n> = line n of the paper text; S<k>/G<k> = step / reading of DESIGN.md
+ * section "Oracle and readings" (same numbering as SURVEY.md section 8(c)).
+ *
+ * What the calls are (section 1: "the core of the framework's photon propagation code is written in
+ * CUDA C"; the problem statement: upload geometry and wavelength-tabulated optical properties, build the
+ * acceleration structure, propagate a photon batch with a step limit, get per-channel hits and fates):
+ *
+ *   dw_create / dw_destroy            context on one CUDA device; owns every device copy it makes
+ *   dw_set_materials                  n, L_abs, L_Rayleigh per material vs wavelength        (Table 2)
+ *   dw_set_surfaces                   detect / diffuse / specular / transmit probabilities
+ *   dw_set_geometry                   triangle mesh + per-triangle inner/outer material, surface, channel
+ *   dw_build_bvh                      device LBVH build (one-off per geometry)
+ *   dw_first_hit                      nearest triangle along rays (S1) -- the parity entry of the query
+ *   dw_propagate                      the Monte Carlo loop S1..S13 for a photon batch, device buffers
+ *   dw_propagate_host                 same, host buffers (copies inside), for end-to-end timing
+ *
+ * Conventions
+ *   - Units mm, ns, nm.  c = 299.792458 mm/ns.  All floating point is IEEE fp32.
+ *   - Triangle normal n_g = normalize((v1-v0)x(v2-v0)) points from the INNER to the OUTER material.
+ *   - Every function returns 0 (DW_OK) or a negative dw_status; nothing throws or aborts across the ABI.
+ *     dw_last_error() gives a context-owned message valid until the next call on that context.
+ *   - "host" / "device" is stated for every pointer.  The library never frees or keeps caller pointers
+ *     after the call returns, except stream-ordered use: device buffers passed to an asynchronous call
+ *     must stay alive until the stream has reached the end of that call's work.
+ *   - Triangle ids in all outputs are the CALLER's numbering (the BVH leaf order is internal).
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - There is no CPU fallback: without a CUDA device dw_create fails with DW_E_CUDA.
+ */
+#ifndef DARWINOPT_H_
+#define DARWINOPT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dw_ctx dw_ctx;
+
+typedef enum dw_status {
+  DW_OK = 0,
+  DW_E_ARG = -1,    /* NULL / negative / inconsistent argument                                  */
+  DW_E_STATE = -2,  /* call out of order (e.g. propagate before build_bvh, geometry before tables) */
+  DW_E_CUDA = -3,   /* a CUDA runtime call failed; message in dw_last_error                     */
+  DW_E_RANGE = -4   /* an index in the geometry is out of range, or a probability table is invalid */
+} dw_status;
+
+/* Photon fate = low 4 bits of the per-photon flags word; exactly one per photon (S10, S11, P9). */
+enum {
+  DW_FATE_DETECTED = 0,         /* hit a triangle with a surface, "detect" drawn        */
+  DW_FATE_BULK_ABSORBED = 1,    /* absorbed in the medium (Table 2 L_abs)                        */
+  DW_FATE_SURFACE_ABSORBED = 2, /* explicit surface, none of detect/reflect/transmit drawn       */
+  DW_FATE_ESCAPED = 3,          /* ray left the world (G3)                                       */
+  DW_FATE_TRUNCATED = 4,        /* max_steps reached                                             */
+  DW_FATE_NAN_ABORT = 5,        /* non-finite state (must count 0)                               */
+  DW_FATE_MASK = 0xF
+};
+/* History bits OR-ed into flags. */
+enum {
+  DW_H_RAYLEIGH = 0x10, DW_H_REFLECT_DIFFUSE = 0x20, DW_H_REFLECT_SPECULAR = 0x40,
+  DW_H_SURFACE_TRANSMIT = 0x80, DW_H_FRESNEL_REFLECT = 0x100, DW_H_FRESNEL_REFRACT = 0x200,
+  DW_H_TIR = 0x400,
+  DW_H_MEDIUM_MISMATCH = 0x800  /* carried medium != medium seen from the hit triangle (ill-formed mesh) */
+};
+
+int dw_create(int cuda_device, dw_ctx** out);
+int dw_destroy(dw_ctx* ctx);
+const char* dw_last_error(const dw_ctx* ctx); /* ctx may be NULL: message of the last failed dw_create */
+int dw_version(void);
+
+/* Materials on a uniform wavelength grid lambda0 + i*dlambda (i < n_lambda, n_lambda >= 1); values between
+ * nodes are linearly interpolated and clamped at the ends (S3, G13).  Arrays are HOST pointers, row-major
+ * [n_mat][n_lambda]; abs_len_mm / scat_len_mm = +inf switches the process off.  n_mat <= 255. */
+int dw_set_materials(dw_ctx* ctx, int n_mat, int n_lambda, float lambda0, float dlambda,
+                     const float* refr_index, const float* abs_len_mm, const float* scat_len_mm);
+
+/* Explicit surfaces (reflectivity "explicitly specified (separately for diffuse and specular
+ * components)", independent of the angle of incidence).  HOST pointers, [n_surf][n_lambda] each.  One uniform
+ * number is compared with the cumulative sums in the order detect, reflect_diffuse, reflect_specular,
+ * transmit; the remainder absorbs (S7).  DW_E_RANGE if an entry is < 0 or a sum exceeds 1 + 1e-6.
+ * n_surf <= 254.  May be called again at any time (a design sweep changes reflectivities without a BVH
+ * rebuild); the grid may differ from the materials' grid. */
+int dw_set_surfaces(dw_ctx* ctx, int n_surf, int n_lambda, float lambda0, float dlambda,
+                    const float* detect, const float* reflect_diffuse, const float* reflect_specular,
+                    const float* transmit);
+
+/* Geometry: xyz [n_vert][3] fp32, idx [n_tri][3] int32, and per triangle the inner / outer material id,
+ * the surface id (-1 = none: Fresnel between the two materials, S8) and the sensor channel (-1 = none).
+ * pointers_are_device = 0: HOST pointers; 1: DEVICE pointers (read on the legacy default stream).
+ * The data is copied; the caller keeps ownership.  Requires materials and surfaces to be set (ids are
+ * validated against them): DW_E_STATE otherwise; DW_E_RANGE on an out-of-range index or id, a non-finite
+ * vertex, or a zero-area triangle.  Invalidates a previous BVH. */
+int dw_set_geometry(dw_ctx* ctx, int64_t n_vert, const float* xyz, int64_t n_tri, const int32_t* idx,
+                    const int32_t* mat_inner, const int32_t* mat_outer, const int32_t* surface,
+                    const int32_t* channel, int pointers_are_device);
+
+typedef struct dw_build_params {
+  int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (4) */
+  int32_t reserved[7];
+} dw_build_params;
+
+typedef struct dw_build_stats {
+  int64_t n_tri, n_nodes, node_bytes, tri_bytes;
+  int32_t max_depth, n_leaves;
+  float scene_lo[3], scene_hi[3];
+  float build_ms; /* device time of the whole build */
+} dw_build_stats;
+
+/* Device LBVH build: triangle boxes -> scene bounds -> 63-bit Morton codes of the centroids -> radix sort ->
+ * binary radix tree -> bottom-up refit -> traversal nodes + triangles permuted to leaf order.
+ * params NULL = defaults; stats may be NULL.  Synchronises the stream before returning (one-off call). */
+int dw_build_bvh(dw_ctx* ctx, const dw_build_params* params, dw_build_stats* stats, void* cuda_stream);
+
+/* First hit (S1): for ray i the triangle with the smallest d > 0 along o + d*dir, ignoring triangle
+ * exclude_tri[i] (caller id; pointer may be NULL); exact ties -> lowest caller id.  DEVICE pointers, length n.
+ * Miss: tri_out = -1, dist_out = +inf.  Asynchronous on the stream. */
+int dw_first_hit(dw_ctx* ctx, int64_t n, const float* ox, const float* oy, const float* oz,
+                 const float* dx, const float* dy, const float* dz, const int32_t* exclude_tri,
+                 int32_t* tri_out, float* dist_out, void* cuda_stream);
+
+/* Photon batch, structure of arrays, each of length n (52 B per photon).  Directions and polarisations are
+ * unit vectors with pol . dir = 0.  photon_id_base + i is photon i's identity in the counter-based random
+ * number generator (Philox4x32-10, key = seed, counter = (id lo, id hi, step, block)), so that splitting or
+ * permuting a batch does not change any photon's result. */
+typedef struct dw_photons {
+  int64_t n;
+  uint64_t photon_id_base;
+  const float *px, *py, *pz;   /* position, mm     */
+  const float *kx, *ky, *kz;   /* direction        */
+  const float *ex, *ey, *ez;   /* polarisation     */
+  const float* wavelength;     /* nm               */
+  const float* t0;             /* start time, ns   */
+} dw_photons;
+
+/* Per-photon results, each of length n; any pointer may be NULL (not written). */
+typedef struct dw_results {
+  uint32_t* flags;    /* fate | history bits                                  */
+  int32_t* channel;   /* sensor channel if DETECTED else -1                   */
+  float* t;           /* time at the end of the track, ns                     */
+  uint32_t* steps;    /* loop iterations executed, including the terminating one */
+  int32_t* last_tri;  /* caller id of the last surface touched, -1 if none / after a scatter */
+  float *x, *y, *z;   /* final position                                       */
+  float *kx, *ky, *kz;/* final direction   (diagnostic)                       */
+  float *ex, *ey, *ez;/* final polarisation (diagnostic)                      */
+} dw_results;
+
+/* Reductions (S13).  All ACCUMULATED into: the caller zeroes them, so that the batches of a sweep add up.
+ * Any pointer may be NULL. */
+typedef struct dw_hists {
+  int64_t n_chan;          /* length of chan_count; detected photons with channel outside [0,n_chan) are not counted */
+  uint64_t* chan_count;    /* [n_chan] photons DETECTED per channel                                 */
+  int64_t n_bins;          /* length of time_hist                                                   */
+  float t_min, dt;         /* bin = floor((t - t_min)/dt) clamped to [0, n_bins-1]                  */
+  uint32_t* time_hist;     /* [n_bins] arrival times of detected photons                            */
+  uint64_t* fate_count;    /* [8] photons per fate code                                             */
+  uint64_t* total_steps;   /* [1] photon-steps executed                                             */
+} dw_hists;
+
+typedef struct dw_propagate_params {
+  uint32_t flags;          /* DW_PROP_* */
+  int32_t block_threads;   /* 0 = default */
+  int32_t blocks_per_sm;   /* 0 = default */
+  int32_t reserved[5];
+} dw_propagate_params;
+enum {
+  /* Follow the oracle literally: every query is unbounded and the medium comes from the hit triangle (S2).
+   * Default (flag clear): the medium is carried in the photon state after the first query and the sampled
+   * bulk distance bounds the ray; equal in distribution in a closed world. */
+  DW_PROP_UNBOUNDED_QUERY = 1u
+};
+
+/* The propagation loop S1..S13 for every photon of the batch, at most max_steps iterations each.
+ * DEVICE pointers throughout.  Asynchronous on the stream; no host synchronisation inside.
+ * params / out / hist may be NULL. */
+int dw_propagate(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps,
+                 const dw_results* out, const dw_hists* hist, const dw_propagate_params* params,
+                 void* cuda_stream);
+
+/* Same computation with HOST pointers in `in`, `out` and `hist` (pinned memory recommended): the call copies
+ * the batch to the device in chunks overlapped with propagation, copies the requested results back and ADDS
+ * the reductions into the host arrays.  Synchronous: returns when the host buffers are complete. */
+int dw_propagate_host(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps,
+                      const dw_results* out, const dw_hists* hist, const dw_propagate_params* params);
+
+/* Diagnostics / tests: raw Philox4x32-10 blocks and the uniforms the kernel derives from them, computed on the
+ * device.  out_raw [n][4] uint32, out_u [n][4] float (either may be NULL), DEVICE pointers; entry i uses
+ * photon id photon_id_base + i, the given step and block. */
+int dw_debug_philox(dw_ctx* ctx, uint64_t seed, uint64_t photon_id_base, uint32_t step, uint32_t block,
+                    int64_t n, uint32_t* out_raw, float* out_u, void* cuda_stream);
+
+/* Last kernel launch configuration used by dw_propagate (grid, block, dynamic smem bytes, kernels launched). */
+int dw_last_launch(const dw_ctx* ctx, int32_t* grid, int32_t* block, int32_t* smem_bytes, int64_t* n_launches);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DARWINOPT_H_ */

@@ -1,0 +1,333 @@
+"""Thin ctypes binding of libdarwinopt.so (include/darwinopt.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's kernels.
+There is no fallback: if the library is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+from . import build as _build
+
+_LIB_PATH = Path(__file__).resolve().parent / "libdarwinopt.so"
+
+DW_OK, DW_E_ARG, DW_E_STATE, DW_E_CUDA, DW_E_RANGE = 0, -1, -2, -3, -4
+FATE_NAMES = ("detected", "bulk_absorbed", "surface_absorbed", "escaped", "truncated", "nan_abort")
+FATE_DETECTED, FATE_BULK_ABSORBED, FATE_SURFACE_ABSORBED, FATE_ESCAPED, FATE_TRUNCATED, FATE_NAN_ABORT = range(6)
+H_RAYLEIGH, H_REFLECT_DIFFUSE, H_REFLECT_SPECULAR, H_SURFACE_TRANSMIT = 0x10, 0x20, 0x40, 0x80
+H_FRESNEL_REFLECT, H_FRESNEL_REFRACT, H_TIR, H_MEDIUM_MISMATCH = 0x100, 0x200, 0x400, 0x800
+PROP_UNBOUNDED_QUERY = 1
+
+EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
+           "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
+           "dw_debug_philox", "dw_last_launch")
+
+vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
+
+
+class BuildParams(C.Structure):
+    _fields_ = [("max_leaf_tris", i32), ("reserved", i32 * 7)]
+
+
+class BuildStats(C.Structure):
+    _fields_ = [("n_tri", i64), ("n_nodes", i64), ("node_bytes", i64), ("tri_bytes", i64), ("max_depth", i32),
+                ("n_leaves", i32), ("scene_lo", f32 * 3), ("scene_hi", f32 * 3), ("build_ms", f32)]
+
+
+class Photons(C.Structure):
+    _fields_ = [("n", i64), ("photon_id_base", u64)] + [(k, vp) for k in
+                ("px", "py", "pz", "kx", "ky", "kz", "ex", "ey", "ez", "wavelength", "t0")]
+
+
+class Results(C.Structure):
+    _fields_ = [(k, vp) for k in ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z",
+                                  "kx", "ky", "kz", "ex", "ey", "ez")]
+
+
+class Hists(C.Structure):
+    _fields_ = [("n_chan", i64), ("chan_count", vp), ("n_bins", i64), ("t_min", f32), ("dt", f32),
+                ("time_hist", vp), ("fate_count", vp), ("total_steps", vp)]
+
+
+class PropagateParams(C.Structure):
+    _fields_ = [("flags", u32), ("block_threads", i32), ("blocks_per_sm", i32), ("reserved", i32 * 5)]
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = True) -> C.CDLL:
+    """dlopen the C-ABI library (building it in-tree with nvcc first if it is not there)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIB_PATH.exists():
+        if not build_if_missing:
+            raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2203_14354_b200.build`")
+        _build.build()
+    L = C.CDLL(str(_LIB_PATH))
+    L.dw_create.argtypes = [C.c_int, C.POINTER(vp)]
+    L.dw_destroy.argtypes = [vp]
+    L.dw_last_error.argtypes = [vp]
+    L.dw_last_error.restype = C.c_char_p
+    L.dw_version.restype = C.c_int
+    L.dw_set_materials.argtypes = [vp, C.c_int, C.c_int, f32, f32, vp, vp, vp]
+    L.dw_set_surfaces.argtypes = [vp, C.c_int, C.c_int, f32, f32, vp, vp, vp, vp]
+    L.dw_set_geometry.argtypes = [vp, i64, vp, i64, vp, vp, vp, vp, vp, C.c_int]
+    L.dw_build_bvh.argtypes = [vp, C.POINTER(BuildParams), C.POINTER(BuildStats), vp]
+    L.dw_first_hit.argtypes = [vp, i64] + [vp] * 9 + [vp]
+    L.dw_propagate.argtypes = [vp, C.POINTER(Photons), u64, i32, C.POINTER(Results), C.POINTER(Hists),
+                               C.POINTER(PropagateParams), vp]
+    L.dw_propagate_host.argtypes = [vp, C.POINTER(Photons), u64, i32, C.POINTER(Results), C.POINTER(Hists),
+                                    C.POINTER(PropagateParams)]
+    L.dw_debug_philox.argtypes = [vp, u64, u64, u32, u32, i64, vp, vp, vp]
+    L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
+    for name in EXPORTS:
+        if name not in ("dw_last_error",):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+class DwError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libdarwinopt error {code}: {msg}")
+        self.code = code
+
+
+def _np(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def _hp(a):
+    return None if a is None else a.ctypes.data_as(vp)
+
+
+def _dp(t):
+    """device (or pinned host) pointer of a torch tensor"""
+    return None if t is None else vp(t.data_ptr())
+
+
+def _stream_ptr(stream=None):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return vp(s.cuda_stream)
+
+
+class Context:
+    """One dw_ctx: a geometry + optical tables + BVH on one CUDA device."""
+
+    def __init__(self, device: int = 0):
+        self.L = load()
+        h = vp()
+        rc = self.L.dw_create(device, C.byref(h))
+        if rc != DW_OK:
+            raise DwError(rc, self.L.dw_last_error(None).decode())
+        self.h = h
+        self.device = device
+        self.n_chan = 0
+        self.stats = None
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.dw_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != DW_OK:
+            raise DwError(rc, self.L.dw_last_error(self.h).decode())
+
+    # ---- uploads -------------------------------------------------------------------------------------
+    def set_materials(self, refr_index, abs_len, scat_len, lambda0=175.0, dlambda=1.0):
+        n, la, ls = (_np(a, np.float32) for a in (refr_index, abs_len, scat_len))
+        n = n.reshape(n.shape[0], -1)
+        self._check(self.L.dw_set_materials(self.h, n.shape[0], n.shape[1], lambda0, dlambda, _hp(n), _hp(la), _hp(ls)))
+
+    def set_surfaces(self, detect, reflect_diffuse, reflect_specular, transmit, lambda0=175.0, dlambda=1.0):
+        d, rd, rs, tr = (_np(a, np.float32) for a in (detect, reflect_diffuse, reflect_specular, transmit))
+        d = d.reshape(d.shape[0], -1)
+        self._check(self.L.dw_set_surfaces(self.h, d.shape[0], d.shape[1], lambda0, dlambda, _hp(d), _hp(rd), _hp(rs), _hp(tr)))
+
+    def set_optics(self, o):
+        self.set_materials(o.refr_index, o.abs_len, o.scat_len, o.lambda0, o.dlambda)
+        self.set_surfaces(o.detect, o.reflect_diffuse, o.reflect_specular, o.transmit, o.lambda0, o.dlambda)
+
+    def set_geometry(self, g):
+        xyz, idx = _np(g.xyz, np.float32), _np(g.idx, np.int32)
+        mi, mo, sf, ch = (_np(a, np.int32) for a in (g.mat_inner, g.mat_outer, g.surface, g.channel))
+        self._check(self.L.dw_set_geometry(self.h, xyz.shape[0], _hp(xyz), idx.shape[0], _hp(idx), _hp(mi), _hp(mo),
+                                           _hp(sf), _hp(ch), 0))
+        self.n_chan = int(g.n_channels)
+
+    def set_geometry_device(self, xyz, idx, mat_inner, mat_outer, surface, channel, n_channels):
+        """torch CUDA tensors (float32 [V,3], int32 [T,3], int32 [T] x4)."""
+        self._check(self.L.dw_set_geometry(self.h, xyz.shape[0], _dp(xyz), idx.shape[0], _dp(idx), _dp(mat_inner),
+                                           _dp(mat_outer), _dp(surface), _dp(channel), 1))
+        self.n_chan = int(n_channels)
+
+    def build_bvh(self, max_leaf_tris: int = 0, stream=None) -> dict:
+        p = BuildParams(max_leaf_tris=max_leaf_tris)
+        st = BuildStats()
+        self._check(self.L.dw_build_bvh(self.h, C.byref(p), C.byref(st), _stream_ptr(stream)))
+        self.stats = {k: (list(getattr(st, k)) if k.startswith("scene") else getattr(st, k)) for k, _ in BuildStats._fields_}
+        return self.stats
+
+    # ---- queries -------------------------------------------------------------------------------------
+    def first_hit(self, origin, direction, exclude=None, stream=None):
+        """origin, direction: torch CUDA float32 [3,n] (rows contiguous).  Returns (tri int32[n], dist float32[n])."""
+        import torch
+        n = origin.shape[1]
+        tri = torch.empty(n, dtype=torch.int32, device=origin.device)
+        dist = torch.empty(n, dtype=torch.float32, device=origin.device)
+        self._check(self.L.dw_first_hit(self.h, n, _dp(origin[0]), _dp(origin[1]), _dp(origin[2]), _dp(direction[0]),
+                                        _dp(direction[1]), _dp(direction[2]), _dp(exclude), _dp(tri), _dp(dist),
+                                        _stream_ptr(stream)))
+        return tri, dist
+
+    def propagate(self, ph: "DevicePhotons", seed: int, max_steps: int, out: "DeviceResults | None" = None,
+                  hist: "DeviceHists | None" = None, flags: int = 0, block_threads: int = 0, blocks_per_sm: int = 0,
+                  stream=None):
+        pp = PropagateParams(flags=flags, block_threads=block_threads, blocks_per_sm=blocks_per_sm)
+        self._check(self.L.dw_propagate(self.h, C.byref(ph.c), seed, max_steps, C.byref(out.c) if out else None,
+                                        C.byref(hist.c) if hist else None, C.byref(pp), _stream_ptr(stream)))
+
+    def propagate_host(self, ph: "HostPhotons", seed: int, max_steps: int, out=None, hist=None, flags: int = 0):
+        pp = PropagateParams(flags=flags)
+        self._check(self.L.dw_propagate_host(self.h, C.byref(ph.c), seed, max_steps, C.byref(out.c) if out else None,
+                                             C.byref(hist.c) if hist else None, C.byref(pp)))
+
+    def debug_philox(self, seed, base, step, block, n):
+        import torch
+        raw = torch.empty((n, 4), dtype=torch.int32, device=f"cuda:{self.device}")
+        u = torch.empty((n, 4), dtype=torch.float32, device=f"cuda:{self.device}")
+        self._check(self.L.dw_debug_philox(self.h, seed, base, step, block, n, _dp(raw), _dp(u), _stream_ptr()))
+        return raw.cpu().numpy().view(np.uint32), u.cpu().numpy()
+
+    def last_launch(self) -> dict:
+        g, b, s, n = i32(), i32(), i32(), i64()
+        self.L.dw_last_launch(self.h, C.byref(g), C.byref(b), C.byref(s), C.byref(n))
+        return dict(grid=g.value, block=b.value, smem=s.value, n_launches=n.value)
+
+
+_IN = ("px", "py", "pz", "kx", "ky", "kz", "ex", "ey", "ez", "wavelength", "t0")
+_OUT_DT = dict(flags="int32", channel="int32", t="float32", steps="int32", last_tri="int32", x="float32", y="float32",
+               z="float32", kx="float32", ky="float32", kz="float32", ex="float32", ey="float32", ez="float32")
+
+
+class _PhotonsBase:
+    def _fill(self, tensors, n, id_base):
+        self.t = tensors
+        self.n = n
+        self.c = Photons(n=n, photon_id_base=id_base, **{k: vp(tensors[k].data_ptr()) for k in _IN})
+
+    @property
+    def nbytes(self):
+        return 4 * 11 * self.n
+
+
+class DevicePhotons(_PhotonsBase):
+    """SoA photon batch resident on the device (torch tensors own the memory)."""
+
+    def __init__(self, ph, device="cuda:0"):
+        import torch
+        rows = dict(px=ph.pos[0], py=ph.pos[1], pz=ph.pos[2], kx=ph.dir[0], ky=ph.dir[1], kz=ph.dir[2],
+                    ex=ph.pol[0], ey=ph.pol[1], ez=ph.pol[2], wavelength=ph.wavelength, t0=ph.t0)
+        self._fill({k: torch.from_numpy(_np(v, np.float32)).to(device) for k, v in rows.items()}, ph.n, ph.id_base)
+
+
+class HostPhotons(_PhotonsBase):
+    """SoA photon batch in pinned host memory (for dw_propagate_host)."""
+
+    def __init__(self, ph, pin=True):
+        import torch
+        rows = dict(px=ph.pos[0], py=ph.pos[1], pz=ph.pos[2], kx=ph.dir[0], ky=ph.dir[1], kz=ph.dir[2],
+                    ex=ph.pol[0], ey=ph.pol[1], ez=ph.pol[2], wavelength=ph.wavelength, t0=ph.t0)
+        ts = {}
+        for k, v in rows.items():
+            t = torch.from_numpy(_np(v, np.float32).copy())
+            ts[k] = t.pin_memory() if pin else t
+        self._fill(ts, ph.n, ph.id_base)
+
+
+class _ResultsBase:
+    def numpy(self):
+        out = {}
+        for k, t in self.t.items():
+            a = t.cpu().numpy()
+            out[k] = a.view(np.uint32) if k in ("flags", "steps") else a
+        if "flags" in out:
+            out["fate"] = out["flags"] & 0xF
+        return out
+
+    @property
+    def nbytes(self):
+        return sum(t.numel() * t.element_size() for t in self.t.values())
+
+
+class DeviceResults(_ResultsBase):
+    def __init__(self, n, fields=("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), device="cuda:0"):
+        import torch
+        self.t = {k: torch.empty(n, dtype=getattr(torch, _OUT_DT[k]), device=device) for k in fields}
+        self.c = Results(**{k: vp(t.data_ptr()) for k, t in self.t.items()})
+
+
+class HostResults(_ResultsBase):
+    def __init__(self, n, fields=("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), pin=True):
+        import torch
+        self.t = {k: torch.empty(n, dtype=getattr(torch, _OUT_DT[k]), pin_memory=pin) for k in fields}
+        self.c = Results(**{k: vp(t.data_ptr()) for k, t in self.t.items()})
+
+
+class _HistsBase:
+    def _make(self, n_chan, n_bins, t_min, dt, **kw):
+        import torch
+        self.chan_count = torch.zeros(max(n_chan, 1), dtype=torch.int64, **kw)
+        self.time_hist = torch.zeros(max(n_bins, 1), dtype=torch.int32, **kw)
+        self.fate_count = torch.zeros(8, dtype=torch.int64, **kw)
+        self.total_steps = torch.zeros(1, dtype=torch.int64, **kw)
+        self.n_chan, self.n_bins = n_chan, n_bins
+        self.c = Hists(n_chan=n_chan, chan_count=vp(self.chan_count.data_ptr()), n_bins=n_bins, t_min=t_min, dt=dt,
+                       time_hist=vp(self.time_hist.data_ptr()) if n_bins > 0 else None,
+                       fate_count=vp(self.fate_count.data_ptr()), total_steps=vp(self.total_steps.data_ptr()))
+
+    def zero_(self):
+        for t in (self.chan_count, self.time_hist, self.fate_count, self.total_steps):
+            t.zero_()
+
+    def numpy(self):
+        return dict(chan_count=self.chan_count.cpu().numpy()[: self.n_chan].astype(np.uint64),
+                    time_hist=self.time_hist.cpu().numpy()[: self.n_bins].view(np.uint32).astype(np.uint64),
+                    fate_count=self.fate_count.cpu().numpy().astype(np.uint64),
+                    total_steps=self.total_steps.cpu().numpy().astype(np.uint64))
+
+    @property
+    def nbytes(self):
+        return 8 * self.n_chan + 4 * self.n_bins + 64 + 8
+
+
+class DeviceHists(_HistsBase):
+    def __init__(self, n_chan, n_bins=0, t_min=0.0, dt=1.0, device="cuda:0"):
+        self._make(n_chan, n_bins, t_min, dt, device=device)
+
+
+class HostHists(_HistsBase):
+    def __init__(self, n_chan, n_bins=0, t_min=0.0, dt=1.0):
+        self._make(n_chan, n_bins, t_min, dt)
+
+
+def make_context(geometry, optics, device: int = 0, max_leaf_tris: int = 0) -> Context:
+    """Upload tables + geometry and build the BVH."""
+    ctx = Context(device)
+    ctx.set_optics(optics)
+    ctx.set_geometry(geometry)
+    ctx.build_bvh(max_leaf_tris)
+    return ctx

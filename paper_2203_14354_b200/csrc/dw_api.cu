@@ -1,0 +1,361 @@
+// dw_api.cu -- host side of the C ABI (include/darwinopt.h): context, table and geometry upload with
+// validation, and the host-buffer (end-to-end) propagation entry.  No arithmetic of the method lives here.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "dw_internal.cuh"
+
+static std::string g_create_err;
+
+int dw_fail(dw_ctx* ctx, int code, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (ctx) ctx->err = buf; else g_create_err = buf;
+  return code;
+}
+
+extern "C" int dw_version(void) { return DW_VERSION; }
+
+extern "C" const char* dw_last_error(const dw_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+extern "C" int dw_create(int cuda_device, dw_ctx** out) {
+  if (!out) return dw_fail(nullptr, DW_E_ARG, "dw_create: out is NULL");
+  *out = nullptr;
+  int n = 0;
+  cudaError_t e = cudaGetDeviceCount(&n);
+  if (e != cudaSuccess || n == 0)
+    return dw_fail(nullptr, DW_E_CUDA, "dw_create: no CUDA device (%s); this library has no CPU fallback",
+                   e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+  if (cuda_device < 0 || cuda_device >= n) return dw_fail(nullptr, DW_E_ARG, "dw_create: device %d of %d", cuda_device, n);
+  e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) return dw_fail(nullptr, DW_E_CUDA, "cudaSetDevice: %s", cudaGetErrorString(e));
+  dw_ctx* c = new dw_ctx();
+  c->device = cuda_device;
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
+  *out = c;
+  return DW_OK;
+}
+
+static void free_geometry(dw_ctx* c) {
+  cudaFree(c->d_xyz); cudaFree(c->d_idx); cudaFree(c->d_code); cudaFree(c->d_chan);
+  c->d_xyz = nullptr; c->d_idx = nullptr; c->d_code = nullptr; c->d_chan = nullptr;
+  cudaFree(c->d_nodes); cudaFree(c->d_tris);
+  c->d_nodes = nullptr; c->d_tris = nullptr;
+  c->have_geom = false; c->built = false;
+}
+
+extern "C" int dw_destroy(dw_ctx* c) {
+  if (!c) return DW_OK;
+  cudaSetDevice(c->device);
+  free_geometry(c);
+  cudaFree(c->d_mat); cudaFree(c->d_surf);
+  if (c->stage) cudaFree(c->stage);
+  for (int i = 0; i < 2; ++i) {
+    if (c->stage_streams[i]) cudaStreamDestroy(c->stage_streams[i]);
+    if (c->stage_events[i]) cudaEventDestroy(c->stage_events[i]);
+  }
+  delete c;
+  return DW_OK;
+}
+
+extern "C" int dw_set_materials(dw_ctx* c, int n_mat, int nl, float l0, float dl, const float* n, const float* la,
+                                const float* ls) {
+  if (!c) return DW_E_ARG;
+  if (n_mat < 1 || n_mat > 255 || nl < 1 || !n || !la || !ls || !(dl > 0.f) || !isfinite(l0))
+    return dw_fail(c, DW_E_ARG, "dw_set_materials: bad argument (n_mat=%d n_lambda=%d dlambda=%g)", n_mat, nl, dl);
+  size_t m = (size_t)n_mat * nl;
+  std::vector<float> h(3 * m);
+  for (size_t i = 0; i < m; ++i) {
+    if (!(n[i] > 0.f) || !isfinite(n[i])) return dw_fail(c, DW_E_RANGE, "dw_set_materials: refractive index [%zu] = %g", i, n[i]);
+    if (!(la[i] > 0.f) || !(ls[i] > 0.f)) return dw_fail(c, DW_E_RANGE, "dw_set_materials: length [%zu] must be > 0 (or +inf)", i);
+    h[i] = n[i]; h[m + i] = la[i]; h[2 * m + i] = ls[i];
+  }
+  DW_CUDA(c, cudaSetDevice(c->device));
+  DW_CUDA(c, cudaDeviceSynchronize());
+  cudaFree(c->d_mat); c->d_mat = nullptr;
+  DW_CUDA(c, cudaMalloc(&c->d_mat, h.size() * sizeof(float)));
+  DW_CUDA(c, cudaMemcpy(c->d_mat, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+  c->tables.mat = c->d_mat; c->tables.n_mat = n_mat; c->tables.nl_mat = nl;
+  c->tables.mat_l0 = l0; c->tables.mat_inv_dl = 1.0f / dl;
+  c->have_mat = true;
+  return DW_OK;
+}
+
+extern "C" int dw_set_surfaces(dw_ctx* c, int n_surf, int nl, float l0, float dl, const float* det, const float* rd,
+                               const float* rs, const float* tr) {
+  if (!c) return DW_E_ARG;
+  if (n_surf < 1 || n_surf > 254 || nl < 1 || !det || !rd || !rs || !tr || !(dl > 0.f) || !isfinite(l0))
+    return dw_fail(c, DW_E_ARG, "dw_set_surfaces: bad argument (n_surf=%d n_lambda=%d dlambda=%g)", n_surf, nl, dl);
+  if (c->have_geom && n_surf < c->tables.n_surf)
+    return dw_fail(c, DW_E_RANGE, "dw_set_surfaces: geometry was validated against %d surfaces, got %d", c->tables.n_surf, n_surf);
+  size_t m = (size_t)n_surf * nl;
+  std::vector<float> h(4 * m);
+  for (size_t i = 0; i < m; ++i) {
+    float p[4] = {det[i], rd[i], rs[i], tr[i]};
+    double s = 0;
+    for (int k = 0; k < 4; ++k) {
+      if (!(p[k] >= 0.f)) return dw_fail(c, DW_E_RANGE, "dw_set_surfaces: probability %d of entry %zu is %g", k, i, p[k]);
+      s += p[k];
+      h[k * m + i] = (float)s;   // cumulative
+    }
+    if (s > 1.0 + 1e-6) return dw_fail(c, DW_E_RANGE, "dw_set_surfaces: probabilities of entry %zu sum to %g > 1", i, s);
+  }
+  DW_CUDA(c, cudaSetDevice(c->device));
+  DW_CUDA(c, cudaDeviceSynchronize());   // a sweep swaps tables between batches: wait for kernels reading the old ones
+  cudaFree(c->d_surf); c->d_surf = nullptr;
+  DW_CUDA(c, cudaMalloc(&c->d_surf, h.size() * sizeof(float)));
+  DW_CUDA(c, cudaMemcpy(c->d_surf, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+  c->tables.surf = c->d_surf; c->tables.n_surf = n_surf; c->tables.nl_surf = nl;
+  c->tables.surf_l0 = l0; c->tables.surf_inv_dl = 1.0f / dl;
+  c->have_surf = true;
+  return DW_OK;
+}
+
+// Validation + packing of the per-triangle codes on the device (one pass, works for host and device input).
+__global__ void validate_pack_kernel(int64_t n_vert, const float* __restrict__ xyz, int64_t n_tri,
+                                     const int32_t* __restrict__ idx, const int32_t* __restrict__ mi,
+                                     const int32_t* __restrict__ mo, const int32_t* __restrict__ sf, int n_mat,
+                                     int n_surf, uint32_t* __restrict__ code, unsigned long long* __restrict__ errs) {
+  int64_t t = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (t >= n_tri) return;
+  int i0 = idx[3 * t], i1 = idx[3 * t + 1], i2 = idx[3 * t + 2];
+  bool bad_idx = i0 < 0 || i1 < 0 || i2 < 0 || i0 >= n_vert || i1 >= n_vert || i2 >= n_vert;
+  int a = mi[t], b = mo[t], s = sf[t];
+  bool bad_id = a < 0 || a >= n_mat || b < 0 || b >= n_mat || s < -1 || s >= n_surf;
+  if (bad_idx) { atomicAdd(&errs[0], 1ull); atomicMin(&errs[4], (unsigned long long)t); return; }
+  if (bad_id) { atomicAdd(&errs[1], 1ull); atomicMin(&errs[4], (unsigned long long)t); }
+  float v[9];
+  bool fin = true;
+  for (int k = 0; k < 3; ++k) {
+    v[k] = xyz[3 * (int64_t)i0 + k]; v[3 + k] = xyz[3 * (int64_t)i1 + k]; v[6 + k] = xyz[3 * (int64_t)i2 + k];
+  }
+  for (int k = 0; k < 9; ++k) fin = fin && isfinite(v[k]);
+  if (!fin) { atomicAdd(&errs[2], 1ull); atomicMin(&errs[4], (unsigned long long)t); return; }
+  double e1x = (double)v[3] - v[0], e1y = (double)v[4] - v[1], e1z = (double)v[5] - v[2];
+  double e2x = (double)v[6] - v[0], e2y = (double)v[7] - v[1], e2z = (double)v[8] - v[2];
+  double cx = e1y * e2z - e1z * e2y, cy = e1z * e2x - e1x * e2z, cz = e1x * e2y - e1y * e2x;
+  if (!(cx * cx + cy * cy + cz * cz > 0.0)) { atomicAdd(&errs[3], 1ull); atomicMin(&errs[4], (unsigned long long)t); }
+  code[t] = (uint32_t)(a & 0xFF) | ((uint32_t)(b & 0xFF) << 8) | ((uint32_t)((s < 0 ? 0xFF : s) & 0xFF) << 16);
+}
+
+extern "C" int dw_set_geometry(dw_ctx* c, int64_t n_vert, const float* xyz, int64_t n_tri, const int32_t* idx,
+                               const int32_t* mi, const int32_t* mo, const int32_t* sf, const int32_t* ch, int on_dev) {
+  if (!c) return DW_E_ARG;
+  if (!c->have_mat || !c->have_surf) return dw_fail(c, DW_E_STATE, "dw_set_geometry: set materials and surfaces first");
+  if (n_vert < 0 || n_tri < 0 || n_tri >= (1ll << 28) || n_vert >= (1ll << 31))
+    return dw_fail(c, DW_E_ARG, "dw_set_geometry: sizes out of range (n_vert=%lld n_tri=%lld)", (long long)n_vert, (long long)n_tri);
+  if ((n_vert > 0 && !xyz) || (n_tri > 0 && (!idx || !mi || !mo || !sf || !ch)))
+    return dw_fail(c, DW_E_ARG, "dw_set_geometry: NULL array");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  DW_CUDA(c, cudaDeviceSynchronize());
+  free_geometry(c);
+  c->n_vert = n_vert; c->n_tri = n_tri;
+  if (n_tri == 0) { c->have_geom = true; return DW_OK; }
+  cudaMemcpyKind kind = on_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  int32_t *d_mi = nullptr, *d_mo = nullptr, *d_sf = nullptr;
+  unsigned long long* d_err = nullptr;
+  auto cleanup = [&]() { cudaFree(d_mi); cudaFree(d_mo); cudaFree(d_sf); cudaFree(d_err); };
+#define DW_TRY(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { cleanup(); free_geometry(c); \
+    return dw_fail(c, DW_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e__)); } } while (0)
+  DW_TRY(cudaMalloc(&c->d_xyz, sizeof(float) * 3 * std::max<int64_t>(n_vert, 1)));
+  DW_TRY(cudaMalloc(&c->d_idx, sizeof(int32_t) * 3 * n_tri));
+  DW_TRY(cudaMalloc(&c->d_code, sizeof(uint32_t) * n_tri));
+  DW_TRY(cudaMalloc(&c->d_chan, sizeof(int32_t) * n_tri));
+  DW_TRY(cudaMalloc(&d_mi, sizeof(int32_t) * n_tri));
+  DW_TRY(cudaMalloc(&d_mo, sizeof(int32_t) * n_tri));
+  DW_TRY(cudaMalloc(&d_sf, sizeof(int32_t) * n_tri));
+  DW_TRY(cudaMalloc(&d_err, sizeof(unsigned long long) * 8));
+  DW_TRY(cudaMemcpy(c->d_xyz, xyz, sizeof(float) * 3 * n_vert, kind));
+  DW_TRY(cudaMemcpy(c->d_idx, idx, sizeof(int32_t) * 3 * n_tri, kind));
+  DW_TRY(cudaMemcpy(c->d_chan, ch, sizeof(int32_t) * n_tri, kind));
+  DW_TRY(cudaMemcpy(d_mi, mi, sizeof(int32_t) * n_tri, kind));
+  DW_TRY(cudaMemcpy(d_mo, mo, sizeof(int32_t) * n_tri, kind));
+  DW_TRY(cudaMemcpy(d_sf, sf, sizeof(int32_t) * n_tri, kind));
+  unsigned long long h_err[8] = {0, 0, 0, 0, ~0ull, 0, 0, 0};
+  DW_TRY(cudaMemcpy(d_err, h_err, sizeof h_err, cudaMemcpyHostToDevice));
+  validate_pack_kernel<<<(unsigned)((n_tri + 255) / 256), 256>>>(n_vert, c->d_xyz, n_tri, c->d_idx, d_mi, d_mo, d_sf,
+                                                                 c->tables.n_mat, c->tables.n_surf, c->d_code, d_err);
+  DW_TRY(cudaGetLastError());
+  DW_TRY(cudaMemcpy(h_err, d_err, sizeof h_err, cudaMemcpyDeviceToHost));
+#undef DW_TRY
+  cleanup();
+  if (h_err[0] || h_err[1] || h_err[2] || h_err[3]) {
+    free_geometry(c);
+    return dw_fail(c, DW_E_RANGE,
+                   "dw_set_geometry: %llu triangles with vertex index out of range, %llu with material/surface id out of "
+                   "range, %llu with non-finite vertices, %llu with zero area (first bad triangle %llu)",
+                   h_err[0], h_err[1], h_err[2], h_err[3], h_err[4]);
+  }
+  c->have_geom = true;
+  return DW_OK;
+}
+
+extern "C" int dw_build_bvh(dw_ctx* c, const dw_build_params* p, dw_build_stats* st, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!c->have_geom) return dw_fail(c, DW_E_STATE, "dw_build_bvh: no geometry");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_bvh_build_impl(c, p, st, (cudaStream_t)stream);
+}
+
+extern "C" int dw_first_hit(dw_ctx* c, int64_t n, const float* ox, const float* oy, const float* oz, const float* dx,
+                            const float* dy, const float* dz, const int32_t* ex, int32_t* tri, float* dist, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!c->built) return dw_fail(c, DW_E_STATE, "dw_first_hit: build the BVH first");
+  if (n < 0 || (n > 0 && (!ox || !oy || !oz || !dx || !dy || !dz || !tri || !dist)))
+    return dw_fail(c, DW_E_ARG, "dw_first_hit: bad argument");
+  if (n == 0) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_first_hit_impl(c, n, ox, oy, oz, dx, dy, dz, ex, tri, dist, (cudaStream_t)stream);
+}
+
+static int check_batch(dw_ctx* c, const char* who, const dw_photons* in, int32_t max_steps, const dw_hists* h) {
+  if (!c->built) return dw_fail(c, DW_E_STATE, "%s: build the BVH first", who);
+  if (!in || in->n < 0 || max_steps < 0) return dw_fail(c, DW_E_ARG, "%s: bad batch / max_steps", who);
+  if (in->n > 0 && (!in->px || !in->py || !in->pz || !in->kx || !in->ky || !in->kz || !in->ex || !in->ey || !in->ez ||
+                    !in->wavelength || !in->t0))
+    return dw_fail(c, DW_E_ARG, "%s: NULL photon array", who);
+  if (h) {
+    if (h->n_chan < 0 || h->n_bins < 0 || (h->chan_count && h->n_chan == 0 && false))
+      return dw_fail(c, DW_E_ARG, "%s: bad histogram sizes", who);
+    if (h->time_hist && h->n_bins > 0 && !(h->dt > 0.f)) return dw_fail(c, DW_E_ARG, "%s: time histogram needs dt > 0", who);
+  }
+  return DW_OK;
+}
+
+extern "C" int dw_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                            const dw_hists* hist, const dw_propagate_params* params, void* stream) {
+  if (!c) return DW_E_ARG;
+  int rc = check_batch(c, "dw_propagate", in, max_steps, hist);
+  if (rc) return rc;
+  if (in->n == 0) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_propagate_impl(c, in, seed, max_steps, out, hist, params, (cudaStream_t)stream);
+}
+
+extern "C" int dw_debug_philox(dw_ctx* c, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
+                               uint32_t* out_raw, float* out_u, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (n < 0) return dw_fail(c, DW_E_ARG, "dw_debug_philox: n < 0");
+  if (n == 0) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_debug_philox_impl(c, seed, base, step, block, n, out_raw, out_u, (cudaStream_t)stream);
+}
+
+extern "C" int dw_last_launch(const dw_ctx* c, int32_t* grid, int32_t* block, int32_t* smem, int64_t* n_launches) {
+  if (!c) return DW_E_ARG;
+  if (grid) *grid = c->last_grid;
+  if (block) *block = c->last_block;
+  if (smem) *smem = c->last_smem;
+  if (n_launches) *n_launches = c->n_launches;
+  return DW_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Host-buffer entry: chunks of the batch are copied to a device staging area on two alternating streams so
+// that the copy of chunk i+1 overlaps the propagation of chunk i; results are copied back per chunk and the
+// reductions are added into the host arrays at the end.
+// ---------------------------------------------------------------------------------------------------------
+namespace {
+struct StageLayout {
+  int64_t chunk;
+  size_t in_off[11], out_off[14], hist_off[4], total;
+};
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+}  // namespace
+
+extern "C" int dw_propagate_host(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps,
+                                 const dw_results* out, const dw_hists* hist, const dw_propagate_params* params) {
+  if (!c) return DW_E_ARG;
+  int rc = check_batch(c, "dw_propagate_host", in, max_steps, hist);
+  if (rc) return rc;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  const int64_t n = in->n;
+  if (n == 0) return DW_OK;
+  const int64_t chunk = std::min<int64_t>(n, 1 << 21);
+  const int64_t n_chan = hist ? hist->n_chan : 0, n_bins = hist ? hist->n_bins : 0;
+  // layout: 2 slots x (11 inputs + up to 14 outputs) + histograms
+  size_t per_slot = 25 * align256(sizeof(float) * chunk);
+  size_t hist_bytes = align256(8 * n_chan) + align256(4 * n_bins) + align256(64) + align256(8);
+  size_t need = 2 * per_slot + hist_bytes;
+  if (c->stage_bytes < need) {
+    if (c->stage) cudaFree(c->stage);
+    c->stage = nullptr; c->stage_bytes = 0;
+    DW_CUDA(c, cudaMalloc(&c->stage, need));
+    c->stage_bytes = need;
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (!c->stage_streams[i]) DW_CUDA(c, cudaStreamCreateWithFlags(&c->stage_streams[i], cudaStreamNonBlocking));
+    if (!c->stage_events[i]) DW_CUDA(c, cudaEventCreateWithFlags(&c->stage_events[i], cudaEventDisableTiming));
+  }
+  char* base = (char*)c->stage;
+  char* hbase = base + 2 * per_slot;
+  uint64_t* d_chan = (uint64_t*)hbase;
+  uint32_t* d_time = (uint32_t*)(hbase + align256(8 * n_chan));
+  uint64_t* d_fate = (uint64_t*)(hbase + align256(8 * n_chan) + align256(4 * n_bins));
+  uint64_t* d_steps = (uint64_t*)(hbase + align256(8 * n_chan) + align256(4 * n_bins) + align256(64));
+  DW_CUDA(c, cudaMemsetAsync(hbase, 0, hist_bytes, c->stage_streams[0]));
+  DW_CUDA(c, cudaEventRecord(c->stage_events[0], c->stage_streams[0]));
+  DW_CUDA(c, cudaStreamWaitEvent(c->stage_streams[1], c->stage_events[0], 0));
+  const float* src[11] = {in->px, in->py, in->pz, in->kx, in->ky, in->kz, in->ex, in->ey, in->ez, in->wavelength, in->t0};
+  void* dst_host[14] = {nullptr};
+  if (out) {
+    void* tmp[14] = {out->flags, out->channel, out->t, out->steps, out->last_tri, out->x, out->y, out->z,
+                     out->kx, out->ky, out->kz, out->ex, out->ey, out->ez};
+    memcpy(dst_host, tmp, sizeof tmp);
+  }
+  int slot = 0;
+  for (int64_t a = 0; a < n; a += chunk, slot ^= 1) {
+    const int64_t m = std::min<int64_t>(chunk, n - a);
+    cudaStream_t s = c->stage_streams[slot];
+    char* sb = base + slot * per_slot;
+    float* din[11];
+    for (int k = 0; k < 11; ++k) {
+      din[k] = (float*)(sb + k * align256(sizeof(float) * chunk));
+      DW_CUDA(c, cudaMemcpyAsync(din[k], src[k] + a, sizeof(float) * m, cudaMemcpyHostToDevice, s));
+    }
+    void* dout[14];
+    for (int k = 0; k < 14; ++k) dout[k] = dst_host[k] ? (void*)(sb + (11 + k) * align256(sizeof(float) * chunk)) : nullptr;
+    dw_photons pin{m, in->photon_id_base + (uint64_t)a, din[0], din[1], din[2], din[3], din[4], din[5], din[6], din[7], din[8], din[9], din[10]};
+    dw_results pout{(uint32_t*)dout[0], (int32_t*)dout[1], (float*)dout[2], (uint32_t*)dout[3], (int32_t*)dout[4],
+                    (float*)dout[5], (float*)dout[6], (float*)dout[7], (float*)dout[8], (float*)dout[9], (float*)dout[10],
+                    (float*)dout[11], (float*)dout[12], (float*)dout[13]};
+    dw_hists ph{n_chan, (hist && hist->chan_count) ? d_chan : nullptr, n_bins, hist ? hist->t_min : 0.f, hist ? hist->dt : 1.f,
+                (hist && hist->time_hist) ? d_time : nullptr, (hist && hist->fate_count) ? d_fate : nullptr,
+                (hist && hist->total_steps) ? d_steps : nullptr};
+    rc = dw_propagate_impl(c, &pin, seed, max_steps, &pout, hist ? &ph : nullptr, params, s);
+    if (rc) return rc;
+    for (int k = 0; k < 14; ++k)
+      if (dst_host[k]) DW_CUDA(c, cudaMemcpyAsync((char*)dst_host[k] + 4 * a, dout[k], 4 * m, cudaMemcpyDeviceToHost, s));
+  }
+  DW_CUDA(c, cudaStreamSynchronize(c->stage_streams[0]));
+  DW_CUDA(c, cudaStreamSynchronize(c->stage_streams[1]));
+  if (hist) {
+    std::vector<uint64_t> hc((size_t)n_chan), hf(8), hs(1);
+    std::vector<uint32_t> ht((size_t)n_bins);
+    if (hist->chan_count && n_chan) {
+      DW_CUDA(c, cudaMemcpy(hc.data(), d_chan, 8 * n_chan, cudaMemcpyDeviceToHost));
+      for (int64_t i = 0; i < n_chan; ++i) hist->chan_count[i] += hc[i];
+    }
+    if (hist->time_hist && n_bins) {
+      DW_CUDA(c, cudaMemcpy(ht.data(), d_time, 4 * n_bins, cudaMemcpyDeviceToHost));
+      for (int64_t i = 0; i < n_bins; ++i) hist->time_hist[i] += ht[i];
+    }
+    if (hist->fate_count) {
+      DW_CUDA(c, cudaMemcpy(hf.data(), d_fate, 64, cudaMemcpyDeviceToHost));
+      for (int i = 0; i < 8; ++i) hist->fate_count[i] += hf[i];
+    }
+    if (hist->total_steps) {
+      DW_CUDA(c, cudaMemcpy(hs.data(), d_steps, 8, cudaMemcpyDeviceToHost));
+      hist->total_steps[0] += hs[0];
+    }
+  }
+  return DW_OK;
+}

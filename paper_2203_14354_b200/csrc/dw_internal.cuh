@@ -1,0 +1,94 @@
+// dw_internal.cuh -- private declarations of libdarwinopt.so (CUDA side only; the oracle shares nothing
+// with this tree).  Public contract: include/darwinopt.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/darwinopt.h"
+
+#define DW_VERSION 100
+
+// ---------------------------------------------------------------------------------------------------------
+// Device-side views (plain structs passed by value to kernels)
+// ---------------------------------------------------------------------------------------------------------
+
+// Optical tables.  mat: [3][n_mat][nl_mat] = refractive index, absorption length, scattering length.
+// surf: [4][n_surf][nl_surf] = CUMULATIVE probabilities detect, +diffuse, +specular, +transmit (S7).
+struct DwTables {
+  const float* mat;
+  const float* surf;
+  int n_mat, nl_mat, n_surf, nl_surf;
+  float mat_l0, mat_inv_dl, surf_l0, surf_inv_dl;
+};
+
+// Binary BVH node, 64 B, read as four float4:
+//   q0 = (lo0.x, lo0.y, lo0.z, hi0.x)  q1 = (hi0.y, hi0.z, lo1.x, lo1.y)  q2 = (lo1.z, hi1.x, hi1.y, hi1.z)
+//   q3 = (as_float(ref0), as_float(ref1), -, -)
+// ref >= 0: internal node index; ref < 0: leaf, ~ref = (first_slot << 3) | (count - 1); DW_REF_NONE = empty.
+#define DW_REF_NONE 0x7fffffff
+
+// Triangle record in leaf order, 48 B, read as three float4 (Moeller-Trumbore form):
+//   a = (v0.x, v0.y, v0.z, e1.x)  b = (e1.y, e1.z, e2.x, e2.y)
+//   c = (e2.z, as_float(caller id), as_float(code), as_float(channel))
+// code = inner | outer << 8 | surface << 16 (0xFF = no surface -> Fresnel)
+struct DwBvh {
+  const float4* nodes;  // [n_nodes][4]
+  const float4* tris;   // [n_tri][3]
+  int n_nodes;
+  int n_tri;
+  float eps_len;        // length tolerance tied to the fp32 spacing of the scene coordinates
+};
+
+struct dw_ctx {
+  int device = 0;
+  int sm_count = 0;
+  std::string err;
+  // tables
+  float* d_mat = nullptr;
+  float* d_surf = nullptr;
+  DwTables tables{};
+  bool have_mat = false, have_surf = false;
+  // geometry, caller order
+  int64_t n_vert = 0, n_tri = 0;
+  float* d_xyz = nullptr;
+  int32_t* d_idx = nullptr;
+  uint32_t* d_code = nullptr;
+  int32_t* d_chan = nullptr;
+  bool have_geom = false;
+  // BVH
+  float4* d_nodes = nullptr;
+  float4* d_tris = nullptr;
+  DwBvh bvh{};
+  bool built = false;
+  // launch record
+  int last_grid = 0, last_block = 0, last_smem = 0;
+  int64_t n_launches = 0;
+  // staging for dw_propagate_host
+  void* stage = nullptr;
+  size_t stage_bytes = 0;
+  cudaStream_t stage_streams[2] = {nullptr, nullptr};
+  cudaEvent_t stage_events[2] = {nullptr, nullptr};
+};
+
+// error helpers --------------------------------------------------------------------------------------------
+int dw_fail(dw_ctx* ctx, int code, const char* fmt, ...);
+#define DW_CUDA(ctx, call)                                                                       \
+  do {                                                                                           \
+    cudaError_t e__ = (call);                                                                    \
+    if (e__ != cudaSuccess)                                                                      \
+      return dw_fail((ctx), DW_E_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), \
+                     __FILE__, __LINE__);                                                        \
+  } while (0)
+
+// implemented in dw_bvh.cu
+int dw_bvh_build_impl(dw_ctx* ctx, const dw_build_params* params, dw_build_stats* stats, cudaStream_t stream);
+// implemented in dw_kernels.cu
+int dw_first_hit_impl(dw_ctx* ctx, int64_t n, const float* ox, const float* oy, const float* oz, const float* dx,
+                      const float* dy, const float* dz, const int32_t* exclude, int32_t* tri, float* dist,
+                      cudaStream_t stream);
+int dw_propagate_impl(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                      const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream);
+int dw_debug_philox_impl(dw_ctx* ctx, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
+                         uint32_t* out_raw, float* out_u, cudaStream_t stream);

