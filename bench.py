@@ -177,6 +177,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
+    ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
+    ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
+    ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
+    ap.add_argument("--blocks-per-sm", type=int, default=0, help="cap on resident blocks per SM (0 = occupancy limit)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -204,7 +208,8 @@ def main():
     flags = dw.PROP_UNBOUNDED_QUERY if args.literal else 0
 
     def step():
-        ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream)
+        ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream, th_phys=args.th_phys,
+                      th_leaf=args.th_leaf, block_threads=args.block, blocks_per_sm=args.blocks_per_sm)
         if world > 1:
             dwdist.merge_hists(hist)        # the only exchange: tens of kB of integer histograms
 

@@ -163,7 +163,9 @@ typedef struct dw_propagate_params {
   uint32_t flags;          /* DW_PROP_* */
   int32_t block_threads;   /* 0 = default */
   int32_t blocks_per_sm;   /* 0 = default */
-  int32_t reserved[5];
+  int32_t th_phys;         /* phase scheduling: run the physics phase once this many lanes of a warp wait for it; 0 = default */
+  int32_t th_leaf;         /* phase scheduling: run the triangle phase once this many lanes wait for it; 0 = default */
+  int32_t reserved[3];
 } dw_propagate_params;
 enum {
   /* Follow the oracle literally: every query is unbounded and the medium comes from the hit triangle (S2).

@@ -53,7 +53,8 @@ class Hists(C.Structure):
 
 
 class PropagateParams(C.Structure):
-    _fields_ = [("flags", u32), ("block_threads", i32), ("blocks_per_sm", i32), ("reserved", i32 * 5)]
+    _fields_ = [("flags", u32), ("block_threads", i32), ("blocks_per_sm", i32), ("th_phys", i32),
+                ("th_leaf", i32), ("reserved", i32 * 3)]
 
 
 _lib = None
@@ -195,8 +196,9 @@ class Context:
 
     def propagate(self, ph: "DevicePhotons", seed: int, max_steps: int, out: "DeviceResults | None" = None,
                   hist: "DeviceHists | None" = None, flags: int = 0, block_threads: int = 0, blocks_per_sm: int = 0,
-                  stream=None):
-        pp = PropagateParams(flags=flags, block_threads=block_threads, blocks_per_sm=blocks_per_sm)
+                  th_phys: int = 0, th_leaf: int = 0, stream=None):
+        pp = PropagateParams(flags=flags, block_threads=block_threads, blocks_per_sm=blocks_per_sm, th_phys=th_phys,
+                             th_leaf=th_leaf)
         self._check(self.L.dw_propagate(self.h, C.byref(ph.c), seed, max_steps, C.byref(out.c) if out else None,
                                         C.byref(hist.c) if hist else None, C.byref(pp), _stream_ptr(stream)))
 

@@ -62,97 +62,104 @@ __device__ __forceinline__ float table_at(const float* __restrict__ tab, int row
 }
 
 // ------------------------------------------------------------------------------------------------ first hit (S1)
-struct Hit {
-  float t;     // distance, +inf = none
-  int slot;    // index into the leaf-ordered triangle array
-  int id;      // caller triangle id
+// The query is written as a resumable state machine so that the propagation kernel can interleave the
+// traversal steps of all lanes of a warp; dw_first_hit runs it to completion.
+struct Ray {
+  V3 o, d;     // origin, unit direction
+  V3 inv, oi;  // 1/d (zero components pushed to +-1e30) and o * inv
 };
+__device__ __forceinline__ void ray_setup(Ray& r, V3 o, V3 d) {
+  const float tiny = 1e-30f;   // zero components become +-tiny so that 0 * inf never appears
+  r.o = o; r.d = d;
+  r.inv = mk(1.0f / (fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), 1.0f / (fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
+             1.0f / (fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
+  r.oi = mk(o.x * r.inv.x, o.y * r.inv.y, o.z * r.inv.z);
+}
 
-// Nearest triangle along o + t d with 0 < t < tmax, excluding caller id `exclude`; ties -> lowest caller id.
-// medium >= 0: only triangles whose near side (the side the ray comes from) is `medium` count
-// (DESIGN.md "medium culling"); medium < 0: every triangle counts (the definition S1).
-// sstack: this thread's column of the shared-memory stack, entries `sstride` ints apart.
-__device__ __forceinline__ Hit trace(const DwBvh& bvh, V3 o, V3 d, float tmax, int exclude, int medium, int* sstack,
-                                     int sstride) {
-  Hit best;
-  best.t = tmax; best.slot = -1; best.id = 0x7fffffff;
-  int lstack[kStackLocal];
-  // inverse direction with zero components pushed to +-tiny so that 0 * inf never appears
-  const float tiny = 1e-30f;
-  V3 inv = mk(1.0f / (fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), 1.0f / (fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
-              1.0f / (fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
-  V3 oi = mk(o.x * inv.x, o.y * inv.y, o.z * inv.z);
-  int sp = 0;
-  int node = 0;
-  const float4* __restrict__ nodes = bvh.nodes;
-  const float4* __restrict__ tris = bvh.tris;
-  while (true) {
-    if (node >= 0) {
-      if (node == DW_REF_NONE) goto pop;
-      {
-        const float4* p = nodes + 4 * (size_t)node;
-        float4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2), q3 = __ldg(p + 3);
-        // child 0: lo (q0.x q0.y q0.z) hi (q0.w q1.x q1.y); child 1: lo (q1.z q1.w q2.x) hi (q2.y q2.z q2.w)
-        float ax = fmaf(q0.x, inv.x, -oi.x), bx = fmaf(q0.w, inv.x, -oi.x);
-        float ay = fmaf(q0.y, inv.y, -oi.y), by = fmaf(q1.x, inv.y, -oi.y);
-        float az = fmaf(q0.z, inv.z, -oi.z), bz = fmaf(q1.y, inv.z, -oi.z);
-        float n0 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
-        float f0 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), best.t));
-        ax = fmaf(q1.z, inv.x, -oi.x); bx = fmaf(q2.y, inv.x, -oi.x);
-        ay = fmaf(q1.w, inv.y, -oi.y); by = fmaf(q2.z, inv.y, -oi.y);
-        az = fmaf(q2.x, inv.z, -oi.z); bz = fmaf(q2.w, inv.z, -oi.z);
-        float n1 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
-        float f1 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), best.t));
-        int r0 = __float_as_int(q3.x), r1 = __float_as_int(q3.y);
-        bool h0 = (n0 <= fmaf(f0, kBoxSlack, bvh.eps_len)) && (r0 != DW_REF_NONE);
-        bool h1 = (n1 <= fmaf(f1, kBoxSlack, bvh.eps_len)) && (r1 != DW_REF_NONE);
-        if (h0 && h1) {
-          int nearr = r0, farr = r1;
-          if (n1 < n0) { nearr = r1; farr = r0; }
-          if (sp < kStackShared) sstack[sp * sstride] = farr; else lstack[sp - kStackShared] = farr;
-          ++sp;
-          node = nearr;
-          continue;
-        }
-        if (h0) { node = r0; continue; }
-        if (h1) { node = r1; continue; }
-        goto pop;
-      }
-    } else {
-      // leaf: ~node = (first << 3) | (count - 1)
-      int code = ~node;
-      int first = code >> 3, cnt = (code & 7) + 1;
-      for (int i = 0; i < cnt; ++i) {
-        const float4* p = tris + 3 * (size_t)(first + i);
-        float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
-        V3 e1 = mk(a.w, b.x, b.y), e2 = mk(b.z, b.w, c.x);
-        V3 pv = cross(d, e2);
-        float det = dot(e1, pv);
-        if (fabsf(det) < 1e-30f) continue;
-        float idet = 1.0f / det;
-        V3 tv = mk(o.x - a.x, o.y - a.y, o.z - a.z);
-        float u = dot(tv, pv) * idet;
-        V3 qv = cross(tv, e1);
-        float v = dot(d, qv) * idet;
-        float t = dot(e2, qv) * idet;
-        int id = __float_as_int(c.y);
-        bool ok = (u >= -kEdgeSlack) && (v >= -kEdgeSlack) && (u + v <= 1.0f + kEdgeSlack) && (t > 0.f) &&
-                  (t < best.t || (t == best.t && id < best.id)) && (id != exclude);
-        if (ok && medium >= 0) {
-          uint32_t cw = __float_as_uint(c.z);
-          int near_side = (det > 0.f) ? (int)((cw >> 8) & 0xFF) : (int)(cw & 0xFF);   // det > 0: ray comes from the outer side
-          ok = (near_side == medium);
-        }
-        if (ok) { best.t = t; best.slot = first + i; best.id = id; }
-      }
-    }
-  pop:
-    if (sp == 0) break;
-    --sp;
-    node = (sp < kStackShared) ? sstack[sp * sstride] : lstack[sp - kStackShared];
+constexpr int kInLeaf = -1;   // TraceState::node: triangles [tri_cur, tri_end) are pending
+constexpr int kDone = -2;     // TraceState::node: traversal finished
+struct TraceState {
+  int node;                   // >= 0: internal node to visit next
+  int sp;                     // stack depth
+  int tri_cur, tri_end;       // pending triangle slots of the current leaf
+  float best_t;               // nearest accepted distance so far (starts at t_max)
+  int best_slot, best_id;     // leaf-order slot and caller id of the nearest triangle (-1 / INT_MAX: none)
+};
+__device__ __forceinline__ void ts_begin(TraceState& s, float tmax) {
+  s.node = 0; s.sp = 0; s.tri_cur = 0; s.tri_end = 0; s.best_t = tmax; s.best_slot = -1; s.best_id = 0x7fffffff;
+}
+// Continue with child reference `ref` (>= 0 internal, < 0 leaf) or, for DW_REF_NONE, with the stack top.
+__device__ __forceinline__ void ts_goto(TraceState& s, int ref, const int* sstack, int sstride, const int* lstack) {
+  if (ref == DW_REF_NONE) {
+    if (s.sp == 0) { s.node = kDone; return; }
+    --s.sp;
+    ref = (s.sp < kStackShared) ? sstack[s.sp * sstride] : lstack[s.sp - kStackShared];
   }
-  if (best.slot < 0) best.t = INFINITY;
-  return best;
+  if (ref >= 0) { s.node = ref; return; }
+  int code = ~ref;                       // leaf: (first << 3) | (count - 1)
+  s.tri_cur = code >> 3;
+  s.tri_end = (code >> 3) + (code & 7) + 1;
+  s.node = kInLeaf;
+}
+
+// One internal node: slab-test both children against [0, best_t], descend into the nearer hit, push the other.
+__device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
+  const float4* p = bvh.nodes + 4 * (size_t)s.node;
+  float4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2), q3 = __ldg(p + 3);
+  // child 0: lo (q0.x q0.y q0.z) hi (q0.w q1.x q1.y); child 1: lo (q1.z q1.w q2.x) hi (q2.y q2.z q2.w)
+  float ax = fmaf(q0.x, r.inv.x, -r.oi.x), bx = fmaf(q0.w, r.inv.x, -r.oi.x);
+  float ay = fmaf(q0.y, r.inv.y, -r.oi.y), by = fmaf(q1.x, r.inv.y, -r.oi.y);
+  float az = fmaf(q0.z, r.inv.z, -r.oi.z), bz = fmaf(q1.y, r.inv.z, -r.oi.z);
+  float n0 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
+  float f0 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), s.best_t));
+  ax = fmaf(q1.z, r.inv.x, -r.oi.x); bx = fmaf(q2.y, r.inv.x, -r.oi.x);
+  ay = fmaf(q1.w, r.inv.y, -r.oi.y); by = fmaf(q2.z, r.inv.y, -r.oi.y);
+  az = fmaf(q2.x, r.inv.z, -r.oi.z); bz = fmaf(q2.w, r.inv.z, -r.oi.z);
+  float n1 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
+  float f1 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), s.best_t));
+  int r0 = __float_as_int(q3.x), r1 = __float_as_int(q3.y);
+  bool h0 = (n0 <= fmaf(f0, kBoxSlack, bvh.eps_len)) && (r0 != DW_REF_NONE);
+  bool h1 = (n1 <= fmaf(f1, kBoxSlack, bvh.eps_len)) && (r1 != DW_REF_NONE);
+  int next = DW_REF_NONE;
+  if (h0 && h1) {
+    int farr = r1;
+    next = r0;
+    if (n1 < n0) { next = r1; farr = r0; }
+    if (s.sp < kStackShared) sstack[s.sp * sstride] = farr; else lstack[s.sp - kStackShared] = farr;
+    ++s.sp;
+  } else if (h0) next = r0;
+  else if (h1) next = r1;
+  ts_goto(s, next, sstack, sstride, lstack);
+}
+
+// One triangle of the current leaf (Moeller-Trumbore on the pre-packed record).  exclude: caller id to ignore.
+// medium >= 0: only triangles whose near side (the side the ray comes from) is `medium` count (DESIGN.md
+// "medium culling"); medium < 0: every triangle counts (the definition S1).  Ties -> lowest caller id.
+__device__ __forceinline__ void step_triangle(const DwBvh& bvh, const Ray& r, TraceState& s, int exclude, int medium,
+                                              const int* sstack, int sstride, const int* lstack) {
+  const float4* p = bvh.tris + 3 * (size_t)s.tri_cur;
+  float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+  V3 e1 = mk(a.w, b.x, b.y), e2 = mk(b.z, b.w, c.x);
+  V3 pv = cross(r.d, e2);
+  float det = dot(e1, pv);
+  if (fabsf(det) >= 1e-30f) {
+    float idet = 1.0f / det;
+    V3 tv = mk(r.o.x - a.x, r.o.y - a.y, r.o.z - a.z);
+    float u = dot(tv, pv) * idet;
+    V3 qv = cross(tv, e1);
+    float v = dot(r.d, qv) * idet;
+    float t = dot(e2, qv) * idet;
+    int id = __float_as_int(c.y);
+    bool ok = (u >= -kEdgeSlack) && (v >= -kEdgeSlack) && (u + v <= 1.0f + kEdgeSlack) && (t > 0.f) &&
+              (t < s.best_t || (t == s.best_t && id < s.best_id)) && (id != exclude);
+    if (ok && medium >= 0) {
+      uint32_t cw = __float_as_uint(c.z);
+      int near_side = (det > 0.f) ? (int)((cw >> 8) & 0xFF) : (int)(cw & 0xFF);   // det > 0: the ray comes from the outer side
+      ok = (near_side == medium);
+    }
+    if (ok) { s.best_t = t; s.best_slot = s.tri_cur; s.best_id = id; }
+  }
+  if (++s.tri_cur == s.tri_end) ts_goto(s, DW_REF_NONE, sstack, sstride, lstack);
 }
 
 __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, const float* __restrict__ ox,
@@ -161,12 +168,21 @@ __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, co
                                                         const float* __restrict__ dz, const int32_t* __restrict__ exclude,
                                                         int32_t* __restrict__ tri, float* __restrict__ dist) {
   extern __shared__ int s_stack[];
+  int lstack[kStackLocal];
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
-  Hit h = trace(bvh, mk(ox[i], oy[i], oz[i]), mk(dx[i], dy[i], dz[i]), INFINITY, exclude ? exclude[i] : -1, -1,
-                s_stack + threadIdx.x, blockDim.x);
-  tri[i] = h.slot >= 0 ? h.id : -1;
-  dist[i] = h.t;
+  Ray r;
+  ray_setup(r, mk(ox[i], oy[i], oz[i]), mk(dx[i], dy[i], dz[i]));
+  TraceState s;
+  ts_begin(s, INFINITY);
+  const int ex = exclude ? exclude[i] : -1;
+  int* my = s_stack + threadIdx.x;
+  while (s.node != kDone) {
+    if (s.node >= 0) step_internal(bvh, r, s, my, blockDim.x, lstack);
+    else step_triangle(bvh, r, s, ex, -1, my, blockDim.x, lstack);
+  }
+  tri[i] = s.best_slot >= 0 ? s.best_id : -1;
+  dist[i] = s.best_slot >= 0 ? s.best_t : INFINITY;
 }
 
 // ------------------------------------------------------------------------------------------------ physics
@@ -253,10 +269,20 @@ struct PropArgs {
   uint64_t seed;
   int32_t max_steps;
   uint32_t flags;
+  int32_t th_phys, th_leaf;         // phase-scheduling thresholds (lanes)
   unsigned long long* queue_head;   // device counter, zeroed before launch
 };
 
 constexpr int kChunk = 8;   // photons claimed per lane per queue transaction (x32 per warp)
+
+// Lane states of the persistent loop.  A warp repeatedly picks ONE of three phases and runs it for the lanes
+// that are in it:
+//   I  internal-node step   for lanes with ts.node >= 0
+//   L  triangle step        for lanes with ts.node == kInLeaf
+//   P  physics              for lanes whose query is finished (or that hold no photon: refill first)
+// so that the expensive code runs with many lanes enabled although the traversals of the 32 rays of a warp
+// have very different lengths (short bounded scatter segments next to long surface-to-surface rays).
+enum : int { LANE_IDLE = 0, LANE_PHYS = 1, LANE_TRACE = 2 };
 
 __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_stack[];
@@ -267,88 +293,96 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
   __syncthreads();
   int* my_stack = s_stack + threadIdx.x;
   const int sstride = blockDim.x;
+  int lstack[kStackLocal];
   const int lane = threadIdx.x & 31;
   const int64_t n = A.in.n;
   const bool literal = (A.flags & DW_PROP_UNBOUNDED_QUERY) != 0;
 
-  // warp-private range of photon indices [w_next, w_end)
-  int64_t w_next = 0, w_end = 0;
-  bool active = false;
+  int64_t w_next = 0, w_end = 0;     // warp-private range of photon indices; w_end < 0: queue exhausted
+  int lstate = LANE_IDLE;
+  bool fresh = false;                // LANE_PHYS without a finished query (photon just loaded)
   // photon state
   int64_t pi = 0;
-  V3 x = mk(0, 0, 0), k = mk(0, 0, 1), e = mk(1, 0, 0);
+  Ray ray;                           // ray.o = position x, ray.d = direction k
+  ray.o = mk(0, 0, 0); ray.d = mk(0, 0, 1); ray.inv = mk(0, 0, 0); ray.oi = mk(0, 0, 0);
+  V3 e = mk(1, 0, 0);
   float lambda = 0.f, t = 0.f;
   int medium = -1, last_tri = -1;
   uint32_t step = 0, hist = 0;
+  // carried from the set-up of a query to its evaluation
+  float dbulk = INFINITY, n1 = 1.f;
+  bool absorb_first = false;
+  TraceState ts;
+  ts_begin(ts, 0.f);
+  ts.node = kDone;
 
-  while (true) {
-    // ---------------------------------------------------------------- a2: refill finished lanes
-    unsigned idle = __ballot_sync(0xffffffffu, !active);
-    if (idle) {
+  for (;;) {
+    const bool exhausted = w_end < 0;
+    const bool tracing = lstate == LANE_TRACE;
+    const int nI = __popc(__ballot_sync(0xffffffffu, tracing && ts.node >= 0));
+    const int nL = __popc(__ballot_sync(0xffffffffu, tracing && ts.node == kInLeaf));
+    const int nP = __popc(__ballot_sync(0xffffffffu, lstate == LANE_PHYS || (lstate == LANE_IDLE && !exhausted)));
+    if (nI + nL + nP == 0) break;
+
+    if (nI + nL > 0 && nP < A.th_phys) {
+      // ------------------------------------------------------------ a4: one traversal step (phase I or L)
+      if (nI > 0 && nL < A.th_leaf) {
+        if (tracing && ts.node >= 0) step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
+      } else {
+        if (tracing && ts.node == kInLeaf)
+          step_triangle(A.bvh, ray, ts, last_tri, (!literal) ? medium : -1, my_stack, sstride, lstack);
+      }
+      if (tracing && ts.node == kDone) { lstate = LANE_PHYS; fresh = false; }
+      continue;
+    }
+
+    // -------------------------------------------------------------- phase P
+    // a2: refill lanes that hold no photon from the warp's private id range
+    unsigned idle = __ballot_sync(0xffffffffu, lstate == LANE_IDLE);
+    if (idle && !exhausted) {
       int need = __popc(idle);
-      if (w_end - w_next < need && w_end >= 0) {           // claim a new chunk for the warp (one atomic per warp)
-        // keep what is left of the old chunk only if it is empty (ranges are consumed in order, so the remainder
-        // is always used up before a new claim is needed); w_end < 0 marks "queue exhausted"
-        if (w_next == w_end) {
-          unsigned long long base = 0;
-          if (lane == 0) base = atomicAdd(A.queue_head, (unsigned long long)(32 * kChunk));
-          base = __shfl_sync(0xffffffffu, base, 0);
-          w_next = (int64_t)base;
-          w_end = (int64_t)base + 32 * kChunk;
-          if (w_next >= n) { w_next = 0; w_end = -1; }
-          else if (w_end > n) w_end = n;
-        }
+      if (w_next == w_end) {                              // claim a new chunk (one atomic per warp)
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(A.queue_head, (unsigned long long)(32 * kChunk));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        w_next = (int64_t)base;
+        w_end = (int64_t)base + 32 * kChunk;
+        if (w_next >= n) { w_next = 0; w_end = -1; }
+        else if (w_end > n) w_end = n;
       }
       if (w_end > w_next) {
         int rank = __popc(idle & ((1u << lane) - 1u));
         int avail = (int)min((int64_t)need, w_end - w_next);
-        if (!active && rank < avail) {
+        if (lstate == LANE_IDLE && rank < avail) {
           pi = w_next + rank;
-          x = mk(A.in.px[pi], A.in.py[pi], A.in.pz[pi]);
-          k = mk(A.in.kx[pi], A.in.ky[pi], A.in.kz[pi]);
+          ray.o = mk(A.in.px[pi], A.in.py[pi], A.in.pz[pi]);
+          ray.d = mk(A.in.kx[pi], A.in.ky[pi], A.in.kz[pi]);
           e = mk(A.in.ex[pi], A.in.ey[pi], A.in.ez[pi]);
           lambda = A.in.wavelength[pi];
           t = A.in.t0[pi];
           medium = -1; last_tri = -1; step = 0; hist = 0;
-          active = true;
+          lstate = LANE_PHYS; fresh = true;
         }
         w_next += avail;
       }
-      if (__ballot_sync(0xffffffffu, active) == 0u) {
-        if (w_end < 0) break;        // nothing running and the queue is exhausted
-        continue;                    // chunk boundary: claim again
-      }
     }
 
-    // ---------------------------------------------------------------- one step of the loop S1..S11
     uint32_t fate = 0xFFu;           // 0xFF = still running
     int channel = -1;
-    if (active) {
+    if (lstate == LANE_PHYS) {
       const uint64_t pid = A.in.photon_id_base + (uint64_t)pi;
-      if ((int32_t)step >= A.max_steps) {
-        fate = DW_FATE_TRUNCATED;                                     // S10
-      } else if (!(isfinite(x.x + x.y + x.z) && isfinite(k.x + k.y + k.z) && isfinite(e.x + e.y + e.z) && isfinite(t))) {
-        fate = DW_FATE_NAN_ABORT;                                     // S11
-      } else {
+      V3 x = ray.o, k = ray.d;
+      if (!fresh) {
+        // ---------------------------------------------------------- evaluate the finished query: S2..S9
         float4 r0 = draw4(A.seed, pid, step, 0u);                     // (u_a, u_s, u_surface, u_fresnel)
-        float n1 = 1.f, dbulk = INFINITY;
-        bool absorb_first = false;
-        bool bounded = (!literal) && (medium >= 0);
-        if (bounded) {                                                // medium known: S3/S4 draws before the query
-          n1 = table_at(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-          float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-          float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-          float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
-          absorb_first = da < ds;
-          dbulk = fminf(da, ds);
-        }
-        Hit h = trace(A.bvh, x, k, bounded ? dbulk + A.bvh.eps_len : INFINITY, last_tri, bounded ? medium : -1, my_stack, sstride);
+        const bool bounded = (!literal) && (medium >= 0);
+        const bool have_hit = ts.best_slot >= 0;
         float4 tc = make_float4(0, 0, 0, 0), ta = tc, tb = tc;
         int m1 = medium, m2 = medium;
         V3 ng = mk(0, 0, 1);
         bool toward_outer = false;
-        if (h.slot >= 0) {                                            // S2 sides
-          const float4* p = A.bvh.tris + 3 * (size_t)h.slot;
+        if (have_hit) {                                               // S2 sides
+          const float4* p = A.bvh.tris + 3 * (size_t)ts.best_slot;
           ta = __ldg(p); tb = __ldg(p + 1); tc = __ldg(p + 2);
           ng = unit(cross(mk(ta.w, tb.x, tb.y), mk(tb.z, tb.w, tc.x)));
           uint32_t cw = __float_as_uint(tc.z);
@@ -358,7 +392,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
           m2 = toward_outer ? mo : mi;
         }
         if (!bounded) {
-          if (h.slot < 0) {
+          if (!have_hit) {
             fate = DW_FATE_ESCAPED;                                   // G3: ray leaves the world
           } else {
             if (medium >= 0 && medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
@@ -372,7 +406,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
           }
         }
         if (fate == 0xFFu) {
-          bool surface_event = (h.slot >= 0) && (bounded ? true : !(dbulk < h.t));
+          const bool surface_event = have_hit && (bounded ? true : !(dbulk < ts.best_t));
           if (!surface_event) {
             if (!(dbulk < INFINITY)) {
               fate = DW_FATE_ESCAPED;                                 // bounded query, no bulk process, nothing hit
@@ -388,9 +422,9 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
               }
             }
           } else {                                                    // S4 third branch, S5
-            x = fma3(h.t, k, x);
-            t = fmaf(h.t * n1, kInvC, t);
-            last_tri = h.id;
+            x = fma3(ts.best_t, k, x);
+            t = fmaf(ts.best_t * n1, kInvC, t);
+            last_tri = ts.best_id;
             if (medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
             V3 nh = toward_outer ? mk(-ng.x, -ng.y, -ng.z) : ng;
             uint32_t cw = __float_as_uint(tc.z);
@@ -418,9 +452,34 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
               if (crossed) medium = m2;
             }
           }
-          ++step;                                                     // S9 (the terminating iteration counts, S13)
+        }
+        ++step;                                                       // S9 (every executed iteration counts, also the last: S13)
+      }
+      if (fate == 0xFFu) {
+        // ---------------------------------------------------------- set up the query of the next iteration: S1 (+S3/S4 draws)
+        if ((int32_t)step >= A.max_steps) {
+          fate = DW_FATE_TRUNCATED;                                   // S10
+        } else if (!(isfinite(x.x + x.y + x.z) && isfinite(k.x + k.y + k.z) && isfinite(e.x + e.y + e.z) && isfinite(t))) {
+          fate = DW_FATE_NAN_ABORT;                                   // S11
+        } else {
+          float tmax = INFINITY;
+          if ((!literal) && medium >= 0) {                            // medium known: S3/S4 draws before the query
+            float4 r0 = draw4(A.seed, pid, step, 0u);
+            n1 = table_at(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
+            absorb_first = da < ds;
+            dbulk = fminf(da, ds);
+            tmax = dbulk + A.bvh.eps_len;
+          }
+          ray_setup(ray, x, k);
+          ts_begin(ts, tmax);
+          lstate = LANE_TRACE;
+          fresh = false;
         }
       }
+      ray.o = x; ray.d = k;
     }
 
     // ---------------------------------------------------------------- a10: outputs and reductions
@@ -430,14 +489,14 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
       if (A.out.t) A.out.t[pi] = t;
       if (A.out.steps) A.out.steps[pi] = step;
       if (A.out.last_tri) A.out.last_tri[pi] = last_tri;
-      if (A.out.x) A.out.x[pi] = x.x;
-      if (A.out.y) A.out.y[pi] = x.y;
-      if (A.out.z) A.out.z[pi] = x.z;
-      if (A.out.kx) { A.out.kx[pi] = k.x; A.out.ky[pi] = k.y; A.out.kz[pi] = k.z; }
+      if (A.out.x) A.out.x[pi] = ray.o.x;
+      if (A.out.y) A.out.y[pi] = ray.o.y;
+      if (A.out.z) A.out.z[pi] = ray.o.z;
+      if (A.out.kx) { A.out.kx[pi] = ray.d.x; A.out.ky[pi] = ray.d.y; A.out.kz[pi] = ray.d.z; }
       if (A.out.ex) { A.out.ex[pi] = e.x; A.out.ey[pi] = e.y; A.out.ez[pi] = e.z; }
       atomicAdd(&s_fate[fate & 7u], 1u);
       atomicAdd(&s_steps, (unsigned long long)step);
-      active = false;
+      lstate = LANE_IDLE;
     }
     // detected photons: per-channel counts and arrival-time histogram, aggregated over equal keys in the warp
     unsigned det = __ballot_sync(0xffffffffu, fate == DW_FATE_DETECTED);
@@ -491,6 +550,8 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
   if (out) A.out = *out;
   if (hist) A.hist = *hist;
   A.seed = seed; A.max_steps = max_steps; A.flags = params ? params->flags : 0u;
+  A.th_phys = (params && params->th_phys > 0) ? params->th_phys : 12;
+  A.th_leaf = (params && params->th_leaf > 0) ? params->th_leaf : 12;
   int B = (params && params->block_threads) ? params->block_threads : 128;
   if (B < 32 || B > 128 || (B & 31)) return dw_fail(c, DW_E_ARG, "dw_propagate: block_threads must be 32, 64, 96 or 128");
   size_t smem = sizeof(int) * kStackShared * B;
@@ -501,7 +562,7 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
   int64_t warps_needed = (in->n + 31) / 32;
   int64_t blocks_needed = (warps_needed + (B / 32) - 1) / (B / 32);
   int grid = (int)std::min<int64_t>((int64_t)c->sm_count * per_sm, std::max<int64_t>(blocks_needed, 1));
-  // queue head lives in a small device allocation owned by the context-less stream-ordered pool
+  // queue head: a stream-ordered 8-byte allocation, so that launches on different streams never share one
   unsigned long long* head = nullptr;
   DW_CUDA(c, cudaMallocAsync((void**)&head, sizeof(unsigned long long), stream));
   DW_CUDA(c, cudaMemsetAsync(head, 0, sizeof(unsigned long long), stream));

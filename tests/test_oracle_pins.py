@@ -469,7 +469,7 @@ def test_seam_between_two_reflecting_planes_is_not_lost():
 
 
 def _random_detector_sphere(f_target, rho, subdiv=4, seed=0):
-    g = synth.sphere_detector(1000.0, subdiv, material=2, surface=0)   # material 2: no bulk process
+    g = synth.sphere_detector(1000.0, subdiv, material=1, surface=0)   # inner 1 / outer 2: no bulk process in either
     rng = np.random.default_rng(seed)
     V = g.xyz.astype(np.float64)
     area = 0.5 * np.linalg.norm(np.cross(V[g.idx[:, 1]] - V[g.idx[:, 0]], V[g.idx[:, 2]] - V[g.idx[:, 0]]), axis=1)
