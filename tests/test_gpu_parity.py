@@ -504,9 +504,30 @@ def test_integrating_sphere_on_device():
     N = 2_000_000
     r = gpu_run(ctx, synth.photons_point(31, N), 31, 5000, fields=("flags", "steps", "t"))
     fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
-    assert fc["detected"] + fc["surface_absorbed"] == N
+    # P9 conservation is exact; the only other fate allowed is ESCAPED through an fp32 seam, within the G3 budget
+    # (G3 / SURVEY.md 8(c) G3: <= 1e-6 N on the GPU).  Measured on B200: 1 of 2e6 (profiles/r01_leaks.md).
+    assert sum(fc.values()) == N
+    assert fc["bulk_absorbed"] == 0 and fc["truncated"] == 0 and fc["nan_abort"] == 0
+    assert fc["escaped"] <= max(1, int(1e-6 * N)), f"{fc['escaped']} photons leaked out of a closed sphere"
+    assert fc["detected"] + fc["surface_absorbed"] + fc["escaped"] == N
     p = f / (1 - rho * (1 - f))
     assert abs(fc["detected"] / N - p) < 4 * math.sqrt(p * (1 - p) / N) + 3e-3   # faceting bias, see the oracle pin
     ref = orc.Oracle(g, op, bvh=True).propagate(synth.photons_point(32, 400_000), 32, 5000, full=False)
     pu.assert_binomial_agrees(fc["detected"], N, int(ref["fate_count"][0]), 400_000, 4.0, "integrating sphere")
     assert abs(r["steps"].mean() - ref["steps"].mean()) < 4 * math.sqrt(r["steps"].var() / N + ref["steps"].var() / 4e5)
+
+
+@pytest.mark.xfail(strict=True, reason="KNOWN DEFECT (profiles/r01_leaks.md): DW_PROP_UNBOUNDED_QUERY leaks 45 of 2e6 photons "
+                                       "(2.25e-5 N) out of a closed Lambertian sphere, 22x the G3 budget of 1e-6 N: without "
+                                       "medium culling a reflected photon whose fp32 position fell behind the neighbouring "
+                                       "facet hits that facet from outside (H_MEDIUM_MISMATCH) and is reflected outwards")
+def test_literal_mode_leak_budget_on_closed_sphere():
+    """G3 held to the same number in the diagnostic literal mode.  Strict xfail: it fails the suite the day it passes,
+    so that the defect note is removed together with the defect."""
+    g, op, f = _random_detector_sphere(0.1, 0.95, subdiv=5)
+    ctx = dw.make_context(g, op)
+    N = 2_000_000
+    r = gpu_run(ctx, synth.photons_point(31, N), 31, 5000, fields=("flags",), flags=dw.PROP_UNBOUNDED_QUERY)
+    fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
+    assert sum(fc.values()) == N
+    assert fc["escaped"] <= max(1, int(1e-6 * N)), f"{fc['escaped']} photons leaked"
