@@ -177,6 +177,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
+    ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
@@ -205,7 +206,7 @@ def main():
     out = dw.DeviceResults(n, ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), dev)   # 32 B / photon
     hist = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0, dev)
     stream = torch.cuda.current_stream()
-    flags = dw.PROP_UNBOUNDED_QUERY if args.literal else 0
+    flags = (dw.PROP_UNBOUNDED_QUERY if args.literal else 0) | (dw.PROP_LEGACY_SCHEDULER if args.legacy else 0)
 
     def step():
         ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream, th_phys=args.th_phys,
@@ -269,7 +270,7 @@ def main():
     achieved_lane = steps_per_launch * ALG_LANE_INSTR_PER_STEP / (kernel_ms * 1e-3)
     alg_bytes = steps_per_launch * ALG_BYTES_PER_STEP + n * ALG_STATE_BYTES_PER_PHOTON
     roofline = dict(bound="alu", achieved=achieved_lane / 1e12, peak=peak_lane / 1e12, unit="Tlane-instr/s",
-                    frac=achieved_lane / peak_lane, traffic=None, kernel="propagate_kernel", kernel_ms=kernel_ms,
+                    frac=achieved_lane / peak_lane, traffic=None, kernel="propagate_kernel" if args.legacy else "propagate_pool_kernel", kernel_ms=kernel_ms,
                     algorithmic_lane_instr_per_photon_step=ALG_LANE_INSTR_PER_STEP,
                     algorithmic_bytes_per_launch=alg_bytes,
                     memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
@@ -290,7 +291,8 @@ def main():
                 data="synthetic",
                 config=dict(workload=c.name, photons_per_step_per_gpu=n, triangles=c.geometry.n_tri, max_steps=c.max_steps,
                             seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
-                            mode="literal" if args.literal else "bounded rays", bvh_nodes=stats["n_nodes"],
+                            mode="literal" if args.literal else "bounded rays",
+                            scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
                             bvh_build_ms=stats["build_ms"], launch=ctx.last_launch()),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),

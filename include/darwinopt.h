@@ -163,15 +163,19 @@ typedef struct dw_propagate_params {
   uint32_t flags;          /* DW_PROP_* */
   int32_t block_threads;   /* 0 = default */
   int32_t blocks_per_sm;   /* 0 = default */
-  int32_t th_phys;         /* phase scheduling: run the physics phase once this many lanes of a warp wait for it; 0 = default */
-  int32_t th_leaf;         /* phase scheduling: run the triangle phase once this many lanes wait for it; 0 = default */
+  int32_t th_phys;         /* pool scheduler (default): idle lanes of a warp that trigger a refetch of queued rays or the
+                            * physics phase; legacy scheduler: lanes waiting for physics that trigger it; 0 = default */
+  int32_t th_leaf;         /* run the triangle phase once this many lanes of a warp wait for it; 0 = default */
   int32_t reserved[3];
 } dw_propagate_params;
 enum {
   /* Follow the oracle literally: every query is unbounded and the medium comes from the hit triangle (S2).
    * Default (flag clear): the medium is carried in the photon state after the first query and the sampled
    * bulk distance bounds the ray; equal in distribution in a closed world. */
-  DW_PROP_UNBOUNDED_QUERY = 1u
+  DW_PROP_UNBOUNDED_QUERY = 1u,
+  /* Diagnostic: run the first-generation kernel (photon state in registers, one photon per lane, physics and
+   * traversal phases chosen per warp) instead of the pool scheduler.  Same results photon by photon. */
+  DW_PROP_LEGACY_SCHEDULER = 2u
 };
 
 /* The propagation loop S1..S13 for every photon of the batch, at most max_steps iterations each.

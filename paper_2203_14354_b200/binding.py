@@ -20,6 +20,7 @@ FATE_DETECTED, FATE_BULK_ABSORBED, FATE_SURFACE_ABSORBED, FATE_ESCAPED, FATE_TRU
 H_RAYLEIGH, H_REFLECT_DIFFUSE, H_REFLECT_SPECULAR, H_SURFACE_TRANSMIT = 0x10, 0x20, 0x40, 0x80
 H_FRESNEL_REFLECT, H_FRESNEL_REFRACT, H_TIR, H_MEDIUM_MISMATCH = 0x100, 0x200, 0x400, 0x800
 PROP_UNBOUNDED_QUERY = 1
+PROP_LEGACY_SCHEDULER = 2
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",

@@ -521,6 +521,340 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
   if (threadIdx.x == 0 && A.hist.total_steps && s_steps) atomicAdd((unsigned long long*)A.hist.total_steps, s_steps);
 }
 
+// ------------------------------------------------------------------------------------------------ propagation, pool scheduler
+// Second scheduler: every warp owns kSlots photon slots in shared memory (SoA, one
+// word per field per slot).  A slot is EMPTY, waits for physics (PHYS: query finished), waits for a lane (TRACE:
+// next query set up) or is being traced by a lane (BUSY).  Lanes keep only the ray and the traversal state of the
+// query they run; when a query ends the lane writes (best_t, best_slot) to the slot and fetches another TRACE slot,
+// so traversal does not wait for physics, and physics runs for 32 slots at a time with every lane enabled.
+constexpr int kSlots = 64;
+enum : int { W_X = 0, W_Y, W_Z, W_KX, W_KY, W_KZ, W_EX, W_EY, W_EZ, W_LAMBDA, W_T, W_MEDIUM, W_LAST, W_STEP, W_HIST, W_PI,
+             W_DBULK, W_N1, W_US, W_UF, W_BEST_T, W_BEST_SLOT, kWords };
+enum : int { S_EMPTY = 0, S_PHYS = 1, S_TRACE = 2, S_BUSY = 3 };
+constexpr uint32_t kAbsorbFirstBit = 0x80000000u;                 // kept in the W_HIST word
+constexpr int kWarpPool = kWords * kSlots;                        // ints
+constexpr int kWarpSt = kWarpPool;                                // status[kSlots]
+constexpr int kWarpQ = kWarpSt + kSlots;                          // queue[kSlots] (rank -> slot scratch)
+constexpr int kWarpStack = kWarpQ + kSlots;                       // stack[kStackShared][32]
+constexpr int kWarpInts = kWarpStack + kStackShared * 32;
+
+__global__ void __launch_bounds__(128, 4) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
+  extern __shared__ int s_dyn[];
+  __shared__ unsigned int s_fate[8];
+  __shared__ unsigned long long s_steps;
+  if (threadIdx.x < 8) s_fate[threadIdx.x] = 0;
+  if (threadIdx.x == 0) s_steps = 0ull;
+  const int lane = threadIdx.x & 31;
+  int* const wbase = s_dyn + (threadIdx.x >> 5) * kWarpInts;
+  int* const pool = wbase;
+  float* const poolf = reinterpret_cast<float*>(wbase);
+  int* const st = wbase + kWarpSt;
+  int* const q = wbase + kWarpQ;
+  int* const my_stack = wbase + kWarpStack + lane;
+  constexpr int sstride = 32;
+  st[lane] = S_EMPTY;
+  st[lane + 32] = S_EMPTY;
+  __syncthreads();
+  int lstack[kStackLocal];
+  const unsigned lt = (1u << lane) - 1u;
+  const int64_t n = A.in.n;
+  const bool literal = (A.flags & DW_PROP_UNBOUNDED_QUERY) != 0;
+  const int th_fetch = A.th_phys, th_leaf = A.th_leaf;
+
+  int64_t w_next = 0, w_end = 0;     // warp-private range of photon indices
+  bool exhausted = false;
+  // the query this lane is running
+  int my = -1;                       // slot, -1: lane idle
+  Ray ray;
+  ray.o = mk(0, 0, 0); ray.d = mk(0, 0, 1); ray.inv = mk(0, 0, 0); ray.oi = mk(0, 0, 0);
+  int q_exclude = -1, q_medium = -1;
+  TraceState ts;
+  ts_begin(ts, 0.f);
+  ts.node = kDone;
+
+  for (;;) {
+    // ---------------------------------------------------------------- census of the warp's slots
+    const int s0 = st[lane], s1 = st[lane + 32];
+    const unsigned p0 = __ballot_sync(0xffffffffu, s0 == S_PHYS), p1 = __ballot_sync(0xffffffffu, s1 == S_PHYS);
+    const unsigned e0 = __ballot_sync(0xffffffffu, s0 == S_EMPTY), e1 = __ballot_sync(0xffffffffu, s1 == S_EMPTY);
+    const unsigned t0 = __ballot_sync(0xffffffffu, s0 == S_TRACE), t1 = __ballot_sync(0xffffffffu, s1 == S_TRACE);
+    const unsigned idle = __ballot_sync(0xffffffffu, my < 0);
+    const int nP = __popc(p0) + __popc(p1);
+    const int nE = exhausted ? 0 : __popc(e0) + __popc(e1);
+    const int nQ = __popc(t0) + __popc(t1);
+    const int nB = 32 - __popc(idle);
+    if (nP + nE + nQ + nB == 0) break;
+
+    const bool do_phys = (nP + nE >= 32) || (nQ == 0 && (nB == 0 || nP + nE >= 8));
+    if (do_phys) {
+      // -------------------------------------------------------------- phase P: up to 32 slots, finished queries first
+      const int nPc = min(nP, 32);
+      int take = min(nE, 32 - nPc);                         // empty slots to refill (a2)
+      if (take > 0 && w_next == w_end) {                    // claim a new chunk of photon ids (one atomic per warp)
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(A.queue_head, (unsigned long long)(32 * kChunk));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        w_next = (int64_t)base;
+        w_end = (int64_t)base + 32 * kChunk;
+        if (w_next >= n) { w_next = w_end = 0; exhausted = true; }
+        else if (w_end > n) w_end = n;
+      }
+      take = (int)min((int64_t)take, w_end - w_next);
+      if (s0 == S_PHYS) q[__popc(p0 & lt)] = lane;
+      if (s1 == S_PHYS) q[__popc(p0) + __popc(p1 & lt)] = lane + 32;
+      if (s0 == S_EMPTY) q[nP + __popc(e0 & lt)] = lane;
+      if (s1 == S_EMPTY) q[nP + __popc(e0) + __popc(e1 & lt)] = lane + 32;
+      __syncwarp();
+      int slot = -1;
+      bool fresh = false;
+      int64_t pi = 0;
+      if (lane < nPc) slot = q[lane];
+      else if (lane < nPc + take) { slot = q[lane]; fresh = true; pi = w_next + (lane - nPc); }
+      w_next += take;
+      if (nPc + take == 0) continue;                        // nothing to do this round (queue just ran dry)
+
+      V3 x = mk(0, 0, 0), k = mk(0, 0, 1), e = mk(1, 0, 0);
+      float lambda = 0.f, t = 0.f, dbulk = INFINITY, n1 = 1.f, us = 0.f, uf = 0.f, best_t = INFINITY;
+      int medium = -1, last_tri = -1, best_slot = -1;
+      uint32_t step = 0, hist = 0;
+      bool absorb_first = false;
+      if (fresh) {
+        x = mk(A.in.px[pi], A.in.py[pi], A.in.pz[pi]);
+        k = mk(A.in.kx[pi], A.in.ky[pi], A.in.kz[pi]);
+        e = mk(A.in.ex[pi], A.in.ey[pi], A.in.ez[pi]);
+        lambda = A.in.wavelength[pi];
+        t = A.in.t0[pi];
+      } else if (slot >= 0) {
+        x = mk(poolf[W_X * kSlots + slot], poolf[W_Y * kSlots + slot], poolf[W_Z * kSlots + slot]);
+        k = mk(poolf[W_KX * kSlots + slot], poolf[W_KY * kSlots + slot], poolf[W_KZ * kSlots + slot]);
+        e = mk(poolf[W_EX * kSlots + slot], poolf[W_EY * kSlots + slot], poolf[W_EZ * kSlots + slot]);
+        lambda = poolf[W_LAMBDA * kSlots + slot];
+        t = poolf[W_T * kSlots + slot];
+        medium = pool[W_MEDIUM * kSlots + slot];
+        last_tri = pool[W_LAST * kSlots + slot];
+        step = (uint32_t)pool[W_STEP * kSlots + slot];
+        hist = (uint32_t)pool[W_HIST * kSlots + slot];
+        absorb_first = (hist & kAbsorbFirstBit) != 0;
+        hist &= ~kAbsorbFirstBit;
+        pi = (int64_t)(uint32_t)pool[W_PI * kSlots + slot];
+        dbulk = poolf[W_DBULK * kSlots + slot];
+        n1 = poolf[W_N1 * kSlots + slot];
+        us = poolf[W_US * kSlots + slot];
+        uf = poolf[W_UF * kSlots + slot];
+        best_t = poolf[W_BEST_T * kSlots + slot];
+        best_slot = pool[W_BEST_SLOT * kSlots + slot];
+      }
+      uint32_t fate = 0xFFu;           // 0xFF = still running
+      int channel = -1;
+      const uint64_t pid = A.in.photon_id_base + (uint64_t)pi;
+      if (slot >= 0 && !fresh) {
+        // ---------------------------------------------------------- evaluate the finished query: S2..S9
+        const bool bounded = (!literal) && (medium >= 0);
+        const bool have_hit = best_slot >= 0;
+        float4 tc = make_float4(0, 0, 0, 0), ta = tc, tb = tc;
+        int m1 = medium, m2 = medium;
+        V3 ng = mk(0, 0, 1);
+        bool toward_outer = false;
+        if (have_hit) {                                               // S2 sides
+          const float4* p = A.bvh.tris + 3 * (size_t)best_slot;
+          ta = __ldg(p); tb = __ldg(p + 1); tc = __ldg(p + 2);
+          ng = unit(cross(mk(ta.w, tb.x, tb.y), mk(tb.z, tb.w, tc.x)));
+          uint32_t cw = __float_as_uint(tc.z);
+          toward_outer = dot(k, ng) > 0.f;
+          int mi = (int)(cw & 0xFF), mo = (int)((cw >> 8) & 0xFF);
+          m1 = toward_outer ? mi : mo;
+          m2 = toward_outer ? mo : mi;
+        }
+        if (!bounded) {
+          if (!have_hit) {
+            fate = DW_FATE_ESCAPED;                                   // G3: ray leaves the world
+          } else {
+            float4 r0 = draw4(A.seed, pid, step, 0u);                 // (u_a, u_s, u_surface, u_fresnel)
+            us = r0.z; uf = r0.w;
+            if (medium >= 0 && medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
+            medium = m1;
+            n1 = table_at(A.tab.mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
+            absorb_first = da < ds;
+            dbulk = fminf(da, ds);
+          }
+        }
+        if (fate == 0xFFu) {
+          const bool surface_event = have_hit && (bounded ? true : !(dbulk < best_t));
+          if (!surface_event) {
+            if (!(dbulk < INFINITY)) {
+              fate = DW_FATE_ESCAPED;                                 // bounded query, no bulk process, nothing hit
+            } else {
+              x = fma3(dbulk, k, x);
+              t = fmaf(dbulk * n1, kInvC, t);
+              if (absorb_first) {
+                fate = DW_FATE_BULK_ABSORBED;                         // S4 first branch
+              } else {                                                // S4 second branch + S6
+                if (!rayleigh(k, e, A.seed, pid, step)) fate = DW_FATE_NAN_ABORT;
+                hist |= DW_H_RAYLEIGH;
+                last_tri = -1;
+              }
+            }
+          } else {                                                    // S4 third branch, S5
+            x = fma3(best_t, k, x);
+            t = fmaf(best_t * n1, kInvC, t);
+            last_tri = __float_as_int(tc.y);
+            if (medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
+            V3 nh = toward_outer ? mk(-ng.x, -ng.y, -ng.z) : ng;
+            uint32_t cw = __float_as_uint(tc.z);
+            int sf = (int)((cw >> 16) & 0xFF);
+            if (sf != 0xFF) {                                         // S7 explicit surface
+              const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
+              float c0 = table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c1 = table_at(A.tab.surf + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c2 = table_at(A.tab.surf + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c3 = table_at(A.tab.surf + 3 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              if (us < c0) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
+              else if (us < c1) { lambert(nh, k, e, draw4(A.seed, pid, step, 1u)); hist |= DW_H_REFLECT_DIFFUSE; }
+              else if (us < c2) {                                     // specular: no plane of incidence needed
+                k = unit(fma3(-2.0f * dot(k, nh), nh, k));
+                e = unit(fma3(-2.0f * dot(e, nh), nh, e));
+                hist |= DW_H_REFLECT_SPECULAR;
+              }
+              else if (us < c3) { hist |= DW_H_SURFACE_TRANSMIT; medium = m2; }
+              else fate = DW_FATE_SURFACE_ABSORBED;
+            } else {                                                  // S8 Fresnel
+              float n2 = table_at(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+              bool crossed;
+              hist |= fresnel(n1, n2, nh, k, e, uf, crossed);
+              if (crossed) medium = m2;
+            }
+          }
+        }
+        ++step;                                                       // S9 (every executed iteration counts, also the last: S13)
+      }
+      if (slot >= 0 && fate == 0xFFu) {
+        // ---------------------------------------------------------- set up the query of the next iteration: S1 (+S3/S4 draws)
+        if ((int32_t)step >= A.max_steps) {
+          fate = DW_FATE_TRUNCATED;                                   // S10
+        } else if (!(isfinite(x.x + x.y + x.z) && isfinite(k.x + k.y + k.z) && isfinite(e.x + e.y + e.z) && isfinite(t))) {
+          fate = DW_FATE_NAN_ABORT;                                   // S11
+        } else {
+          float tmax = INFINITY;
+          if ((!literal) && medium >= 0) {                            // medium known: S3/S4 draws before the query
+            float4 r0 = draw4(A.seed, pid, step, 0u);
+            us = r0.z; uf = r0.w;
+            n1 = table_at(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
+            absorb_first = da < ds;
+            dbulk = fminf(da, ds);
+            tmax = dbulk + A.bvh.eps_len;
+          }
+          poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
+          poolf[W_KX * kSlots + slot] = k.x; poolf[W_KY * kSlots + slot] = k.y; poolf[W_KZ * kSlots + slot] = k.z;
+          poolf[W_EX * kSlots + slot] = e.x; poolf[W_EY * kSlots + slot] = e.y; poolf[W_EZ * kSlots + slot] = e.z;
+          poolf[W_LAMBDA * kSlots + slot] = lambda;
+          poolf[W_T * kSlots + slot] = t;
+          pool[W_MEDIUM * kSlots + slot] = medium;
+          pool[W_LAST * kSlots + slot] = last_tri;
+          pool[W_STEP * kSlots + slot] = (int)step;
+          pool[W_HIST * kSlots + slot] = (int)(hist | (absorb_first ? kAbsorbFirstBit : 0u));
+          pool[W_PI * kSlots + slot] = (int)(uint32_t)pi;
+          poolf[W_DBULK * kSlots + slot] = dbulk;
+          poolf[W_N1 * kSlots + slot] = n1;
+          poolf[W_US * kSlots + slot] = us;
+          poolf[W_UF * kSlots + slot] = uf;
+          poolf[W_BEST_T * kSlots + slot] = tmax;                     // the query starts from t_max
+          pool[W_BEST_SLOT * kSlots + slot] = -1;
+          st[slot] = S_TRACE;
+        }
+      }
+
+      // -------------------------------------------------------------- a10: outputs and reductions
+      if (fate != 0xFFu) {
+        if (A.out.flags) A.out.flags[pi] = fate | hist;
+        if (A.out.channel) A.out.channel[pi] = channel;
+        if (A.out.t) A.out.t[pi] = t;
+        if (A.out.steps) A.out.steps[pi] = step;
+        if (A.out.last_tri) A.out.last_tri[pi] = last_tri;
+        if (A.out.x) A.out.x[pi] = x.x;
+        if (A.out.y) A.out.y[pi] = x.y;
+        if (A.out.z) A.out.z[pi] = x.z;
+        if (A.out.kx) { A.out.kx[pi] = k.x; A.out.ky[pi] = k.y; A.out.kz[pi] = k.z; }
+        if (A.out.ex) { A.out.ex[pi] = e.x; A.out.ey[pi] = e.y; A.out.ez[pi] = e.z; }
+        atomicAdd(&s_fate[fate & 7u], 1u);
+        atomicAdd(&s_steps, (unsigned long long)step);
+        st[slot] = S_EMPTY;
+      }
+      // detected photons: per-channel counts and arrival-time histogram, aggregated over equal keys in the warp
+      unsigned det = __ballot_sync(0xffffffffu, fate == DW_FATE_DETECTED);
+      if (det) {
+        bool mine = fate == DW_FATE_DETECTED;
+        if (A.hist.chan_count) {
+          bool ok = mine && channel >= 0 && channel < A.hist.n_chan;
+          unsigned peers = __match_any_sync(0xffffffffu, ok ? channel : -1 - lane);
+          if (ok && lane == (__ffs(peers) - 1)) atomicAdd((unsigned long long*)&A.hist.chan_count[channel], (unsigned long long)__popc(peers));
+        }
+        if (A.hist.time_hist && A.hist.n_bins > 0) {
+          float fb = floorf((t - A.hist.t_min) / A.hist.dt);
+          int bin = fb < 0.f ? 0 : (fb > (float)(A.hist.n_bins - 1) ? (int)(A.hist.n_bins - 1) : (int)fb);
+          unsigned peers = __match_any_sync(0xffffffffu, mine ? bin : -1 - lane);
+          if (mine && lane == (__ffs(peers) - 1)) atomicAdd(&A.hist.time_hist[bin], (unsigned)__popc(peers));
+        }
+      }
+      __syncwarp();
+      continue;
+    }
+
+    // ---------------------------------------------------------------- phase T: idle lanes fetch TRACE slots, then a4
+    if (nQ > 0 && idle) {
+      if (s0 == S_TRACE) q[__popc(t0 & lt)] = lane;
+      if (s1 == S_TRACE) q[__popc(t0) + __popc(t1 & lt)] = lane + 32;
+      __syncwarp();
+      const int r = __popc(idle & lt);
+      if (my < 0 && r < nQ) {
+        my = q[r];
+        V3 x = mk(poolf[W_X * kSlots + my], poolf[W_Y * kSlots + my], poolf[W_Z * kSlots + my]);
+        V3 k = mk(poolf[W_KX * kSlots + my], poolf[W_KY * kSlots + my], poolf[W_KZ * kSlots + my]);
+        ray_setup(ray, x, k);
+        ts_begin(ts, poolf[W_BEST_T * kSlots + my]);
+        q_exclude = pool[W_LAST * kSlots + my];
+        q_medium = literal ? -1 : pool[W_MEDIUM * kSlots + my];
+        st[my] = S_BUSY;
+      }
+      __syncwarp();
+    }
+    int nQ_rem = max(0, nQ - __popc(idle));
+    int nReady = nP + nE;                                   // slots the physics phase could take
+    int prevAct = -1;
+    for (;;) {
+      const bool act = my >= 0;
+      const int nI = __popc(__ballot_sync(0xffffffffu, act && ts.node >= 0));
+      const int nL = __popc(__ballot_sync(0xffffffffu, act && ts.node == kInLeaf));
+      const int nAct = nI + nL;
+      if (prevAct >= 0) nReady += prevAct - nAct;           // queries that ended in the last iteration
+      prevAct = nAct;
+      if (nAct == 0) break;
+      if (32 - nAct >= th_fetch && (nQ_rem > 0 || nReady >= 32)) break;
+      if (nI > 0 && nL < th_leaf) {
+        if (act && ts.node >= 0) step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
+      } else {
+        if (act && ts.node == kInLeaf) step_triangle(A.bvh, ray, ts, q_exclude, q_medium, my_stack, sstride, lstack);
+      }
+      if (act && ts.node == kDone) {                        // query finished: hand the slot to the physics phase
+        poolf[W_BEST_T * kSlots + my] = ts.best_t;
+        pool[W_BEST_SLOT * kSlots + my] = ts.best_slot;
+        st[my] = S_PHYS;
+        my = -1;
+      }
+    }
+    __syncwarp();
+  }
+
+  __syncthreads();
+  if (threadIdx.x < 8 && A.hist.fate_count && s_fate[threadIdx.x]) atomicAdd((unsigned long long*)&A.hist.fate_count[threadIdx.x], (unsigned long long)s_fate[threadIdx.x]);
+  if (threadIdx.x == 0 && A.hist.total_steps && s_steps) atomicAdd((unsigned long long*)A.hist.total_steps, s_steps);
+}
+
 __global__ void philox_debug_kernel(uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
                                     uint32_t* __restrict__ out_raw, float* __restrict__ out_u) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -542,24 +876,28 @@ int dw_first_hit_impl(dw_ctx* c, int64_t n, const float* ox, const float* oy, co
   return DW_OK;
 }
 
-int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
-                      const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream) {
+// One launch over photons [0, in->n) of `in`; n <= kMaxLaunch for the pool kernel (slot word W_PI is 32 bits).
+static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                            const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream) {
   static_assert(sizeof(PropArgs) <= 4000, "kernel parameter block too large");
   PropArgs A{};
   A.bvh = c->bvh; A.tab = c->tables; A.in = *in;
   if (out) A.out = *out;
   if (hist) A.hist = *hist;
   A.seed = seed; A.max_steps = max_steps; A.flags = params ? params->flags : 0u;
-  A.th_phys = (params && params->th_phys > 0) ? params->th_phys : 12;
+  const bool legacy = (A.flags & DW_PROP_LEGACY_SCHEDULER) != 0;
+  A.th_phys = (params && params->th_phys > 0) ? params->th_phys : (legacy ? 12 : 8);
   A.th_leaf = (params && params->th_leaf > 0) ? params->th_leaf : 12;
   int B = (params && params->block_threads) ? params->block_threads : 128;
   if (B < 32 || B > 128 || (B & 31)) return dw_fail(c, DW_E_ARG, "dw_propagate: block_threads must be 32, 64, 96 or 128");
-  size_t smem = sizeof(int) * kStackShared * B;
+  size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)kWarpInts * (B / 32);
   int per_sm = 0;
-  DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, propagate_kernel, B, smem));
+  if (legacy) DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, propagate_kernel, B, smem));
+  else DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, propagate_pool_kernel, B, smem));
   if (params && params->blocks_per_sm > 0) per_sm = std::min(per_sm, params->blocks_per_sm);
   if (per_sm < 1) return dw_fail(c, DW_E_CUDA, "dw_propagate: kernel does not fit on an SM");
-  int64_t warps_needed = (in->n + 31) / 32;
+  const int64_t per_warp = legacy ? 32 : kSlots;
+  int64_t warps_needed = (in->n + per_warp - 1) / per_warp;
   int64_t blocks_needed = (warps_needed + (B / 32) - 1) / (B / 32);
   int grid = (int)std::min<int64_t>((int64_t)c->sm_count * per_sm, std::max<int64_t>(blocks_needed, 1));
   // queue head: a stream-ordered 8-byte allocation, so that launches on different streams never share one
@@ -567,11 +905,40 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
   DW_CUDA(c, cudaMallocAsync((void**)&head, sizeof(unsigned long long), stream));
   DW_CUDA(c, cudaMemsetAsync(head, 0, sizeof(unsigned long long), stream));
   A.queue_head = head;
-  propagate_kernel<<<grid, B, smem, stream>>>(A);
+  if (legacy) propagate_kernel<<<grid, B, smem, stream>>>(A);
+  else propagate_pool_kernel<<<grid, B, smem, stream>>>(A);
   cudaError_t e = cudaGetLastError();
   cudaFreeAsync(head, stream);
-  if (e != cudaSuccess) return dw_fail(c, DW_E_CUDA, "propagate_kernel launch failed: %s", cudaGetErrorString(e));
+  if (e != cudaSuccess) return dw_fail(c, DW_E_CUDA, "propagate kernel launch failed: %s", cudaGetErrorString(e));
   c->last_grid = grid; c->last_block = B; c->last_smem = (int)smem; c->n_launches += 1;
+  return DW_OK;
+}
+
+template <class T> static inline T* off(T* p, int64_t o) { return p ? p + o : p; }
+
+int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                      const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream) {
+  constexpr int64_t kMaxLaunch = int64_t(1) << 30;
+  if (in->n <= kMaxLaunch) return launch_propagate(c, in, seed, max_steps, out, hist, params, stream);
+  for (int64_t o = 0; o < in->n; o += kMaxLaunch) {       // larger batches: consecutive launches over id sub-ranges
+    dw_photons pi = *in;
+    pi.n = std::min(kMaxLaunch, in->n - o);
+    pi.photon_id_base = in->photon_id_base + (uint64_t)o;
+    pi.px = off(in->px, o); pi.py = off(in->py, o); pi.pz = off(in->pz, o);
+    pi.kx = off(in->kx, o); pi.ky = off(in->ky, o); pi.kz = off(in->kz, o);
+    pi.ex = off(in->ex, o); pi.ey = off(in->ey, o); pi.ez = off(in->ez, o);
+    pi.wavelength = off(in->wavelength, o); pi.t0 = off(in->t0, o);
+    dw_results po{};
+    if (out) {
+      po = *out;
+      po.flags = off(out->flags, o); po.channel = off(out->channel, o); po.t = off(out->t, o); po.steps = off(out->steps, o);
+      po.last_tri = off(out->last_tri, o); po.x = off(out->x, o); po.y = off(out->y, o); po.z = off(out->z, o);
+      po.kx = off(out->kx, o); po.ky = off(out->ky, o); po.kz = off(out->kz, o);
+      po.ex = off(out->ex, o); po.ey = off(out->ey, o); po.ez = off(out->ez, o);
+    }
+    int rc = launch_propagate(c, &pi, seed, max_steps, out ? &po : nullptr, hist, params, stream);
+    if (rc != DW_OK) return rc;
+  }
   return DW_OK;
 }
 

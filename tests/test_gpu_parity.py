@@ -531,3 +531,18 @@ def test_literal_mode_leak_budget_on_closed_sphere():
     fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
     assert sum(fc.values()) == N
     assert fc["escaped"] <= max(1, int(1e-6 * N)), f"{fc['escaped']} photons leaked"
+
+
+@pytest.mark.parametrize("cfg,n,mode", [(1, 300_000, 0), (1, 100_000, dw.PROP_UNBOUNDED_QUERY), (2, 300_000, 0), (0, 100_000, 0)])
+def test_pool_scheduler_bit_identical_to_legacy(cfg, n, mode):
+    """The pool scheduler (default) only changes WHEN each photon's steps are executed, never what they compute:
+    with the counter-based RNG (P11) every per-photon output and every integer reduction must be bit-identical to the
+    first-generation kernel, in both query modes, including a batch that is not a multiple of the slot count."""
+    c, ctx = ctx_for(cfg)
+    n = n - 37                                               # ragged: not a multiple of 32, 64 or the 256-id chunk
+    ph = c.make_photons(n)
+    a = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=200, dt=2.0, flags=mode)
+    b = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=200, dt=2.0, flags=mode | dw.PROP_LEGACY_SCHEDULER)
+    for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
+        assert np.array_equal(a[key], b[key]), f"C{cfg} mode {mode}: '{key}' differs between schedulers"
+    assert int(a["fate_count"].sum()) == n
