@@ -99,14 +99,17 @@ int dw_set_geometry(dw_ctx* ctx, int64_t n_vert, const float* xyz, int64_t n_tri
 
 typedef struct dw_build_params {
   int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (4) */
-  int32_t reserved[7];
+  int32_t ploc_radius;   /* 1..256, search radius of the clustering rounds in Morton order; 0 = default (16) */
+  int32_t reserved[6];
 } dw_build_params;
 
 typedef struct dw_build_stats {
   int64_t n_tri, n_nodes, node_bytes, tri_bytes;
-  int32_t max_depth, n_leaves;
+  int32_t max_depth, n_leaves; /* max_depth: levels of the 4-wide traversal tree */
   float scene_lo[3], scene_hi[3];
   float build_ms; /* device time of the whole build */
+  int32_t ploc_rounds;  /* clustering rounds executed */
+  int32_t binary_depth; /* depth of the binary tree before the collapse into 4-wide nodes */
 } dw_build_stats;
 
 /* Device LBVH build: triangle boxes -> scene bounds -> 63-bit Morton codes of the centroids -> radix sort ->

@@ -1,7 +1,10 @@
-// dw_bvh.cu -- device LBVH build (the paper names no structure, only GPU ray
-// traversal [27]): triangle boxes -> scene bounds -> 63-bit Morton codes of centroids -> radix sort ->
-// binary radix tree (Karras 2012) -> bottom-up refit -> subtree collapse into <= max_leaf triangle leaves ->
-// compacted 64-byte traversal nodes + triangles permuted to leaf order in Moeller-Trumbore form.
+// dw_bvh.cu -- device BVH build (the paper names no structure, only GPU ray traversal [27],
+// P:111): triangle boxes -> scene bounds -> 63-bit Morton codes of box centres -> radix sort -> bottom-up binary tree by
+// parallel locally-ordered clustering over the Morton order (PLOC, Meister & Bittner 2018: every cluster looks
+// +-radius positions around itself for the partner that gives the smallest merged box; mutual choices merge) ->
+// depth-first triangle order, subtrees of <= max_leaf triangles folded into leaves -> greedy collapse into 4-wide
+// nodes (open the child of largest area first) -> 128-byte SoA traversal nodes + Moeller-Trumbore triangle records.
+// Why PLOC and 4-wide: DESIGN.md section 5 (node visits and box tests per query against the Morton radix tree).
 #include <float.h>
 
 #include <cub/device/device_radix_sort.cuh>
@@ -76,123 +79,179 @@ __global__ void morton_kernel(int n, const float* __restrict__ tlo, const float*
   vals[t] = (unsigned)t;
 }
 
-// ---- Karras 2012 binary radix tree over sorted keys.  Node numbering: internal i in [0, n-2], leaf j in [0, n-1]
-// stored as (n - 1 + j) in the parent / box arrays.
-__device__ __forceinline__ int delta(const unsigned long long* __restrict__ keys, int n, int i, int j) {
-  if (j < 0 || j >= n) return -1;
-  unsigned long long a = keys[i], b = keys[j];
-  if (a == b) return 64 + __clz(i ^ j);
-  return __clzll((long long)(a ^ b));
+// ---- binary tree.  Node numbering: leaf j in [0, n-1] = the j-th triangle in Morton order; internal nodes n .. 2n-2 in
+// the order PLOC creates them (children always before parents), so the root is node 2n-2.  Boxes: blo/bhi[node].xyz.
+__device__ __forceinline__ float half_area(float4 lo, float4 hi) {
+  float ex = hi.x - lo.x, ey = hi.y - lo.y, ez = hi.z - lo.z;
+  return fmaf(ex, ey, fmaf(ey, ez, ex * ez));
 }
+__device__ __forceinline__ float4 min4(float4 a, float4 b) { return make_float4(fminf(a.x, b.x), fminf(a.y, b.y), fminf(a.z, b.z), 0.f); }
+__device__ __forceinline__ float4 max4(float4 a, float4 b) { return make_float4(fmaxf(a.x, b.x), fmaxf(a.y, b.y), fmaxf(a.z, b.z), 0.f); }
 
-__global__ void radix_tree_kernel(int n, const unsigned long long* __restrict__ keys, int* __restrict__ left,
-                                  int* __restrict__ right, int* __restrict__ parent, int* __restrict__ rfirst,
-                                  int* __restrict__ rlast) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n - 1) return;
-  int d = (delta(keys, n, i, i + 1) - delta(keys, n, i, i - 1)) >= 0 ? 1 : -1;
-  int dmin = delta(keys, n, i, i - d);
-  int lmax = 2;
-  while (delta(keys, n, i, i + lmax * d) > dmin) lmax <<= 1;
-  int l = 0;
-  for (int t = lmax >> 1; t >= 1; t >>= 1)
-    if (delta(keys, n, i, i + (l + t) * d) > dmin) l += t;
-  int j = i + l * d;
-  int dnode = delta(keys, n, i, j);
-  int s = 0, t = l;
-  do {
-    t = (t + 1) >> 1;
-    if (delta(keys, n, i, i + (s + t) * d) > dnode) s += t;
-  } while (t > 1);
-  int gamma = i + s * d + min(d, 0);
-  int lo = min(i, j), hi = max(i, j);
-  int L = (lo == gamma) ? (n - 1 + gamma) : gamma;
-  int R = (hi == gamma + 1) ? (n - 1 + gamma + 1) : (gamma + 1);
-  left[i] = L; right[i] = R;
-  parent[L] = i; parent[R] = i;
-  rfirst[i] = lo; rlast[i] = hi;
-  if (i == 0) parent[0] = -1;
-}
-
-// bottom-up refit: second arrival at a node computes its box.  Boxes: [2n-1][6]
-__global__ void refit_kernel(int n, const unsigned* __restrict__ vals, const float* __restrict__ tlo,
-                             const float* __restrict__ thi, const int* __restrict__ left, const int* __restrict__ right,
-                             const int* __restrict__ parent, float* __restrict__ box, int* __restrict__ flag) {
+__global__ void ploc_init_kernel(int n, const unsigned* __restrict__ vals, const float* __restrict__ tlo,
+                                 const float* __restrict__ thi, float4* __restrict__ blo, float4* __restrict__ bhi,
+                                 int* __restrict__ cnode, float4* __restrict__ clo, float4* __restrict__ chi,
+                                 int* __restrict__ size, int* __restrict__ parent, int* __restrict__ leftmost) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   int t = vals[j];
-  int me = n - 1 + j;
-  for (int a = 0; a < 3; ++a) { box[6 * (int64_t)me + a] = tlo[3 * (int64_t)t + a]; box[6 * (int64_t)me + 3 + a] = thi[3 * (int64_t)t + a]; }
-  __threadfence();
-  int p = (n > 1) ? parent[me] : -1;
-  while (p >= 0) {
-    if (atomicAdd(&flag[p], 1) == 0) return;   // first arrival: the sibling subtree is not done yet
-    __threadfence();
-    int L = left[p], R = right[p];
-    for (int a = 0; a < 3; ++a) {
-      box[6 * (int64_t)p + a] = fminf(__ldcg(&box[6 * (int64_t)L + a]), __ldcg(&box[6 * (int64_t)R + a]));
-      box[6 * (int64_t)p + 3 + a] = fmaxf(__ldcg(&box[6 * (int64_t)L + 3 + a]), __ldcg(&box[6 * (int64_t)R + 3 + a]));
-    }
-    __threadfence();
-    p = parent[p];
+  float4 lo = make_float4(tlo[3 * (int64_t)t], tlo[3 * (int64_t)t + 1], tlo[3 * (int64_t)t + 2], 0.f);
+  float4 hi = make_float4(thi[3 * (int64_t)t], thi[3 * (int64_t)t + 1], thi[3 * (int64_t)t + 2], 0.f);
+  blo[j] = lo; bhi[j] = hi; clo[j] = lo; chi[j] = hi;
+  cnode[j] = j; size[j] = 1; parent[j] = -1; leftmost[j] = j;
+}
+
+// Nearest neighbour of cluster i among positions i-radius .. i+radius: smallest merged half-area, ties -> smallest
+// position.  The pair that is smallest in (area, i, j) order always chooses each other, so every round merges.
+__global__ void ploc_nn_kernel(int m, int radius, const float4* __restrict__ clo, const float4* __restrict__ chi,
+                               int* __restrict__ nn) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m) return;
+  float4 lo = clo[i], hi = chi[i];
+  float best = FLT_MAX;
+  int bj = -1;
+  int j0 = max(i - radius, 0), j1 = min(i + radius, m - 1);
+  for (int j = j0; j <= j1; ++j) {
+    if (j == i) continue;
+    float a = half_area(min4(lo, clo[j]), max4(hi, chi[j]));
+    if (a < best || bj < 0) { best = a; bj = j; }          // strict <: the first (smallest) position wins ties
+  }
+  nn[i] = bj;
+}
+
+// keep[i] = 0 for the higher position of a mutual pair (it disappears); isnew[i] = 1 for the lower one (a node is made).
+__global__ void ploc_mark_kernel(int m, const int* __restrict__ nn, int* __restrict__ keep, int* __restrict__ isnew) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m) return;
+  int j = nn[i];
+  bool mutual = j >= 0 && nn[j] == i;
+  keep[i] = (mutual && i > j) ? 0 : 1;
+  isnew[i] = (mutual && i < j) ? 1 : 0;
+}
+
+__global__ void ploc_apply_kernel(int m, int base, const int* __restrict__ nn, const int* __restrict__ keep,
+                                  const int* __restrict__ isnew, const int* __restrict__ kpos, const int* __restrict__ npos,
+                                  const int* __restrict__ cnode_in, const float4* __restrict__ clo_in,
+                                  const float4* __restrict__ chi_in, int* __restrict__ cnode_out,
+                                  float4* __restrict__ clo_out, float4* __restrict__ chi_out, int* __restrict__ left,
+                                  int* __restrict__ right, int* __restrict__ parent, float4* __restrict__ blo,
+                                  float4* __restrict__ bhi, int* __restrict__ size) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= m || !keep[i]) return;
+  int pos = kpos[i];
+  if (isnew[i]) {
+    int j = nn[i];
+    int node = base + npos[i];
+    int a = cnode_in[i], b = cnode_in[j];
+    float4 lo = min4(clo_in[i], clo_in[j]), hi = max4(chi_in[i], chi_in[j]);
+    left[node] = a; right[node] = b; parent[a] = node; parent[b] = node; parent[node] = -1;
+    blo[node] = lo; bhi[node] = hi;
+    size[node] = size[a] + size[b];
+    cnode_out[pos] = node; clo_out[pos] = lo; chi_out[pos] = hi;
+  } else {
+    cnode_out[pos] = cnode_in[i]; clo_out[pos] = clo_in[i]; chi_out[pos] = chi_in[i];
   }
 }
 
-// statistics only: depth of the deepest leaf of the binary radix tree
-__global__ void depth_kernel(int n, const int* __restrict__ parent, int* __restrict__ depth_max) {
+// Depth-first slot of every triangle: walking from leaf j to the root, every time the walk arrives from a right child
+// the whole left sibling subtree lies before j.  While the walk has only taken left-child steps, j is the leftmost
+// leaf of the node reached (leftmost[] gives a leaf group its first slot later).
+__global__ void leaf_walk_kernel(int n, const int* __restrict__ left, const int* __restrict__ parent,
+                                 const int* __restrict__ size, int* __restrict__ slot, int* __restrict__ leftmost,
+                                 int* __restrict__ depth_max) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   int depth = 0;
-  if (j < n) for (int p = parent[n - 1 + j]; p >= 0; p = parent[p]) ++depth;
+  if (j < n) {
+    int off = 0, cur = j;
+    bool all_left = true;
+    for (int p = parent[cur]; p >= 0; p = parent[cur]) {
+      int l = left[p];
+      if (l != cur) { off += size[l]; all_left = false; }
+      else if (all_left) leftmost[p] = j;
+      cur = p;
+      ++depth;
+    }
+    slot[j] = off;
+  }
   for (int o = 16; o; o >>= 1) depth = max(depth, __shfl_xor_sync(0xffffffffu, depth, o));
   if ((threadIdx.x & 31) == 0) atomicMax(depth_max, depth);
 }
 
-// alive[i] = 1 for internal nodes that appear in the traversal structure: the root, and every internal node
-// whose range holds more than max_leaf triangles (smaller subtrees are folded into a leaf of their parent).
-__global__ void alive_kernel(int n, int max_leaf, const int* __restrict__ rfirst, const int* __restrict__ rlast,
-                             int* __restrict__ alive) {
+struct WideTask { int bnode, widx; };
+
+__device__ __forceinline__ void write_wide(float4* __restrict__ nodes, int w, const float4* lo, const float4* hi, const int* ref) {
+  float4* o = nodes + 8 * (int64_t)w;
+  o[0] = make_float4(lo[0].x, lo[1].x, lo[2].x, lo[3].x);
+  o[1] = make_float4(lo[0].y, lo[1].y, lo[2].y, lo[3].y);
+  o[2] = make_float4(lo[0].z, lo[1].z, lo[2].z, lo[3].z);
+  o[3] = make_float4(hi[0].x, hi[1].x, hi[2].x, hi[3].x);
+  o[4] = make_float4(hi[0].y, hi[1].y, hi[2].y, hi[3].y);
+  o[5] = make_float4(hi[0].z, hi[1].z, hi[2].z, hi[3].z);
+  o[6] = make_float4(__int_as_float(ref[0]), __int_as_float(ref[1]), __int_as_float(ref[2]), __int_as_float(ref[3]));
+  o[7] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+// One level of the collapse: binary node b (more than max_leaf triangles) becomes wide node w.  Its two children are
+// opened greedily, largest box first, until four remain or none can be opened (a subtree of <= max_leaf triangles is a
+// leaf and stays closed).  Children that are still subtrees get a wide index and a task for the next level.
+__global__ void wide_collapse_kernel(int n_tasks, const WideTask* __restrict__ tasks, WideTask* __restrict__ next,
+                                     int* __restrict__ counters /* [0] next count, [1] wide nodes, [2] leaves */,
+                                     int max_leaf, const int* __restrict__ left, const int* __restrict__ right,
+                                     const int* __restrict__ size, const float4* __restrict__ blo,
+                                     const float4* __restrict__ bhi, const int* __restrict__ slot,
+                                     const int* __restrict__ leftmost, float4* __restrict__ nodes) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n - 1) return;
-  alive[i] = (i == 0 || (rlast[i] - rfirst[i] + 1) > max_leaf) ? 1 : 0;
+  if (i >= n_tasks) return;
+  const int b = tasks[i].bnode, w = tasks[i].widx;
+  int kid[4];
+  int nk = 2;
+  kid[0] = left[b]; kid[1] = right[b];
+  while (nk < 4) {
+    int pick = -1;
+    float amax = -1.f;
+    for (int k = 0; k < nk; ++k) {
+      if (size[kid[k]] <= max_leaf) continue;
+      float a = half_area(blo[kid[k]], bhi[kid[k]]);
+      if (a > amax) { amax = a; pick = k; }
+    }
+    if (pick < 0) break;
+    int c = kid[pick];
+    kid[pick] = left[c];
+    kid[nk++] = right[c];
+  }
+  float4 lo[4], hi[4];
+  int ref[4];
+  for (int k = 0; k < 4; ++k) {
+    lo[k] = make_float4(FLT_MAX, FLT_MAX, FLT_MAX, 0.f); hi[k] = make_float4(-FLT_MAX, -FLT_MAX, -FLT_MAX, 0.f); ref[k] = DW_REF_NONE;
+    if (k >= nk) continue;
+    int c = kid[k];
+    lo[k] = blo[c]; hi[k] = bhi[c];
+    if (size[c] <= max_leaf) {
+      ref[k] = ~((slot[leftmost[c]] << 3) | (size[c] - 1));
+      atomicAdd(&counters[2], 1);
+    } else {
+      int widx = atomicAdd(&counters[1], 1);
+      ref[k] = widx;
+      next[atomicAdd(&counters[0], 1)] = WideTask{c, widx};
+    }
+  }
+  write_wide(nodes, w, lo, hi, ref);
 }
 
-__device__ __forceinline__ int child_ref(int c, int n, int max_leaf, const int* rfirst, const int* rlast, const int* newidx,
-                                         int* n_leaves) {
-  if (c >= n - 1) { atomicAdd(n_leaves, 1); return ~(((c - (n - 1)) << 3) | 0); }       // single-triangle leaf
-  int cnt = rlast[c] - rfirst[c] + 1;
-  if (cnt <= max_leaf) { atomicAdd(n_leaves, 1); return ~((rfirst[c] << 3) | (cnt - 1)); }
-  return newidx[c];
+// A world of <= max_leaf triangles (or none): one wide node whose first child is the only leaf (or nothing).
+__global__ void wide_single_kernel(int n, const float4* __restrict__ blo, const float4* __restrict__ bhi, float4* __restrict__ nodes) {
+  float4 lo[4], hi[4];
+  int ref[4];
+  for (int k = 0; k < 4; ++k) { lo[k] = make_float4(FLT_MAX, FLT_MAX, FLT_MAX, 0.f); hi[k] = make_float4(-FLT_MAX, -FLT_MAX, -FLT_MAX, 0.f); ref[k] = DW_REF_NONE; }
+  if (n > 0) { lo[0] = blo[2 * n - 2]; hi[0] = bhi[2 * n - 2]; ref[0] = ~((0 << 3) | (n - 1)); }
+  write_wide(nodes, 0, lo, hi, ref);
 }
 
-__global__ void emit_nodes_kernel(int n, int max_leaf, const int* __restrict__ left, const int* __restrict__ right,
-                                  const int* __restrict__ rfirst, const int* __restrict__ rlast,
-                                  const int* __restrict__ alive, const int* __restrict__ newidx,
-                                  const float* __restrict__ box, float4* __restrict__ nodes, int* __restrict__ n_leaves) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n - 1 || !alive[i]) return;
-  int L = left[i], R = right[i];
-  const float* b0 = box + 6 * (int64_t)L;
-  const float* b1 = box + 6 * (int64_t)R;
-  int r0 = child_ref(L, n, max_leaf, rfirst, rlast, newidx, n_leaves);
-  int r1 = child_ref(R, n, max_leaf, rfirst, rlast, newidx, n_leaves);
-  float4* o = nodes + 4 * (int64_t)newidx[i];
-  o[0] = make_float4(b0[0], b0[1], b0[2], b0[3]);
-  o[1] = make_float4(b0[4], b0[5], b1[0], b1[1]);
-  o[2] = make_float4(b1[2], b1[3], b1[4], b1[5]);
-  o[3] = make_float4(__int_as_float(r0), __int_as_float(r1), 0.f, 0.f);
-}
-
-// n == 1: a root whose first child is the only triangle and whose second child is empty
-__global__ void emit_single_kernel(const float* __restrict__ tlo, const float* __restrict__ thi, float4* __restrict__ nodes) {
-  nodes[0] = make_float4(tlo[0], tlo[1], tlo[2], thi[0]);
-  nodes[1] = make_float4(thi[1], thi[2], FLT_MAX, FLT_MAX);
-  nodes[2] = make_float4(FLT_MAX, -FLT_MAX, -FLT_MAX, -FLT_MAX);
-  nodes[3] = make_float4(__int_as_float(~0), __int_as_float(DW_REF_NONE), 0.f, 0.f);
-}
-
-__global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const float* __restrict__ xyz,
-                                 const int32_t* __restrict__ idx, const uint32_t* __restrict__ code,
-                                 const int32_t* __restrict__ chan, float4* __restrict__ tris) {
+// triangle j of the Morton order goes to depth-first slot[j]
+__global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const int* __restrict__ slot,
+                                 const float* __restrict__ xyz, const int32_t* __restrict__ idx,
+                                 const uint32_t* __restrict__ code, const int32_t* __restrict__ chan,
+                                 float4* __restrict__ tris) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   int t = vals[j];
@@ -203,7 +262,7 @@ __global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const
     e1[a] = xyz[3 * (int64_t)i1 + a] - v0[a];
     e2[a] = xyz[3 * (int64_t)i2 + a] - v0[a];
   }
-  float4* o = tris + 3 * (int64_t)j;
+  float4* o = tris + 3 * (int64_t)slot[j];
   o[0] = make_float4(v0[0], v0[1], v0[2], e1[0]);
   o[1] = make_float4(e1[1], e1[2], e2[0], e2[1]);
   o[2] = make_float4(e2[2], __int_as_float(t), __uint_as_float(code[t]), __int_as_float(chan[t]));
@@ -217,109 +276,145 @@ __global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const
 int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* stats, cudaStream_t stream) {
   int rc = DW_OK;
   const int n = (int)c->n_tri;
-  int max_leaf = (params && params->max_leaf_tris) ? params->max_leaf_tris : 4;
+  const int max_leaf = (params && params->max_leaf_tris) ? params->max_leaf_tris : 4;
+  const int radius = (params && params->ploc_radius) ? params->ploc_radius : 16;
   if (max_leaf < 1 || max_leaf > 8) return dw_fail(c, DW_E_ARG, "dw_build_bvh: max_leaf_tris must be in 1..8");
+  if (radius < 1 || radius > 256) return dw_fail(c, DW_E_ARG, "dw_build_bvh: ploc_radius must be in 1..256");
   cudaFree(c->d_nodes); cudaFree(c->d_tris);
   c->d_nodes = nullptr; c->d_tris = nullptr; c->built = false;
   if (stats) memset(stats, 0, sizeof *stats);
 
-  float *tlo = nullptr, *thi = nullptr, *box = nullptr;
+  const size_t N = (size_t)std::max(n, 1), N2 = 2 * N;
+  float *tlo = nullptr, *thi = nullptr;
+  float4 *blo = nullptr, *bhi = nullptr, *cl[2] = {nullptr, nullptr}, *ch[2] = {nullptr, nullptr}, *nodes_tmp = nullptr;
   unsigned *scene = nullptr, *vals = nullptr, *vals2 = nullptr;
   unsigned long long *keys = nullptr, *keys2 = nullptr;
-  int *left = nullptr, *right = nullptr, *parent = nullptr, *rfirst = nullptr, *rlast = nullptr, *flag = nullptr,
-      *alive = nullptr, *newidx = nullptr, *misc = nullptr;
+  int *left = nullptr, *right = nullptr, *parent = nullptr, *size = nullptr, *leftmost = nullptr, *cn[2] = {nullptr, nullptr},
+      *nn = nullptr, *keep = nullptr, *isnew = nullptr, *kpos = nullptr, *npos = nullptr, *slot = nullptr, *misc = nullptr;
+  WideTask* tasks[2] = {nullptr, nullptr};
   void* tmp = nullptr;
   size_t tmp_bytes = 0, tmp2 = 0;
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-  unsigned h_scene[6];
-  int h_misc[4] = {0, 0, 0, 0};
-  int n_nodes = 1;
+  unsigned h_scene[6] = {0, 0, 0, 0, 0, 0};
+  int h_misc[4] = {0, 0, 0, 0};      // [0] next-level tasks, [1] wide nodes, [2] leaves, [3] binary depth
+  int n_nodes = 1, wide_depth = 1, ploc_rounds = 0;
   const int B = 256;
-  const unsigned G = (unsigned)((std::max(n, 1) + B - 1) / B);
-
-  if (n == 0) {   // empty world: one node with two empty children
-    float4 h[4] = {make_float4(FLT_MAX, FLT_MAX, FLT_MAX, -FLT_MAX), make_float4(-FLT_MAX, -FLT_MAX, FLT_MAX, FLT_MAX),
-                   make_float4(FLT_MAX, -FLT_MAX, -FLT_MAX, -FLT_MAX), make_float4(0, 0, 0, 0)};
-    int none = DW_REF_NONE;
-    memcpy(&h[3].x, &none, 4); memcpy(&h[3].y, &none, 4);
-    DW_B(cudaMalloc(&c->d_nodes, sizeof h));
-    DW_B(cudaMalloc(&c->d_tris, 48));
-    DW_B(cudaMemcpy(c->d_nodes, h, sizeof h, cudaMemcpyHostToDevice));
-    c->bvh = DwBvh{c->d_nodes, c->d_tris, 1, 0, 0.f};
-    c->built = true;
-    return DW_OK;
-  }
+  const unsigned G = (unsigned)((N + B - 1) / B);
 
   DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
-  DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * n)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * n));
-  DW_B(cudaMalloc(&box, sizeof(float) * 6 * (2 * (size_t)n)));
+  DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * N)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * N));
+  DW_B(cudaMalloc(&blo, sizeof(float4) * N2)); DW_B(cudaMalloc(&bhi, sizeof(float4) * N2));
+  for (int k = 0; k < 2; ++k) {
+    DW_B(cudaMalloc(&cl[k], sizeof(float4) * N)); DW_B(cudaMalloc(&ch[k], sizeof(float4) * N)); DW_B(cudaMalloc(&cn[k], 4 * N));
+    DW_B(cudaMalloc(&tasks[k], sizeof(WideTask) * N));
+  }
   DW_B(cudaMalloc(&scene, sizeof(unsigned) * 6));
-  DW_B(cudaMalloc(&keys, 8 * (size_t)n)); DW_B(cudaMalloc(&keys2, 8 * (size_t)n));
-  DW_B(cudaMalloc(&vals, 4 * (size_t)n)); DW_B(cudaMalloc(&vals2, 4 * (size_t)n));
-  DW_B(cudaMalloc(&left, 4 * (size_t)n)); DW_B(cudaMalloc(&right, 4 * (size_t)n));
-  DW_B(cudaMalloc(&parent, 4 * (2 * (size_t)n))); DW_B(cudaMalloc(&rfirst, 4 * (size_t)n)); DW_B(cudaMalloc(&rlast, 4 * (size_t)n));
-  DW_B(cudaMalloc(&flag, 4 * (size_t)n)); DW_B(cudaMalloc(&alive, 4 * (size_t)n)); DW_B(cudaMalloc(&newidx, 4 * (size_t)n));
+  DW_B(cudaMalloc(&keys, 8 * N)); DW_B(cudaMalloc(&keys2, 8 * N));
+  DW_B(cudaMalloc(&vals, 4 * N)); DW_B(cudaMalloc(&vals2, 4 * N));
+  DW_B(cudaMalloc(&left, 4 * N2)); DW_B(cudaMalloc(&right, 4 * N2)); DW_B(cudaMalloc(&parent, 4 * N2));
+  DW_B(cudaMalloc(&size, 4 * N2)); DW_B(cudaMalloc(&leftmost, 4 * N2));
+  DW_B(cudaMalloc(&nn, 4 * N)); DW_B(cudaMalloc(&keep, 4 * N)); DW_B(cudaMalloc(&isnew, 4 * N));
+  DW_B(cudaMalloc(&kpos, 4 * N)); DW_B(cudaMalloc(&npos, 4 * N)); DW_B(cudaMalloc(&slot, 4 * N));
   DW_B(cudaMalloc(&misc, 16));
-  DW_B(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, n, 0, 63, stream));
-  DW_B(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, alive, newidx, std::max(n - 1, 1), stream));
+  DW_B(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)N, 0, 63, stream));
+  DW_B(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, keep, kpos, (int)N, stream));
   tmp_bytes = std::max(tmp_bytes, tmp2);
   DW_B(cudaMalloc(&tmp, tmp_bytes));
+  DW_B(cudaMalloc(&c->d_tris, 48 * N));
 
   DW_B(cudaEventRecord(ev0, stream));
-  {
+  DW_B(cudaMemsetAsync(misc, 0, 16, stream));
+  if (n > 0) {
     unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
     DW_B(cudaMemcpyAsync(scene, init, sizeof init, cudaMemcpyHostToDevice, stream));
+    tri_bounds_kernel<<<G, B, 0, stream>>>(n, c->d_xyz, c->d_idx, tlo, thi, scene);
+    morton_kernel<<<G, B, 0, stream>>>(n, tlo, thi, scene, keys, vals);
+    DW_B(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, n, 0, 63, stream));
+    ploc_init_kernel<<<G, B, 0, stream>>>(n, vals2, tlo, thi, blo, bhi, cn[0], cl[0], ch[0], size, parent, leftmost);
+    // ---- PLOC rounds: clusters [0, m) in buffer `cur`; every round makes at least one node
+    int m = n, base = n, cur = 0;
+    while (m > 1) {
+      const unsigned Gm = (unsigned)((m + B - 1) / B);
+      ploc_nn_kernel<<<Gm, B, 0, stream>>>(m, radius, cl[cur], ch[cur], nn);
+      ploc_mark_kernel<<<Gm, B, 0, stream>>>(m, nn, keep, isnew);
+      DW_B(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, keep, kpos, m, stream));
+      DW_B(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, isnew, npos, m, stream));
+      ploc_apply_kernel<<<Gm, B, 0, stream>>>(m, base, nn, keep, isnew, kpos, npos, cn[cur], cl[cur], ch[cur], cn[cur ^ 1],
+                                              cl[cur ^ 1], ch[cur ^ 1], left, right, parent, blo, bhi, size);
+      int h_last[2];
+      DW_B(cudaMemcpyAsync(&h_last[0], kpos + (m - 1), 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaMemcpyAsync(&h_last[1], keep + (m - 1), 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaStreamSynchronize(stream));
+      const int m_new = h_last[0] + h_last[1];
+      if (m_new >= m || m_new < 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: clustering round made no progress (%d -> %d)", m, m_new); goto done; }
+      base += m - m_new;
+      m = m_new;
+      cur ^= 1;
+      ++ploc_rounds;
+    }
+    if (base != 2 * n - 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: %d of %d nodes made", base - n, n - 1); goto done; }
+    leaf_walk_kernel<<<G, B, 0, stream>>>(n, left, parent, size, slot, leftmost, misc + 3);
+    pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris);
   }
-  DW_B(cudaMemsetAsync(flag, 0, 4 * (size_t)n, stream));
-  DW_B(cudaMemsetAsync(misc, 0, 16, stream));
-  tri_bounds_kernel<<<G, B, 0, stream>>>(n, c->d_xyz, c->d_idx, tlo, thi, scene);
-  morton_kernel<<<G, B, 0, stream>>>(n, tlo, thi, scene, keys, vals);
-  DW_B(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, n, 0, 63, stream));
-  DW_B(cudaMalloc(&c->d_tris, 48 * (size_t)n));
-  pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris);
-  if (n >= 2) {
-    radix_tree_kernel<<<G, B, 0, stream>>>(n, keys2, left, right, parent, rfirst, rlast);
-    refit_kernel<<<G, B, 0, stream>>>(n, vals2, tlo, thi, left, right, parent, box, flag);
-    depth_kernel<<<G, B, 0, stream>>>(n, parent, misc + 0);
-    alive_kernel<<<G, B, 0, stream>>>(n, max_leaf, rfirst, rlast, alive);
-    DW_B(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, alive, newidx, n - 1, stream));
-    // number of alive nodes = newidx[n-2] + alive[n-2]
-    int h_last[2];
-    DW_B(cudaMemcpyAsync(&h_last[0], newidx + (n - 2), 4, cudaMemcpyDeviceToHost, stream));
-    DW_B(cudaMemcpyAsync(&h_last[1], alive + (n - 2), 4, cudaMemcpyDeviceToHost, stream));
-    DW_B(cudaStreamSynchronize(stream));
-    n_nodes = h_last[0] + h_last[1];
-    DW_B(cudaMalloc(&c->d_nodes, 64 * (size_t)n_nodes));
-    emit_nodes_kernel<<<G, B, 0, stream>>>(n, max_leaf, left, right, rfirst, rlast, alive, newidx, box, c->d_nodes, misc + 1);
+  if (n <= max_leaf) {
+    DW_B(cudaMalloc(&c->d_nodes, 128));
+    wide_single_kernel<<<1, 1, 0, stream>>>(n, blo, bhi, c->d_nodes);
+    h_misc[1] = 1; h_misc[2] = n > 0 ? 1 : 0;
   } else {
-    DW_B(cudaMalloc(&c->d_nodes, 64));
-    emit_single_kernel<<<1, 1, 0, stream>>>(tlo, thi, c->d_nodes);
-    h_misc[0] = 1; h_misc[1] = 1;
+    // ---- collapse, one launch per level of the wide tree
+    DW_B(cudaMalloc(&nodes_tmp, 128 * N));
+    WideTask t0{2 * n - 2, 0};
+    int init[3] = {0, 1, 0};
+    DW_B(cudaMemcpyAsync(tasks[0], &t0, sizeof t0, cudaMemcpyHostToDevice, stream));
+    DW_B(cudaMemcpyAsync(misc, init, sizeof init, cudaMemcpyHostToDevice, stream));
+    int count = 1, cur = 0;
+    wide_depth = 0;
+    while (count > 0) {
+      wide_collapse_kernel<<<(unsigned)((count + B - 1) / B), B, 0, stream>>>(count, tasks[cur], tasks[cur ^ 1], misc, max_leaf, left, right,
+                                                                            size, blo, bhi, slot, leftmost, nodes_tmp);
+      DW_B(cudaMemcpyAsync(&count, misc, 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaStreamSynchronize(stream));
+      DW_B(cudaMemsetAsync(misc, 0, 4, stream));
+      cur ^= 1;
+      ++wide_depth;
+    }
+    DW_B(cudaMemcpyAsync(h_misc, misc, 16, cudaMemcpyDeviceToHost, stream));
+    DW_B(cudaStreamSynchronize(stream));
+    n_nodes = h_misc[1];
+    DW_B(cudaMalloc(&c->d_nodes, 128 * (size_t)n_nodes));
+    DW_B(cudaMemcpyAsync(c->d_nodes, nodes_tmp, 128 * (size_t)n_nodes, cudaMemcpyDeviceToDevice, stream));
   }
   DW_B(cudaGetLastError());
   DW_B(cudaEventRecord(ev1, stream));
-  DW_B(cudaMemcpyAsync(h_scene, scene, sizeof h_scene, cudaMemcpyDeviceToHost, stream));
-  if (n >= 2) DW_B(cudaMemcpyAsync(h_misc, misc, 8, cudaMemcpyDeviceToHost, stream));
+  if (n > 0) DW_B(cudaMemcpyAsync(h_scene, scene, sizeof h_scene, cudaMemcpyDeviceToHost, stream));
+  DW_B(cudaMemcpyAsync(&h_misc[3], misc + 3, 4, cudaMemcpyDeviceToHost, stream));
   DW_B(cudaStreamSynchronize(stream));
+  if (3 * wide_depth > kDwStackShared + kDwStackLocal) {
+    rc = dw_fail(c, DW_E_RANGE, "dw_build_bvh: tree depth %d exceeds the traversal stack (%d entries)", wide_depth, kDwStackShared + kDwStackLocal);
+    goto done;
+  }
   {
     float mx = 0.f;
-    float lo[3], hi[3];
-    for (int a = 0; a < 3; ++a) { lo[a] = o2f(h_scene[a]); hi[a] = o2f(h_scene[3 + a]); mx = fmaxf(mx, fmaxf(fabsf(lo[a]), fabsf(hi[a]))); }
+    float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    if (n > 0)
+      for (int a = 0; a < 3; ++a) { lo[a] = o2f(h_scene[a]); hi[a] = o2f(h_scene[3 + a]); mx = fmaxf(mx, fmaxf(fabsf(lo[a]), fabsf(hi[a]))); }
     // Length tolerance: a few fp32 spacings of the largest coordinate (positions cannot be resolved finer).
     float eps_len = 4.0f * 1.1920929e-7f * mx;
     c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len};
     c->built = true;
     if (stats) {
-      stats->n_tri = n; stats->n_nodes = n_nodes; stats->node_bytes = 64ll * n_nodes; stats->tri_bytes = 48ll * n;
-      stats->max_depth = h_misc[0]; stats->n_leaves = h_misc[1];
+      stats->n_tri = n; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
+      stats->max_depth = wide_depth; stats->n_leaves = h_misc[2];
       for (int a = 0; a < 3; ++a) { stats->scene_lo[a] = lo[a]; stats->scene_hi[a] = hi[a]; }
       cudaEventElapsedTime(&stats->build_ms, ev0, ev1);
+      stats->ploc_rounds = ploc_rounds; stats->binary_depth = h_misc[3];
     }
   }
 done:
-  cudaFree(tlo); cudaFree(thi); cudaFree(box); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
-  cudaFree(vals2); cudaFree(left); cudaFree(right); cudaFree(parent); cudaFree(rfirst); cudaFree(rlast); cudaFree(flag);
-  cudaFree(alive); cudaFree(newidx); cudaFree(misc); cudaFree(tmp);
+  cudaFree(tlo); cudaFree(thi); cudaFree(blo); cudaFree(bhi); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
+  cudaFree(vals2); cudaFree(left); cudaFree(right); cudaFree(parent); cudaFree(size); cudaFree(leftmost); cudaFree(nn);
+  cudaFree(keep); cudaFree(isnew); cudaFree(kpos); cudaFree(npos); cudaFree(slot); cudaFree(misc); cudaFree(tmp); cudaFree(nodes_tmp);
+  for (int k = 0; k < 2; ++k) { cudaFree(cl[k]); cudaFree(ch[k]); cudaFree(cn[k]); cudaFree(tasks[k]); }
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
   if (rc != DW_OK) { cudaFree(c->d_nodes); cudaFree(c->d_tris); c->d_nodes = nullptr; c->d_tris = nullptr; c->built = false; }

@@ -8,7 +8,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 100
+#define DW_VERSION 101
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
@@ -23,10 +23,14 @@ struct DwTables {
   float mat_l0, mat_inv_dl, surf_l0, surf_inv_dl;
 };
 
-// Binary BVH node, 64 B, read as four float4:
-//   q0 = (lo0.x, lo0.y, lo0.z, hi0.x)  q1 = (hi0.y, hi0.z, lo1.x, lo1.y)  q2 = (lo1.z, hi1.x, hi1.y, hi1.z)
-//   q3 = (as_float(ref0), as_float(ref1), -, -)
-// ref >= 0: internal node index; ref < 0: leaf, ~ref = (first_slot << 3) | (count - 1); DW_REF_NONE = empty.
+// 4-wide BVH node, 128 B, read as seven float4 (SoA over the four children; the eighth float4 is padding):
+//   q0 = lo.x[0..3]  q1 = lo.y[0..3]  q2 = lo.z[0..3]  q3 = hi.x[0..3]  q4 = hi.y[0..3]  q5 = hi.z[0..3]
+//   q6 = as_float(ref[0..3])
+// ref >= 0: wide node index; ref < 0: leaf, ~ref = (first_slot << 3) | (count - 1); DW_REF_NONE = empty child.
+// Traversal stack: kDwStackShared entries per thread in shared memory, kDwStackLocal more in local memory; a step
+// pushes at most 3, so trees up to (kDwStackShared + kDwStackLocal) / 3 levels fit (dw_build_bvh checks).
+constexpr int kDwStackShared = 12;
+constexpr int kDwStackLocal = 84;
 #define DW_REF_NONE 0x7fffffff
 
 // Triangle record in leaf order, 48 B, read as three float4 (Moeller-Trumbore form):
@@ -34,7 +38,7 @@ struct DwTables {
 //   c = (e2.z, as_float(caller id), as_float(code), as_float(channel))
 // code = inner | outer << 8 | surface << 16 (0xFF = no surface -> Fresnel)
 struct DwBvh {
-  const float4* nodes;  // [n_nodes][4]
+  const float4* nodes;  // [n_nodes][8]
   const float4* tris;   // [n_tri][3]
   int n_nodes;
   int n_tri;

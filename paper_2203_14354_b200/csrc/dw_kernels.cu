@@ -9,8 +9,8 @@
 namespace {
 
 constexpr float kInvC = 1.0f / 299.792458f;   // ns per mm in vacuum
-constexpr int kStackShared = 12;              // per-thread traversal stack entries kept in shared memory
-constexpr int kStackLocal = 64;               // overflow entries (local memory; only deep LBVH chains reach it)
+constexpr int kStackShared = kDwStackShared;  // per-thread traversal stack entries kept in shared memory
+constexpr int kStackLocal = kDwStackLocal;    // overflow entries (local memory; only unusually deep trees reach it)
 constexpr float kEdgeSlack = 2e-6f;           // barycentric slack that closes fp32 cracks between triangles
 constexpr float kBoxSlack = 1.0000005f;       // conservative slab test (robust traversal)
 
@@ -102,33 +102,45 @@ __device__ __forceinline__ void ts_goto(TraceState& s, int ref, const int* sstac
   s.node = kInLeaf;
 }
 
-// One internal node: slab-test both children against [0, best_t], descend into the nearer hit, push the other.
+// One 4-wide node: slab-test the four children against [0, best_t]; the nearest hit is visited next, the others are
+// pushed.  Empty children carry DW_REF_NONE (their inverted boxes alone would not reject: inf arithmetic).
+__device__ __forceinline__ bool slab(const Ray& r, float best_t, float eps, float lox, float loy, float loz, float hix,
+                                     float hiy, float hiz, float& tnear) {
+  float ax = fmaf(lox, r.inv.x, -r.oi.x), bx = fmaf(hix, r.inv.x, -r.oi.x);
+  float ay = fmaf(loy, r.inv.y, -r.oi.y), by = fmaf(hiy, r.inv.y, -r.oi.y);
+  float az = fmaf(loz, r.inv.z, -r.oi.z), bz = fmaf(hiz, r.inv.z, -r.oi.z);
+  tnear = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
+  float tfar = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), best_t));
+  return tnear <= fmaf(tfar, kBoxSlack, eps);
+}
+__device__ __forceinline__ void ts_push(TraceState& s, int ref, int* sstack, int sstride, int* lstack) {
+  if (s.sp < kStackShared) sstack[s.sp * sstride] = ref; else lstack[s.sp - kStackShared] = ref;
+  ++s.sp;
+}
 __device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
-  const float4* p = bvh.nodes + 4 * (size_t)s.node;
-  float4 q0 = __ldg(p), q1 = __ldg(p + 1), q2 = __ldg(p + 2), q3 = __ldg(p + 3);
-  // child 0: lo (q0.x q0.y q0.z) hi (q0.w q1.x q1.y); child 1: lo (q1.z q1.w q2.x) hi (q2.y q2.z q2.w)
-  float ax = fmaf(q0.x, r.inv.x, -r.oi.x), bx = fmaf(q0.w, r.inv.x, -r.oi.x);
-  float ay = fmaf(q0.y, r.inv.y, -r.oi.y), by = fmaf(q1.x, r.inv.y, -r.oi.y);
-  float az = fmaf(q0.z, r.inv.z, -r.oi.z), bz = fmaf(q1.y, r.inv.z, -r.oi.z);
-  float n0 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
-  float f0 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), s.best_t));
-  ax = fmaf(q1.z, r.inv.x, -r.oi.x); bx = fmaf(q2.y, r.inv.x, -r.oi.x);
-  ay = fmaf(q1.w, r.inv.y, -r.oi.y); by = fmaf(q2.z, r.inv.y, -r.oi.y);
-  az = fmaf(q2.x, r.inv.z, -r.oi.z); bz = fmaf(q2.w, r.inv.z, -r.oi.z);
-  float n1 = fmaxf(fmaxf(fminf(ax, bx), fminf(ay, by)), fmaxf(fminf(az, bz), 0.f));
-  float f1 = fminf(fminf(fmaxf(ax, bx), fmaxf(ay, by)), fminf(fmaxf(az, bz), s.best_t));
-  int r0 = __float_as_int(q3.x), r1 = __float_as_int(q3.y);
-  bool h0 = (n0 <= fmaf(f0, kBoxSlack, bvh.eps_len)) && (r0 != DW_REF_NONE);
-  bool h1 = (n1 <= fmaf(f1, kBoxSlack, bvh.eps_len)) && (r1 != DW_REF_NONE);
+  const float4* p = bvh.nodes + 8 * (size_t)s.node;
+  const float4 lx = __ldg(p), ly = __ldg(p + 1), lz = __ldg(p + 2), hx = __ldg(p + 3), hy = __ldg(p + 4), hz = __ldg(p + 5);
+  const float4 rf = __ldg(p + 6);
+  const int r0 = __float_as_int(rf.x), r1 = __float_as_int(rf.y), r2 = __float_as_int(rf.z), r3 = __float_as_int(rf.w);
+  float n0, n1, n2, n3;
+  const bool h0 = slab(r, s.best_t, bvh.eps_len, lx.x, ly.x, lz.x, hx.x, hy.x, hz.x, n0) && (r0 != DW_REF_NONE);
+  const bool h1 = slab(r, s.best_t, bvh.eps_len, lx.y, ly.y, lz.y, hx.y, hy.y, hz.y, n1) && (r1 != DW_REF_NONE);
+  const bool h2 = slab(r, s.best_t, bvh.eps_len, lx.z, ly.z, lz.z, hx.z, hy.z, hz.z, n2) && (r2 != DW_REF_NONE);
+  const bool h3 = slab(r, s.best_t, bvh.eps_len, lx.w, ly.w, lz.w, hx.w, hy.w, hz.w, n3) && (r3 != DW_REF_NONE);
+  // Nearest hit child by compare-and-select on the references themselves (children of a node are distinct).  Do NOT
+  // index the children by a computed position: nvcc turns that into a jump table (BRX) inside the traversal loop, and
+  // on sm_100a lanes that diverge at that indirect branch were observed not to reconverge before the warp votes of
+  // the schedulers (profiles/r01_pool_hang.md).
   int next = DW_REF_NONE;
-  if (h0 && h1) {
-    int farr = r1;
-    next = r0;
-    if (n1 < n0) { next = r1; farr = r0; }
-    if (s.sp < kStackShared) sstack[s.sp * sstride] = farr; else lstack[s.sp - kStackShared] = farr;
-    ++s.sp;
-  } else if (h0) next = r0;
-  else if (h1) next = r1;
+  float bn = INFINITY;
+  if (h0) { next = r0; bn = n0; }
+  if (h1 && (next == DW_REF_NONE || n1 < bn)) { next = r1; bn = n1; }
+  if (h2 && (next == DW_REF_NONE || n2 < bn)) { next = r2; bn = n2; }
+  if (h3 && (next == DW_REF_NONE || n3 < bn)) { next = r3; bn = n3; }
+  if (h0 && next != r0) ts_push(s, r0, sstack, sstride, lstack);
+  if (h1 && next != r1) ts_push(s, r1, sstack, sstride, lstack);
+  if (h2 && next != r2) ts_push(s, r2, sstack, sstride, lstack);
+  if (h3 && next != r3) ts_push(s, r3, sstack, sstride, lstack);
   ts_goto(s, next, sstack, sstride, lstack);
 }
 

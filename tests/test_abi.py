@@ -33,7 +33,7 @@ def test_struct_layouts_match_header_sizes():
     assert C.sizeof(binding.Hists) == 8 + 8 + 8 + 4 + 4 + 8 + 8 + 8
     assert C.sizeof(binding.PropagateParams) == 32
     assert C.sizeof(binding.BuildParams) == 32
-    assert C.sizeof(binding.BuildStats) == 4 * 8 + 2 * 4 + 6 * 4 + 4 + 4  # + tail padding to 8
+    assert C.sizeof(binding.BuildStats) == 4 * 8 + 2 * 4 + 6 * 4 + 4 + 2 * 4 + 4  # build_ms, ploc_rounds, binary_depth + tail padding to 8
 
 
 def test_no_cpu_fallback_without_gpu():
@@ -62,3 +62,17 @@ def test_product_path_does_not_import_the_oracle():
             assert "oracle" not in p.read_text().replace("the oracle", "").replace("The oracle", "").replace("oracle's", "").replace("oracle/", "").replace("oracle ", "").replace("oracle,", "").replace("oracle)", "").replace("oracle.", "X") or True
             src = p.read_text()
             assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, p
+
+
+def test_no_indirect_branches_in_device_code():
+    """profiles/r01_pool_hang.md: an indirect branch (jump table) inside the traversal loop left a warp split for good on
+    sm_100a, and the schedulers take warp-wide decisions from votes.  The built library must contain none."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    lib = binding._LIB_PATH
+    binding.load()
+    sass = subprocess.run([cuobjdump, "-sass", str(lib)], capture_output=True, text=True, check=True).stdout
+    assert "Function :" in sass, "no device code found in the library"
+    bad = [ln.strip() for ln in sass.splitlines() if " BRX" in ln or " JMX" in ln or " BRXU" in ln or " JMXU" in ln]
+    assert not bad, f"{len(bad)} indirect branches in device code, e.g. {bad[0]}"
