@@ -177,6 +177,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
+    ap.add_argument("--max-leaf", type=int, default=0, help="triangles per BVH leaf (0 = library default)")
+    ap.add_argument("--ploc-radius", type=int, default=0, help="search radius of the BVH clustering rounds (0 = library default)")
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
@@ -199,7 +201,7 @@ def main():
     ctx = dw.Context(local)
     ctx.set_optics(c.optics)
     ctx.set_geometry(c.geometry)
-    stats = ctx.build_bvh()
+    stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius)
     id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
     ph = c.make_photons(n, id_base)
     d_ph = dw.DevicePhotons(ph, dev)
@@ -293,7 +295,7 @@ def main():
                             seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
                             mode="literal" if args.literal else "bounded rays",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
-                            bvh_build_ms=stats["build_ms"], launch=ctx.last_launch()),
+                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], launch=ctx.last_launch()),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},

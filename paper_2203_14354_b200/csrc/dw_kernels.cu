@@ -550,7 +550,11 @@ constexpr int kWarpQ = kWarpSt + kSlots;                          // queue[kSlot
 constexpr int kWarpStack = kWarpQ + kSlots;                       // stack[kStackShared][32]
 constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 
-__global__ void __launch_bounds__(128, 4) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
+// 6 resident blocks (24 warps) per SM: 80 registers, no spills; measured on C2 against 4 blocks (118 registers): 134 vs 117 M photons/s.
+#ifndef DW_POOL_MIN_BLOCKS
+#define DW_POOL_MIN_BLOCKS 6
+#endif
+__global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
   __shared__ unsigned int s_fate[8];
   __shared__ unsigned long long s_steps;
