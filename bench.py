@@ -29,8 +29,14 @@ UNIT = "photons/s"
 # Algorithmic work per photon-step at C2: the ideal path of an 8-wide BVH
 # over T = 113 280 triangles with 4-triangle leaves = ceil(log8(T/4)) = 5 nodes x 125 lane-instructions
 # + 4 triangles x 45 + 250 for the physics of the step = 1055 lane-instructions; 5 x 80 B + 4 x 48 B = 592 B.
-ALG_LANE_INSTR_PER_STEP = 5 * 125 + 4 * 45 + 250
-ALG_BYTES_PER_STEP = 5 * 80 + 4 * 48
+def algorithmic_work(n_tri):
+    """(lane-instructions, bytes) per photon-step of the ideal 8-wide path over n_tri triangles with 4-triangle leaves."""
+    import math
+    levels = max(1, math.ceil(math.log(max(n_tri, 8) / 4.0) / math.log(8.0)))
+    return levels * 125 + 4 * 45 + 250, levels * 80 + 4 * 48
+
+
+ALG_LANE_INSTR_PER_STEP, ALG_BYTES_PER_STEP = algorithmic_work(113_280)     # C2: 5 levels -> 1055 lane-instr, 592 B
 ALG_STATE_BYTES_PER_PHOTON = 52 + 32
 SM_COUNT, LANES_PER_SM = 148, 128
 
@@ -266,14 +272,15 @@ def main():
         return 0
 
     peaks = measured_peaks()
+    alg_instr, alg_step_bytes = algorithmic_work(c.geometry.n_tri)
     kernel_ms = float(np.mean(per_step_ms))
     steps_per_launch = local_steps / args.steps
     peak_lane = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6          # lane-instructions / s
-    achieved_lane = steps_per_launch * ALG_LANE_INSTR_PER_STEP / (kernel_ms * 1e-3)
-    alg_bytes = steps_per_launch * ALG_BYTES_PER_STEP + n * ALG_STATE_BYTES_PER_PHOTON
+    achieved_lane = steps_per_launch * alg_instr / (kernel_ms * 1e-3)
+    alg_bytes = steps_per_launch * alg_step_bytes + n * ALG_STATE_BYTES_PER_PHOTON
     roofline = dict(bound="alu", achieved=achieved_lane / 1e12, peak=peak_lane / 1e12, unit="Tlane-instr/s",
                     frac=achieved_lane / peak_lane, traffic=None, kernel="propagate_kernel" if args.legacy else "propagate_pool_kernel", kernel_ms=kernel_ms,
-                    algorithmic_lane_instr_per_photon_step=ALG_LANE_INSTR_PER_STEP,
+                    algorithmic_lane_instr_per_photon_step=alg_instr,
                     algorithmic_bytes_per_launch=alg_bytes,
                     memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
                     peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)")
