@@ -185,6 +185,8 @@ def main():
     ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
     ap.add_argument("--max-leaf", type=int, default=0, help="triangles per BVH leaf (0 = library default)")
     ap.add_argument("--ploc-radius", type=int, default=0, help="search radius of the BVH clustering rounds (0 = library default)")
+    ap.add_argument("--grid-res", type=int, default=0, help="cells per axis of the empty-space grid (0 = default, -1 = none)")
+    ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
@@ -207,14 +209,14 @@ def main():
     ctx = dw.Context(local)
     ctx.set_optics(c.optics)
     ctx.set_geometry(c.geometry)
-    stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius)
+    stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res)
     id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
     ph = c.make_photons(n, id_base)
     d_ph = dw.DevicePhotons(ph, dev)
     out = dw.DeviceResults(n, ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), dev)   # 32 B / photon
     hist = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0, dev)
     stream = torch.cuda.current_stream()
-    flags = (dw.PROP_UNBOUNDED_QUERY if args.literal else 0) | (dw.PROP_LEGACY_SCHEDULER if args.legacy else 0)
+    flags = (dw.PROP_UNBOUNDED_QUERY if args.literal else 0) | (dw.PROP_LEGACY_SCHEDULER if args.legacy else 0) | (dw.PROP_NO_EMPTY_SKIP if args.no_skip else 0)
 
     def step():
         ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream, th_phys=args.th_phys,
@@ -302,7 +304,8 @@ def main():
                             seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
                             mode="literal" if args.literal else "bounded rays",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
-                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], launch=ctx.last_launch()),
+                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"],
+                            grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch()),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},

@@ -100,7 +100,8 @@ int dw_set_geometry(dw_ctx* ctx, int64_t n_vert, const float* xyz, int64_t n_tri
 typedef struct dw_build_params {
   int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (4) */
   int32_t ploc_radius;   /* 1..256, search radius of the clustering rounds in Morton order; 0 = default (16) */
-  int32_t reserved[6];
+  int32_t grid_res;      /* 8..128, cells per axis of the empty-space grid; 0 = default (64); -1 = no grid */
+  int32_t reserved[5];
 } dw_build_params;
 
 typedef struct dw_build_stats {
@@ -110,6 +111,8 @@ typedef struct dw_build_stats {
   float build_ms; /* device time of the whole build */
   int32_t ploc_rounds;  /* clustering rounds executed */
   int32_t binary_depth; /* depth of the binary tree before the collapse into 4-wide nodes */
+  int32_t grid_res;        /* cells per axis of the empty-space grid actually built (0 = none) */
+  int32_t grid_free_cells; /* cells that got a triangle-free box */
 } dw_build_stats;
 
 /* Device LBVH build: triangle boxes -> scene bounds -> 63-bit Morton codes of the centroids -> radix sort ->
@@ -178,7 +181,9 @@ enum {
   DW_PROP_UNBOUNDED_QUERY = 1u,
   /* Diagnostic: run the first-generation kernel (photon state in registers, one photon per lane, physics and
    * traversal phases chosen per warp) instead of the pool scheduler.  Same results photon by photon. */
-  DW_PROP_LEGACY_SCHEDULER = 2u
+  DW_PROP_LEGACY_SCHEDULER = 2u,
+  /* Diagnostic: never answer a bounded query from the empty-space grid (every query is traversed).  Same results. */
+  DW_PROP_NO_EMPTY_SKIP = 4u
 };
 
 /* The propagation loop S1..S13 for every photon of the batch, at most max_steps iterations each.

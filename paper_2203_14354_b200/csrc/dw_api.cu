@@ -47,8 +47,8 @@ extern "C" int dw_create(int cuda_device, dw_ctx** out) {
 static void free_geometry(dw_ctx* c) {
   cudaFree(c->d_xyz); cudaFree(c->d_idx); cudaFree(c->d_code); cudaFree(c->d_chan);
   c->d_xyz = nullptr; c->d_idx = nullptr; c->d_code = nullptr; c->d_chan = nullptr;
-  cudaFree(c->d_nodes); cudaFree(c->d_tris);
-  c->d_nodes = nullptr; c->d_tris = nullptr;
+  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
+  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr;
   c->have_geom = false; c->built = false;
 }
 

@@ -268,7 +268,80 @@ __global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const
   o[2] = make_float4(e2[2], __int_as_float(t), __uint_as_float(code[t]), __int_as_float(chan[t]));
 }
 
+
+// ---- empty-space grid.  G^3 cells over the scene box.  A cell is OCCUPIED if the box of any
+// triangle, grown by `margin`, overlaps it.  Every free cell gets one axis-aligned box of free cells that contains it
+// (grown greedily, one layer of cells at a time, faces in turn); a ray segment whose two ends lie in that box cannot touch
+// a triangle, so the propagation kernel answers such a query without traversal.  Conservative by construction: margin is
+// larger than every tolerance the traversal uses (edge slack, eps_len, fp32 rounding of the end point).
+__global__ void grid_mark_kernel(int n, const float* __restrict__ tlo, const float* __restrict__ thi, float3 glo, float3 inv_cs,
+                                 float margin, int G, int* __restrict__ occ) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  int c0[3], c1[3];
+  const float g[3] = {glo.x, glo.y, glo.z}, ic[3] = {inv_cs.x, inv_cs.y, inv_cs.z};
+  for (int a = 0; a < 3; ++a) {
+    float lo = (tlo[3 * (int64_t)t + a] - margin - g[a]) * ic[a], hi = (thi[3 * (int64_t)t + a] + margin - g[a]) * ic[a];
+    c0[a] = min(max((int)floorf(lo), 0), G - 1);
+    c1[a] = min(max((int)floorf(hi), 0), G - 1);
+  }
+  for (int k = c0[2]; k <= c1[2]; ++k)
+    for (int j = c0[1]; j <= c1[1]; ++j)
+      for (int i = c0[0]; i <= c1[0]; ++i) occ[(k * G + j) * G + i] = 1;
+}
+
+// Summed-area table S[(k+1),(j+1),(i+1)] = number of occupied cells in [0..i] x [0..j] x [0..k]; borders are zero.
+__global__ void sat_x_kernel(int G, const int* __restrict__ occ, int* __restrict__ S) {
+  int id = blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= G * G) return;
+  int j = id % G, k = id / G, P = G + 1, run = 0;
+  for (int i = 0; i < G; ++i) { run += occ[(k * G + j) * G + i]; S[((k + 1) * P + (j + 1)) * P + (i + 1)] = run; }
+}
+__global__ void sat_y_kernel(int G, int* __restrict__ S) {
+  int id = blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= G * G) return;
+  int i = id % G, k = id / G, P = G + 1, run = 0;
+  for (int j = 0; j < G; ++j) { int* p = &S[((k + 1) * P + (j + 1)) * P + (i + 1)]; run += *p; *p = run; }
+}
+__global__ void sat_z_kernel(int G, int* __restrict__ S) {
+  int id = blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= G * G) return;
+  int i = id % G, j = id / G, P = G + 1, run = 0;
+  for (int k = 0; k < G; ++k) { int* p = &S[((k + 1) * P + (j + 1)) * P + (i + 1)]; run += *p; *p = run; }
+}
+__device__ __forceinline__ int sat_sum(const int* __restrict__ S, int P, int x0, int x1, int y0, int y1, int z0, int z1) {
+  auto at = [&](int k, int j, int i) { return S[(k * P + j) * P + i]; };
+  return at(z1 + 1, y1 + 1, x1 + 1) - at(z0, y1 + 1, x1 + 1) - at(z1 + 1, y0, x1 + 1) - at(z1 + 1, y1 + 1, x0) +
+         at(z0, y0, x1 + 1) + at(z0, y1 + 1, x0) + at(z1 + 1, y0, x0) - at(z0, y0, x0);
+}
+// cells[c] = (x0 | x1<<8 | y0<<16 | y1<<24, z0 | z1<<8 | valid<<16): inclusive cell bounds of the free box of cell c.
+__global__ void grid_grow_kernel(int G, const int* __restrict__ occ, const int* __restrict__ S, uint2* __restrict__ cells,
+                                 int* __restrict__ n_free) {
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= G * G * G) return;
+  if (occ[c]) { cells[c] = make_uint2(0u, 0u); return; }
+  const int P = G + 1;
+  int b[6] = {c % G, c % G, (c / G) % G, (c / G) % G, c / (G * G), c / (G * G)};   // x0 x1 y0 y1 z0 z1
+  bool grew = true;
+  while (grew) {
+    grew = false;
+    for (int f = 0; f < 6; ++f) {
+      const bool low = (f & 1) == 0;
+      if (low ? b[f] == 0 : b[f] == G - 1) continue;
+      int s[6] = {b[0], b[1], b[2], b[3], b[4], b[5]};
+      const int layer = low ? b[f] - 1 : b[f] + 1;
+      s[f & ~1] = layer; s[f | 1] = layer;                                         // the one-cell layer next to face f
+      if (sat_sum(S, P, s[0], s[1], s[2], s[3], s[4], s[5]) == 0) { b[f] = layer; grew = true; }
+    }
+  }
+  cells[c] = make_uint2((unsigned)b[0] | (unsigned)b[1] << 8 | (unsigned)b[2] << 16 | (unsigned)b[3] << 24,
+                        (unsigned)b[4] | (unsigned)b[5] << 8 | 1u << 16);
+  atomicAdd(n_free, 1);
+}
+
 }  // namespace
+
+static inline unsigned G_blocks(int64_t n, int B) { return (unsigned)((n + B - 1) / B); }
 
 #define DW_B(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = dw_fail(c, DW_E_CUDA, "%s failed: %s (%s:%d)", \
     #call, cudaGetErrorString(e__), __FILE__, __LINE__); goto done; } } while (0)
@@ -280,8 +353,11 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   const int radius = (params && params->ploc_radius) ? params->ploc_radius : 16;
   if (max_leaf < 1 || max_leaf > 8) return dw_fail(c, DW_E_ARG, "dw_build_bvh: max_leaf_tris must be in 1..8");
   if (radius < 1 || radius > 256) return dw_fail(c, DW_E_ARG, "dw_build_bvh: ploc_radius must be in 1..256");
-  cudaFree(c->d_nodes); cudaFree(c->d_tris);
-  c->d_nodes = nullptr; c->d_tris = nullptr; c->built = false;
+  const int grid_req = params ? params->grid_res : 0;
+  const int GR = grid_req == 0 ? 64 : grid_req;
+  if (grid_req != -1 && (GR < 8 || GR > 128)) return dw_fail(c, DW_E_ARG, "dw_build_bvh: grid_res must be -1, 0 or in 8..128");
+  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
+  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
   if (stats) memset(stats, 0, sizeof *stats);
 
   const size_t N = (size_t)std::max(n, 1), N2 = 2 * N;
@@ -290,7 +366,9 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   unsigned *scene = nullptr, *vals = nullptr, *vals2 = nullptr;
   unsigned long long *keys = nullptr, *keys2 = nullptr;
   int *left = nullptr, *right = nullptr, *parent = nullptr, *size = nullptr, *leftmost = nullptr, *cn[2] = {nullptr, nullptr},
-      *nn = nullptr, *keep = nullptr, *isnew = nullptr, *kpos = nullptr, *npos = nullptr, *slot = nullptr, *misc = nullptr;
+      *nn = nullptr, *keep = nullptr, *isnew = nullptr, *kpos = nullptr, *npos = nullptr, *slot = nullptr, *misc = nullptr,
+      *occ = nullptr, *sat = nullptr;
+  int grid_built = 0, grid_free = 0;
   WideTask* tasks[2] = {nullptr, nullptr};
   void* tmp = nullptr;
   size_t tmp_bytes = 0, tmp2 = 0;
@@ -400,23 +478,56 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
       for (int a = 0; a < 3; ++a) { lo[a] = o2f(h_scene[a]); hi[a] = o2f(h_scene[3 + a]); mx = fmaxf(mx, fmaxf(fabsf(lo[a]), fabsf(hi[a]))); }
     // Length tolerance: a few fp32 spacings of the largest coordinate (positions cannot be resolved finer).
     float eps_len = 4.0f * 1.1920929e-7f * mx;
-    c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len};
+    float tree_ms = 0.f, grid_ms = 0.f;
+    cudaEventElapsedTime(&tree_ms, ev0, ev1);                                     // before the events are reused below
+    c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len, nullptr, 0, make_float3(0, 0, 0), make_float3(0, 0, 0), make_float3(0, 0, 0)};
+    // ---- empty-space grid over the scene box (skipped for an empty or flat world)
+    float ext[3] = {hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]};
+    const float emax = fmaxf(ext[0], fmaxf(ext[1], ext[2]));
+    if (grid_req != -1 && n > 0 && emax > 0.f) {
+      for (int a = 0; a < 3; ++a) ext[a] = fmaxf(ext[a], 1e-3f * emax);           // a flat axis still gets cells of finite size
+      const float3 glo = make_float3(lo[0], lo[1], lo[2]);
+      const float3 cs = make_float3(ext[0] / GR, ext[1] / GR, ext[2] / GR);
+      const float3 ics = make_float3(GR / ext[0], GR / ext[1], GR / ext[2]);
+      // margin > edge slack (2e-6 x longest edge <= 15 eps_len) + eps_len of t_max + fp32 rounding of the segment end
+      const float margin = 32.0f * eps_len;
+      const int G3 = GR * GR * GR, P = GR + 1;
+      DW_B(cudaMalloc(&occ, 4 * (size_t)G3)); DW_B(cudaMalloc(&sat, 4 * (size_t)P * P * P));
+      DW_B(cudaMalloc(&c->d_cells, sizeof(uint2) * (size_t)G3));
+      DW_B(cudaMemsetAsync(occ, 0, 4 * (size_t)G3, stream));
+      DW_B(cudaMemsetAsync(sat, 0, 4 * (size_t)P * P * P, stream));
+      DW_B(cudaMemsetAsync(misc, 0, 4, stream));
+      DW_B(cudaEventRecord(ev0, stream));
+      grid_mark_kernel<<<G_blocks(n, B), B, 0, stream>>>(n, tlo, thi, glo, ics, margin, GR, occ);
+      sat_x_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, occ, sat);
+      sat_y_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
+      sat_z_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
+      grid_grow_kernel<<<G_blocks(G3, B), B, 0, stream>>>(GR, occ, sat, c->d_cells, misc);
+      DW_B(cudaGetLastError());
+      DW_B(cudaEventRecord(ev1, stream));
+      DW_B(cudaMemcpyAsync(&grid_free, misc, 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaStreamSynchronize(stream));
+      cudaEventElapsedTime(&grid_ms, ev0, ev1);
+      grid_built = GR;
+      c->bvh.cells = c->d_cells; c->bvh.grid_n = GR; c->bvh.grid_lo = glo; c->bvh.grid_cs = cs; c->bvh.grid_inv_cs = ics;
+    }
     c->built = true;
     if (stats) {
       stats->n_tri = n; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
       stats->max_depth = wide_depth; stats->n_leaves = h_misc[2];
       for (int a = 0; a < 3; ++a) { stats->scene_lo[a] = lo[a]; stats->scene_hi[a] = hi[a]; }
-      cudaEventElapsedTime(&stats->build_ms, ev0, ev1);
+      stats->build_ms = tree_ms + grid_ms;
       stats->ploc_rounds = ploc_rounds; stats->binary_depth = h_misc[3];
+      stats->grid_res = grid_built; stats->grid_free_cells = grid_free;
     }
   }
 done:
   cudaFree(tlo); cudaFree(thi); cudaFree(blo); cudaFree(bhi); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
   cudaFree(vals2); cudaFree(left); cudaFree(right); cudaFree(parent); cudaFree(size); cudaFree(leftmost); cudaFree(nn);
-  cudaFree(keep); cudaFree(isnew); cudaFree(kpos); cudaFree(npos); cudaFree(slot); cudaFree(misc); cudaFree(tmp); cudaFree(nodes_tmp);
+  cudaFree(keep); cudaFree(isnew); cudaFree(kpos); cudaFree(npos); cudaFree(slot); cudaFree(misc); cudaFree(tmp); cudaFree(nodes_tmp); cudaFree(occ); cudaFree(sat);
   for (int k = 0; k < 2; ++k) { cudaFree(cl[k]); cudaFree(ch[k]); cudaFree(cn[k]); cudaFree(tasks[k]); }
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
-  if (rc != DW_OK) { cudaFree(c->d_nodes); cudaFree(c->d_tris); c->d_nodes = nullptr; c->d_tris = nullptr; c->built = false; }
+  if (rc != DW_OK) { cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells); c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false; }
   return rc;
 }

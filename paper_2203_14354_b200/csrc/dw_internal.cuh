@@ -8,7 +8,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 101
+#define DW_VERSION 102
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
@@ -43,6 +43,10 @@ struct DwBvh {
   int n_nodes;
   int n_tri;
   float eps_len;        // length tolerance tied to the fp32 spacing of the scene coordinates
+  // empty-space grid (nullptr = none): cells[(z*G+y)*G+x] = inclusive cell bounds of a triangle-free box around the cell
+  const uint2* cells;
+  int grid_n;
+  float3 grid_lo, grid_cs, grid_inv_cs;
 };
 
 struct dw_ctx {
@@ -64,6 +68,7 @@ struct dw_ctx {
   // BVH
   float4* d_nodes = nullptr;
   float4* d_tris = nullptr;
+  uint2* d_cells = nullptr;
   DwBvh bvh{};
   bool built = false;
   // launch record

@@ -576,6 +576,7 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
   const int64_t n = A.in.n;
   const bool literal = (A.flags & DW_PROP_UNBOUNDED_QUERY) != 0;
   const int th_fetch = A.th_phys, th_leaf = A.th_leaf;
+  const bool use_grid = A.bvh.cells != nullptr && !(A.flags & DW_PROP_NO_EMPTY_SKIP);
 
   int64_t w_next = 0, w_end = 0;     // warp-private range of photon indices
   bool exhausted = false;
@@ -754,6 +755,7 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
           fate = DW_FATE_NAN_ABORT;                                   // S11
         } else {
           float tmax = INFINITY;
+          bool skip = false;
           if ((!literal) && medium >= 0) {                            // medium known: S3/S4 draws before the query
             float4 r0 = draw4(A.seed, pid, step, 0u);
             us = r0.z; uf = r0.w;
@@ -764,6 +766,27 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
             absorb_first = da < ds;
             dbulk = fminf(da, ds);
             tmax = dbulk + A.bvh.eps_len;
+            // empty boxes: if the whole segment lies in the triangle-free box of the origin's cell, the answer is "no hit"
+            if (use_grid) {
+              const float fx = (x.x - A.bvh.grid_lo.x) * A.bvh.grid_inv_cs.x, fy = (x.y - A.bvh.grid_lo.y) * A.bvh.grid_inv_cs.y,
+                          fz = (x.z - A.bvh.grid_lo.z) * A.bvh.grid_inv_cs.z;
+              const int G = A.bvh.grid_n;
+              const int cx = (int)floorf(fx), cy = (int)floorf(fy), cz = (int)floorf(fz);
+              if (cx >= 0 && cy >= 0 && cz >= 0 && cx < G && cy < G && cz < G) {
+                const uint2 cb = __ldg(&A.bvh.cells[(cz * G + cy) * G + cx]);
+                if (cb.y >> 16) {
+                  const V3 blo = mk(fmaf((float)(cb.x & 0xFF), A.bvh.grid_cs.x, A.bvh.grid_lo.x),
+                                    fmaf((float)((cb.x >> 16) & 0xFF), A.bvh.grid_cs.y, A.bvh.grid_lo.y),
+                                    fmaf((float)(cb.y & 0xFF), A.bvh.grid_cs.z, A.bvh.grid_lo.z));
+                  const V3 bhi = mk(fmaf((float)(((cb.x >> 8) & 0xFF) + 1), A.bvh.grid_cs.x, A.bvh.grid_lo.x),
+                                    fmaf((float)(((cb.x >> 24) & 0xFF) + 1), A.bvh.grid_cs.y, A.bvh.grid_lo.y),
+                                    fmaf((float)(((cb.y >> 8) & 0xFF) + 1), A.bvh.grid_cs.z, A.bvh.grid_lo.z));
+                  const V3 p1 = fma3(tmax, k, x);
+                  skip = x.x >= blo.x && x.x <= bhi.x && x.y >= blo.y && x.y <= bhi.y && x.z >= blo.z && x.z <= bhi.z &&
+                         p1.x >= blo.x && p1.x <= bhi.x && p1.y >= blo.y && p1.y <= bhi.y && p1.z >= blo.z && p1.z <= bhi.z;
+                }
+              }
+            }
           }
           poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
           poolf[W_KX * kSlots + slot] = k.x; poolf[W_KY * kSlots + slot] = k.y; poolf[W_KZ * kSlots + slot] = k.z;
@@ -781,7 +804,7 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
           poolf[W_UF * kSlots + slot] = uf;
           poolf[W_BEST_T * kSlots + slot] = tmax;                     // the query starts from t_max
           pool[W_BEST_SLOT * kSlots + slot] = -1;
-          st[slot] = S_TRACE;
+          st[slot] = skip ? S_PHYS : S_TRACE;                         // a skipped query is already finished: no hit
         }
       }
 

@@ -546,3 +546,18 @@ def test_pool_scheduler_bit_identical_to_legacy(cfg, n, mode):
     for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
         assert np.array_equal(a[key], b[key]), f"C{cfg} mode {mode}: '{key}' differs between schedulers"
     assert int(a["fate_count"].sum()) == n
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 400_000), (2, 400_000), (3, 400_000), (4, 200_000)])
+def test_empty_space_skip_is_invisible(cfg, n):
+    """a bounded query whose segment lies in the triangle-free box of its origin cell is answered
+    'no hit' without traversal.  That is exactly what traversal returns, so every per-photon output and every reduction must
+    be bit-identical with the skip switched off -- also next to the 0.1 mm wires of C3/C4, where a margin that is too
+    small would show first."""
+    c, ctx = ctx_for(cfg)
+    assert ctx.stats["grid_res"] == 64 and ctx.stats["grid_free_cells"] > 0
+    ph = c.make_photons(n)
+    a = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=200, dt=2.0)
+    b = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=200, dt=2.0, flags=dw.PROP_NO_EMPTY_SKIP)
+    for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
+        assert np.array_equal(a[key], b[key]), f"C{cfg}: '{key}' changes when queries are skipped"
