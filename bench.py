@@ -185,6 +185,7 @@ def main():
     ap.add_argument("--literal", action="store_true", help="DW_PROP_UNBOUNDED_QUERY (the oracle's literal loop)")
     ap.add_argument("--max-leaf", type=int, default=0, help="triangles per BVH leaf (0 = library default)")
     ap.add_argument("--ploc-radius", type=int, default=0, help="search radius of the BVH clustering rounds (0 = library default)")
+    ap.add_argument("--split-div", type=int, default=0, help="split triangles longer than scene extent / this (0 = default, -1 = never)")
     ap.add_argument("--grid-res", type=int, default=0, help="cells per axis of the empty-space grid (0 = default, -1 = none)")
     ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
@@ -209,7 +210,7 @@ def main():
     ctx = dw.Context(local)
     ctx.set_optics(c.optics)
     ctx.set_geometry(c.geometry)
-    stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res)
+    stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res, split_div=args.split_div)
     id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
     ph = c.make_photons(n, id_base)
     d_ph = dw.DevicePhotons(ph, dev)
@@ -304,7 +305,7 @@ def main():
                             seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
                             mode="literal" if args.literal else "bounded rays",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
-                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"],
+                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch()),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),

@@ -101,7 +101,10 @@ typedef struct dw_build_params {
   int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (4) */
   int32_t ploc_radius;   /* 1..256, search radius of the clustering rounds in Morton order; 0 = default (16) */
   int32_t grid_res;      /* 8..128, cells per axis of the empty-space grid; 0 = default (64); -1 = no grid */
-  int32_t reserved[5];
+  int32_t split_div;     /* a triangle longer than (largest scene extent) / split_div gets several box references;
+                          * 1..4096; 0 = default (32); -1 = never split.  Halved automatically while the references
+                          * would exceed 2 n_tri + 65536. */
+  int32_t reserved[4];
 } dw_build_params;
 
 typedef struct dw_build_stats {
@@ -113,6 +116,8 @@ typedef struct dw_build_stats {
   int32_t binary_depth; /* depth of the binary tree before the collapse into 4-wide nodes */
   int32_t grid_res;        /* cells per axis of the empty-space grid actually built (0 = none) */
   int32_t grid_free_cells; /* cells that got a triangle-free box */
+  int32_t n_refs;          /* box references the tree is built over (>= n_tri); tri_bytes = 48 * n_refs */
+  int32_t split_div;       /* divisor actually used (0 = nothing was split) */
 } dw_build_stats;
 
 /* Device LBVH build: triangle boxes -> scene bounds -> 63-bit Morton codes of the centroids -> radix sort ->

@@ -31,13 +31,13 @@ vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_
 
 
 class BuildParams(C.Structure):
-    _fields_ = [("max_leaf_tris", i32), ("ploc_radius", i32), ("grid_res", i32), ("reserved", i32 * 5)]
+    _fields_ = [("max_leaf_tris", i32), ("ploc_radius", i32), ("grid_res", i32), ("split_div", i32), ("reserved", i32 * 4)]
 
 
 class BuildStats(C.Structure):
     _fields_ = [("n_tri", i64), ("n_nodes", i64), ("node_bytes", i64), ("tri_bytes", i64), ("max_depth", i32),
                 ("n_leaves", i32), ("scene_lo", f32 * 3), ("scene_hi", f32 * 3), ("build_ms", f32),
-                ("ploc_rounds", i32), ("binary_depth", i32), ("grid_res", i32), ("grid_free_cells", i32)]
+                ("ploc_rounds", i32), ("binary_depth", i32), ("grid_res", i32), ("grid_free_cells", i32), ("n_refs", i32), ("split_div", i32)]
 
 
 class Photons(C.Structure):
@@ -178,8 +178,8 @@ class Context:
                                            _dp(mat_outer), _dp(surface), _dp(channel), 1))
         self.n_chan = int(n_channels)
 
-    def build_bvh(self, max_leaf_tris: int = 0, stream=None, ploc_radius: int = 0, grid_res: int = 0) -> dict:
-        p = BuildParams(max_leaf_tris=max_leaf_tris, ploc_radius=ploc_radius, grid_res=grid_res)
+    def build_bvh(self, max_leaf_tris: int = 0, stream=None, ploc_radius: int = 0, grid_res: int = 0, split_div: int = 0) -> dict:
+        p = BuildParams(max_leaf_tris=max_leaf_tris, ploc_radius=ploc_radius, grid_res=grid_res, split_div=split_div)
         st = BuildStats()
         self._check(self.L.dw_build_bvh(self.h, C.byref(p), C.byref(st), _stream_ptr(stream)))
         self.stats = {k: (list(getattr(st, k)) if k.startswith("scene") else getattr(st, k)) for k, _ in BuildStats._fields_}

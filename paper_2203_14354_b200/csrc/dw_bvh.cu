@@ -50,6 +50,120 @@ __global__ void tri_bounds_kernel(int n, const float* __restrict__ xyz, const in
   }
 }
 
+// ---- triangle references.  A triangle whose box is longer than smax = (largest scene extent) / split_div is represented by
+// several references, each with the tight box of the part of the triangle inside a sub-box (clip, bound, halve the longest
+// axis, repeat): the long slivers of fans and the tall wall panels otherwise give leaf boxes that overlap over metres and
+// most triangle tests are misses (profiles/r01_propagate_bvh4_c2.md, capture 5).  A reference is only a box: leaves hold
+// the whole triangle, so a triangle can be tested twice by one ray, which the first-hit rule (nearest, then lowest id)
+// does not notice.  The union of the boxes of a triangle covers it; boxes are padded by `pad`.
+constexpr int kClipMax = 10;      // a triangle clipped by an axis-aligned box has at most 9 vertices
+constexpr int kSplitStack = 24;
+
+// Sutherland-Hodgman against one axis plane: keep coordinate[axis] >= val (keep_ge) or <= val.
+__device__ int clip_axis(const float (*in)[3], int n, int axis, float val, bool keep_ge, float (*out)[3]) {
+  int m = 0;
+  for (int i = 0; i < n; ++i) {
+    const float* a = in[i];
+    const float* b = in[(i + 1 == n) ? 0 : i + 1];
+    const bool ia = keep_ge ? a[axis] >= val : a[axis] <= val;
+    const bool ib = keep_ge ? b[axis] >= val : b[axis] <= val;
+    if (ia && m < kClipMax) { out[m][0] = a[0]; out[m][1] = a[1]; out[m][2] = a[2]; ++m; }
+    if (ia != ib && m < kClipMax) {
+      const float w = (val - a[axis]) / (b[axis] - a[axis]);
+      for (int c = 0; c < 3; ++c) out[m][c] = fmaf(w, b[c] - a[c], a[c]);
+      out[m][axis] = val;
+      ++m;
+    }
+  }
+  return m;
+}
+
+// References of one triangle.  out_lo / out_hi == nullptr: count only.  Returns the number of references.
+__device__ int split_triangle(const float v[3][3], const float tlo[3], const float thi[3], float smax, float pad,
+                              float* out_lo, float* out_hi) {
+  float ext = fmaxf(thi[0] - tlo[0], fmaxf(thi[1] - tlo[1], thi[2] - tlo[2]));
+  if (!(ext > smax)) {
+    if (out_lo) for (int c = 0; c < 3; ++c) { out_lo[c] = tlo[c]; out_hi[c] = thi[c]; }
+    return 1;
+  }
+  float slo[kSplitStack][3], shi[kSplitStack][3];
+  float pa[kClipMax][3], pb[kClipMax][3];
+  int sp = 0, cnt = 0;
+  for (int c = 0; c < 3; ++c) { slo[0][c] = tlo[c]; shi[0][c] = thi[c]; }
+  sp = 1;
+  for (int iter = 0; iter < 8192 && sp > 0; ++iter) {
+    --sp;
+    float blo[3] = {slo[sp][0], slo[sp][1], slo[sp][2]}, bhi[3] = {shi[sp][0], shi[sp][1], shi[sp][2]};
+    int np = 3;
+    for (int i = 0; i < 3; ++i) for (int c = 0; c < 3; ++c) pa[i][c] = v[i][c];
+    for (int axis = 0; axis < 3 && np > 0; ++axis) {
+      np = clip_axis(pa, np, axis, blo[axis], true, pb);
+      if (np > 0) np = clip_axis(pb, np, axis, bhi[axis], false, pa);
+    }
+    if (np == 0) continue;                                       // this sub-box holds nothing of the triangle
+    float lo[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, hi[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+    for (int i = 0; i < np; ++i) for (int c = 0; c < 3; ++c) { lo[c] = fminf(lo[c], pa[i][c]); hi[c] = fmaxf(hi[c], pa[i][c]); }
+    for (int c = 0; c < 3; ++c) { lo[c] = fmaxf(lo[c], blo[c]); hi[c] = fminf(hi[c], bhi[c]); }
+    int ax = 0;
+    float e = hi[0] - lo[0];
+    if (hi[1] - lo[1] > e) { e = hi[1] - lo[1]; ax = 1; }
+    if (hi[2] - lo[2] > e) { e = hi[2] - lo[2]; ax = 2; }
+    if (e <= smax || sp + 2 > kSplitStack) {
+      if (out_lo) for (int c = 0; c < 3; ++c) { out_lo[3 * cnt + c] = lo[c] - pad; out_hi[3 * cnt + c] = hi[c] + pad; }
+      ++cnt;
+      continue;
+    }
+    const float mid = 0.5f * (lo[ax] + hi[ax]);
+    for (int c = 0; c < 3; ++c) { slo[sp][c] = lo[c]; shi[sp][c] = hi[c]; slo[sp + 1][c] = lo[c]; shi[sp + 1][c] = hi[c]; }
+    shi[sp][ax] = mid; slo[sp + 1][ax] = mid;
+    sp += 2;
+  }
+  if (cnt == 0) {                                                // rounding clipped everything away: one reference, the whole box
+    if (out_lo) for (int c = 0; c < 3; ++c) { out_lo[c] = tlo[c] - pad; out_hi[c] = thi[c] + pad; }
+    cnt = 1;
+  }
+  return cnt;
+}
+
+__device__ __forceinline__ void load_tri(const float* __restrict__ xyz, const int32_t* __restrict__ idx, int t, float v[3][3]) {
+  for (int k = 0; k < 3; ++k) {
+    const int vi = idx[3 * (int64_t)t + k];
+    for (int c = 0; c < 3; ++c) v[k][c] = xyz[3 * (int64_t)vi + c];
+  }
+}
+__device__ __forceinline__ float split_smax(const unsigned* __restrict__ scene, int split_div) {
+  if (split_div <= 0) return FLT_MAX;
+  const float e = fmaxf(o2f(scene[3]) - o2f(scene[0]), fmaxf(o2f(scene[4]) - o2f(scene[1]), o2f(scene[5]) - o2f(scene[2])));
+  return e / (float)split_div;
+}
+__global__ void split_count_kernel(int n, const float* __restrict__ xyz, const int32_t* __restrict__ idx,
+                                   const float* __restrict__ tlo, const float* __restrict__ thi,
+                                   const unsigned* __restrict__ scene, int split_div, int* __restrict__ counts) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  float v[3][3];
+  load_tri(xyz, idx, t, v);
+  counts[t] = split_triangle(v, tlo + 3 * (int64_t)t, thi + 3 * (int64_t)t, split_smax(scene, split_div), 0.f, nullptr, nullptr);
+}
+__global__ void split_emit_kernel(int n, const float* __restrict__ xyz, const int32_t* __restrict__ idx,
+                                  const float* __restrict__ tlo, const float* __restrict__ thi,
+                                  const unsigned* __restrict__ scene, int split_div, float pad, const int* __restrict__ offs,
+                                  const int* __restrict__ counts, float* __restrict__ rlo, float* __restrict__ rhi,
+                                  int* __restrict__ ref_tri) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  float v[3][3];
+  load_tri(xyz, idx, t, v);
+  const int o = offs[t], cnt = counts[t];
+  const int made = split_triangle(v, tlo + 3 * (int64_t)t, thi + 3 * (int64_t)t, split_smax(scene, split_div), cnt > 1 ? pad : 0.f,
+                                  rlo + 3 * (int64_t)o, rhi + 3 * (int64_t)o);
+  for (int k = 0; k < cnt; ++k) {
+    ref_tri[o + k] = t;
+    if (k >= made)                                               // cannot happen (same arithmetic as the count pass); keep the box valid
+      for (int c = 0; c < 3; ++c) { rlo[3 * (int64_t)(o + k) + c] = tlo[3 * (int64_t)t + c]; rhi[3 * (int64_t)(o + k) + c] = thi[3 * (int64_t)t + c]; }
+  }
+}
+
 __device__ __forceinline__ unsigned long long spread21(unsigned long long x) {
   x &= 0x1fffffull;
   x = (x | x << 32) & 0x1f00000000ffffull;
@@ -248,13 +362,13 @@ __global__ void wide_single_kernel(int n, const float4* __restrict__ blo, const 
 }
 
 // triangle j of the Morton order goes to depth-first slot[j]
-__global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const int* __restrict__ slot,
+__global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const int* __restrict__ ref_tri, const int* __restrict__ slot,
                                  const float* __restrict__ xyz, const int32_t* __restrict__ idx,
                                  const uint32_t* __restrict__ code, const int32_t* __restrict__ chan,
                                  float4* __restrict__ tris) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
-  int t = vals[j];
+  int t = ref_tri[vals[j]];                  // reference -> triangle (several references may share one)
   int i0 = idx[3 * (int64_t)t], i1 = idx[3 * (int64_t)t + 1], i2 = idx[3 * (int64_t)t + 2];
   float v0[3], e1[3], e2[3];
   for (int a = 0; a < 3; ++a) {
@@ -348,27 +462,33 @@ static inline unsigned G_blocks(int64_t n, int B) { return (unsigned)((n + B - 1
 
 int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* stats, cudaStream_t stream) {
   int rc = DW_OK;
-  const int n = (int)c->n_tri;
+  const int nt = (int)c->n_tri;     // triangles
+  int n = nt;                       // references (>= nt once long triangles are split): what the tree is built over
   const int max_leaf = (params && params->max_leaf_tris) ? params->max_leaf_tris : 4;
   const int radius = (params && params->ploc_radius) ? params->ploc_radius : 16;
   if (max_leaf < 1 || max_leaf > 8) return dw_fail(c, DW_E_ARG, "dw_build_bvh: max_leaf_tris must be in 1..8");
   if (radius < 1 || radius > 256) return dw_fail(c, DW_E_ARG, "dw_build_bvh: ploc_radius must be in 1..256");
   const int grid_req = params ? params->grid_res : 0;
   const int GR = grid_req == 0 ? 64 : grid_req;
+  const int split_req = params ? params->split_div : 0;
+  const int split_div = split_req == 0 ? 32 : split_req;
+  if (split_req != -1 && (split_div < 1 || split_div > 4096)) return dw_fail(c, DW_E_ARG, "dw_build_bvh: split_div must be -1, 0 or in 1..4096");
   if (grid_req != -1 && (GR < 8 || GR > 128)) return dw_fail(c, DW_E_ARG, "dw_build_bvh: grid_res must be -1, 0 or in 8..128");
   cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
   c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
   if (stats) memset(stats, 0, sizeof *stats);
 
-  const size_t N = (size_t)std::max(n, 1), N2 = 2 * N;
-  float *tlo = nullptr, *thi = nullptr;
+  size_t N = 0, N2 = 0;             // set after stage 0
+  const size_t NT = (size_t)std::max(nt, 1);
+  float *tlo = nullptr, *thi = nullptr, *tlo_t = nullptr, *thi_t = nullptr;   // tlo/thi: boxes of the references; *_t: of the triangles
+  int *counts = nullptr, *offs = nullptr, *ref_tri = nullptr;
   float4 *blo = nullptr, *bhi = nullptr, *cl[2] = {nullptr, nullptr}, *ch[2] = {nullptr, nullptr}, *nodes_tmp = nullptr;
   unsigned *scene = nullptr, *vals = nullptr, *vals2 = nullptr;
   unsigned long long *keys = nullptr, *keys2 = nullptr;
   int *left = nullptr, *right = nullptr, *parent = nullptr, *size = nullptr, *leftmost = nullptr, *cn[2] = {nullptr, nullptr},
       *nn = nullptr, *keep = nullptr, *isnew = nullptr, *kpos = nullptr, *npos = nullptr, *slot = nullptr, *misc = nullptr,
       *occ = nullptr, *sat = nullptr;
-  int grid_built = 0, grid_free = 0;
+  int grid_built = 0, grid_free = 0, split_used = 0;
   WideTask* tasks[2] = {nullptr, nullptr};
   void* tmp = nullptr;
   size_t tmp_bytes = 0, tmp2 = 0;
@@ -377,35 +497,67 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   int h_misc[4] = {0, 0, 0, 0};      // [0] next-level tasks, [1] wide nodes, [2] leaves, [3] binary depth
   int n_nodes = 1, wide_depth = 1, ploc_rounds = 0;
   const int B = 256;
-  const unsigned G = (unsigned)((N + B - 1) / B);
+  unsigned G = 0;
+  const unsigned GT = (unsigned)((NT + B - 1) / B);
 
   DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
-  DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * N)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * N));
+  DW_B(cudaMalloc(&scene, sizeof(unsigned) * 6));
+  DW_B(cudaMalloc(&misc, 16));
+  DW_B(cudaEventRecord(ev0, stream));
+  DW_B(cudaMemsetAsync(misc, 0, 16, stream));
+  // ---- stage 0: triangle boxes, scene bounds, references (long triangles split)
+  DW_B(cudaMalloc(&tlo_t, sizeof(float) * 3 * NT)); DW_B(cudaMalloc(&thi_t, sizeof(float) * 3 * NT));
+  DW_B(cudaMalloc(&counts, 4 * NT)); DW_B(cudaMalloc(&offs, 4 * NT));
+  if (nt > 0) {
+    unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    DW_B(cudaMemcpyAsync(scene, init, sizeof init, cudaMemcpyHostToDevice, stream));
+    tri_bounds_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene);
+    DW_B(cudaMemcpyAsync(h_scene, scene, sizeof h_scene, cudaMemcpyDeviceToHost, stream));
+    DW_B(cudaStreamSynchronize(stream));
+    float mx0 = 0.f;
+    for (int a = 0; a < 6; ++a) mx0 = fmaxf(mx0, fabsf(o2f(h_scene[a])));
+    const float pad = 4.0f * 1.1920929e-7f * mx0;               // = eps_len: boxes of split references are padded by it
+    int div = split_req == -1 ? 0 : split_div;
+    size_t scan_bytes = 0;
+    DW_B(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, counts, offs, nt, stream));
+    DW_B(cudaMalloc(&tmp, scan_bytes));
+    for (;;) {                                                  // coarser splitting if the references would more than double
+      split_count_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene, div, counts);
+      DW_B(cub::DeviceScan::ExclusiveSum(tmp, scan_bytes, counts, offs, nt, stream));
+      int h_last[2];
+      DW_B(cudaMemcpyAsync(&h_last[0], offs + (nt - 1), 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaMemcpyAsync(&h_last[1], counts + (nt - 1), 4, cudaMemcpyDeviceToHost, stream));
+      DW_B(cudaStreamSynchronize(stream));
+      n = h_last[0] + h_last[1];
+      if (div <= 1 || (int64_t)n <= 2 * (int64_t)nt + 65536) break;
+      div /= 2;
+    }
+    split_used = div;
+    DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * (size_t)n)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * (size_t)n));
+    DW_B(cudaMalloc(&ref_tri, 4 * (size_t)n));
+    split_emit_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene, div, pad, offs, counts, tlo, thi, ref_tri);
+    cudaFree(tmp); tmp = nullptr;
+  }
+  N = (size_t)std::max(n, 1); N2 = 2 * N;
+  G = (unsigned)((N + B - 1) / B);
   DW_B(cudaMalloc(&blo, sizeof(float4) * N2)); DW_B(cudaMalloc(&bhi, sizeof(float4) * N2));
   for (int k = 0; k < 2; ++k) {
     DW_B(cudaMalloc(&cl[k], sizeof(float4) * N)); DW_B(cudaMalloc(&ch[k], sizeof(float4) * N)); DW_B(cudaMalloc(&cn[k], 4 * N));
     DW_B(cudaMalloc(&tasks[k], sizeof(WideTask) * N));
   }
-  DW_B(cudaMalloc(&scene, sizeof(unsigned) * 6));
   DW_B(cudaMalloc(&keys, 8 * N)); DW_B(cudaMalloc(&keys2, 8 * N));
   DW_B(cudaMalloc(&vals, 4 * N)); DW_B(cudaMalloc(&vals2, 4 * N));
   DW_B(cudaMalloc(&left, 4 * N2)); DW_B(cudaMalloc(&right, 4 * N2)); DW_B(cudaMalloc(&parent, 4 * N2));
   DW_B(cudaMalloc(&size, 4 * N2)); DW_B(cudaMalloc(&leftmost, 4 * N2));
   DW_B(cudaMalloc(&nn, 4 * N)); DW_B(cudaMalloc(&keep, 4 * N)); DW_B(cudaMalloc(&isnew, 4 * N));
   DW_B(cudaMalloc(&kpos, 4 * N)); DW_B(cudaMalloc(&npos, 4 * N)); DW_B(cudaMalloc(&slot, 4 * N));
-  DW_B(cudaMalloc(&misc, 16));
   DW_B(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)N, 0, 63, stream));
   DW_B(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, keep, kpos, (int)N, stream));
   tmp_bytes = std::max(tmp_bytes, tmp2);
   DW_B(cudaMalloc(&tmp, tmp_bytes));
   DW_B(cudaMalloc(&c->d_tris, 48 * N));
 
-  DW_B(cudaEventRecord(ev0, stream));
-  DW_B(cudaMemsetAsync(misc, 0, 16, stream));
   if (n > 0) {
-    unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
-    DW_B(cudaMemcpyAsync(scene, init, sizeof init, cudaMemcpyHostToDevice, stream));
-    tri_bounds_kernel<<<G, B, 0, stream>>>(n, c->d_xyz, c->d_idx, tlo, thi, scene);
     morton_kernel<<<G, B, 0, stream>>>(n, tlo, thi, scene, keys, vals);
     DW_B(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, n, 0, 63, stream));
     ploc_init_kernel<<<G, B, 0, stream>>>(n, vals2, tlo, thi, blo, bhi, cn[0], cl[0], ch[0], size, parent, leftmost);
@@ -432,7 +584,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     }
     if (base != 2 * n - 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: %d of %d nodes made", base - n, n - 1); goto done; }
     leaf_walk_kernel<<<G, B, 0, stream>>>(n, left, parent, size, slot, leftmost, misc + 3);
-    pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris);
+    pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, ref_tri, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris);
   }
   if (n <= max_leaf) {
     DW_B(cudaMalloc(&c->d_nodes, 128));
@@ -513,7 +665,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     }
     c->built = true;
     if (stats) {
-      stats->n_tri = n; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
+      stats->n_tri = nt; stats->n_refs = n; stats->split_div = split_used; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
       stats->max_depth = wide_depth; stats->n_leaves = h_misc[2];
       for (int a = 0; a < 3; ++a) { stats->scene_lo[a] = lo[a]; stats->scene_hi[a] = hi[a]; }
       stats->build_ms = tree_ms + grid_ms;
@@ -522,7 +674,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     }
   }
 done:
-  cudaFree(tlo); cudaFree(thi); cudaFree(blo); cudaFree(bhi); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
+  cudaFree(tlo); cudaFree(thi); cudaFree(tlo_t); cudaFree(thi_t); cudaFree(counts); cudaFree(offs); cudaFree(ref_tri); cudaFree(blo); cudaFree(bhi); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
   cudaFree(vals2); cudaFree(left); cudaFree(right); cudaFree(parent); cudaFree(size); cudaFree(leftmost); cudaFree(nn);
   cudaFree(keep); cudaFree(isnew); cudaFree(kpos); cudaFree(npos); cudaFree(slot); cudaFree(misc); cudaFree(tmp); cudaFree(nodes_tmp); cudaFree(occ); cudaFree(sat);
   for (int k = 0; k < 2; ++k) { cudaFree(cl[k]); cudaFree(ch[k]); cudaFree(cn[k]); cudaFree(tasks[k]); }

@@ -8,7 +8,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 102
+#define DW_VERSION 103
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
