@@ -8,6 +8,29 @@
 
 namespace {
 
+// Inlining of helpers that are called from many places (profiles/r01_propagate_bvh4_c2.md, capture 6: instruction fetch
+// became the largest stall once the kernel grew to ~2900 instructions).  Level 0: everything inline; 1: Philox out of line;
+// 2: + table look-up; 3: + Rayleigh / Lambert / Fresnel.
+// Measured on C2 (alternating A/B, two rounds): level 0 173.8, 1 175.2, 2 188.6, 3 151.0 M photons/s.
+#ifndef DW_OUTLINE
+#define DW_OUTLINE 2
+#endif
+#if DW_OUTLINE >= 1
+#define DW_INL_PHILOX __noinline__
+#else
+#define DW_INL_PHILOX __forceinline__
+#endif
+#if DW_OUTLINE >= 2
+#define DW_INL_TABLE __noinline__
+#else
+#define DW_INL_TABLE __forceinline__
+#endif
+#if DW_OUTLINE >= 3
+#define DW_INL_PHYS __noinline__
+#else
+#define DW_INL_PHYS __forceinline__
+#endif
+
 constexpr float kInvC = 1.0f / 299.792458f;   // ns per mm in vacuum
 constexpr int kStackShared = kDwStackShared;  // per-thread traversal stack entries kept in shared memory
 constexpr int kStackLocal = kDwStackLocal;    // overflow entries (local memory; only unusually deep trees reach it)
@@ -29,7 +52,7 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
 }
 // ((x >> 9) + 0.5) * 2^-23: 24 significant bits, exact in fp32, strictly inside (0,1)
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
-__device__ __forceinline__ float4 draw4(uint64_t seed, uint64_t pid, uint32_t step, uint32_t block) {
+__device__ DW_INL_PHILOX float4 draw4(uint64_t seed, uint64_t pid, uint32_t step, uint32_t block) {
   uint4 r = philox4x32_10(make_uint4((uint32_t)pid, (uint32_t)(pid >> 32), step, block), (uint32_t)seed, (uint32_t)(seed >> 32));
   return make_float4(u01(r.x), u01(r.y), u01(r.z), u01(r.w));
 }
@@ -48,7 +71,7 @@ __device__ __forceinline__ V3 unit(V3 a) { return rsqrtf(dot(a, a)) * a; }
 __device__ __forceinline__ V3 fma3(float s, V3 a, V3 b) { return mk(fmaf(s, a.x, b.x), fmaf(s, a.y, b.y), fmaf(s, a.z, b.z)); }
 
 // ------------------------------------------------------------------------------------------------ tables (S3)
-__device__ __forceinline__ float table_at(const float* __restrict__ tab, int row, int nl, float l0, float inv_dl, float lambda) {
+__device__ DW_INL_TABLE float table_at(const float* __restrict__ tab, int row, int nl, float l0, float inv_dl, float lambda) {
   const float* r = tab + (size_t)row * nl;
   if (nl == 1) return __ldg(r);
   float f = (lambda - l0) * inv_dl;
@@ -207,7 +230,7 @@ __device__ __forceinline__ void frame(V3 w, V3& a, V3& b) {
 
 // S6 Rayleigh scattering: the algorithm that reproduces the theoretical distribution:
 // isotropic k', accept with probability |e - (e.k')k'|^2; iteration j uses Philox block 1 + j.
-__device__ __forceinline__ bool rayleigh(V3& k, V3& e, uint64_t seed, uint64_t pid, uint32_t step) {
+__device__ DW_INL_PHYS bool rayleigh(V3& k, V3& e, uint64_t seed, uint64_t pid, uint32_t step) {
   for (uint32_t j = 0; j < 4096u; ++j) {
     float4 r = draw4(seed, pid, step, 1u + j);
     float ct = 1.0f - 2.0f * r.x;
@@ -223,7 +246,7 @@ __device__ __forceinline__ bool rayleigh(V3& k, V3& e, uint64_t seed, uint64_t p
 }
 
 // S7 diffuse reflection (Lambert): block 1 = (cos^2 theta, azimuth, polarisation angle, -)
-__device__ __forceinline__ void lambert(V3 nh, V3& k, V3& e, float4 r) {
+__device__ DW_INL_PHYS void lambert(V3 nh, V3& k, V3& e, float4 r) {
   float ct = sqrtf(r.x), st = sqrtf(fmaxf(0.f, 1.0f - r.x));
   float sp, cp;
   sincospif(2.0f * r.y, &sp, &cp);
@@ -236,7 +259,7 @@ __device__ __forceinline__ void lambert(V3 nh, V3& k, V3& e, float4 r) {
 }
 
 // S8 Fresnel; nh faces the photon.  Returns history bits.
-__device__ __forceinline__ uint32_t fresnel(float n1, float n2, V3 nh, V3& k, V3& e, float u, bool& crossed) {
+__device__ DW_INL_PHYS uint32_t fresnel(float n1, float n2, V3 nh, V3& k, V3& e, float u, bool& crossed) {
   float ci = -dot(k, nh);
   V3 sv = cross(k, nh);
   float si2 = dot(sv, sv);
