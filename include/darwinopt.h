@@ -98,7 +98,7 @@ int dw_set_geometry(dw_ctx* ctx, int64_t n_vert, const float* xyz, int64_t n_tri
                     const int32_t* channel, int pointers_are_device);
 
 typedef struct dw_build_params {
-  int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (4) */
+  int32_t max_leaf_tris; /* 1..8, triangles per BVH leaf; 0 = default (2) */
   int32_t ploc_radius;   /* 1..256, search radius of the clustering rounds in Morton order; 0 = default (16) */
   int32_t grid_res;      /* 8..128, cells per axis of the empty-space grid; 0 = default (64); -1 = no grid */
   int32_t split_div;     /* a triangle longer than (largest scene extent) / split_div gets several box references;

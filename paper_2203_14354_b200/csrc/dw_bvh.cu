@@ -464,7 +464,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   int rc = DW_OK;
   const int nt = (int)c->n_tri;     // triangles
   int n = nt;                       // references (>= nt once long triangles are split): what the tree is built over
-  const int max_leaf = (params && params->max_leaf_tris) ? params->max_leaf_tris : 4;
+  const int max_leaf = (params && params->max_leaf_tris) ? params->max_leaf_tris : 2;
   const int radius = (params && params->ploc_radius) ? params->ploc_radius : 16;
   if (max_leaf < 1 || max_leaf > 8) return dw_fail(c, DW_E_ARG, "dw_build_bvh: max_leaf_tris must be in 1..8");
   if (radius < 1 || radius > 256) return dw_fail(c, DW_E_ARG, "dw_build_bvh: ploc_radius must be in 1..256");
