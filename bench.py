@@ -287,10 +287,15 @@ def main():
                     algorithmic_bytes_per_launch=alg_bytes,
                     memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
                     peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)")
-    traffic_file = ROOT / "profiles" / "traffic.json"
-    if traffic_file.exists():
+    # measured DRAM traffic per launch of the dominant kernel, from the ncu capture named in the file (null if none for this workload)
+    traffic_file = ROOT / "profiles" / "traffic.csv"
+    if traffic_file.exists() and n == c.n_photons and not args.legacy:
         try:
-            roofline["traffic"] = json.loads(traffic_file.read_text()).get(f"C{args.config}")
+            import csv
+            for row in csv.DictReader(traffic_file.open()):
+                if row["config"] == f"C{args.config}":
+                    roofline["traffic"] = int(row["dram_bytes_per_launch"])
+                    roofline["traffic_source"] = row["source"]
         except Exception:
             pass
 
