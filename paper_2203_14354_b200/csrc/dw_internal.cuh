@@ -29,7 +29,10 @@ struct DwTables {
 // ref >= 0: wide node index; ref < 0: leaf, ~ref = (first_slot << 3) | (count - 1); DW_REF_NONE = empty child.
 // Traversal stack: kDwStackShared entries per thread in shared memory, kDwStackLocal more in local memory; a step
 // pushes at most 3, so trees up to (kDwStackShared + kDwStackLocal) / 3 levels fit (dw_build_bvh checks).
-constexpr int kDwStackShared = 12;
+#ifndef DW_STACK_SHARED
+#define DW_STACK_SHARED 12
+#endif
+constexpr int kDwStackShared = DW_STACK_SHARED;
 constexpr int kDwStackLocal = 84;
 #define DW_REF_NONE 0x7fffffff
 

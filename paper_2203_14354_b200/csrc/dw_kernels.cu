@@ -12,6 +12,9 @@ namespace {
 // became the largest stall once the kernel grew to ~2900 instructions).  Level 0: everything inline; 1: Philox out of line;
 // 2: + table look-up; 3: + Rayleigh / Lambert / Fresnel.
 // Measured on C2 (alternating A/B, two rounds): level 0 173.8, 1 175.2, 2 188.6, 3 151.0 M photons/s.
+#ifndef DW_NODE_LDG256
+#define DW_NODE_LDG256 0
+#endif
 #ifndef DW_OUTLINE
 #define DW_OUTLINE 2
 #endif
@@ -140,10 +143,21 @@ __device__ __forceinline__ void ts_push(TraceState& s, int ref, int* sstack, int
   if (s.sp < kStackShared) sstack[s.sp * sstride] = ref; else lstack[s.sp - kStackShared] = ref;
   ++s.sp;
 }
+// 256-bit read-only load (sm_100: LDG.E.256): a node visit is 4 load instructions instead of 7, and the L1 cost of a divergent
+// load is paid per instruction and line (profiles/r01_final_c2.md: L1 throughput is the nearest limit).  p must be 32-byte aligned.
+__device__ __forceinline__ void ldg256(const float4* p, float4& a, float4& b) {
+  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(p));
+}
 __device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
   const float4* p = bvh.nodes + 8 * (size_t)s.node;
-  const float4 lx = __ldg(p), ly = __ldg(p + 1), lz = __ldg(p + 2), hx = __ldg(p + 3), hy = __ldg(p + 4), hz = __ldg(p + 5);
-  const float4 rf = __ldg(p + 6);
+  float4 lx, ly, lz, hx, hy, hz, rf, pad_;
+#if DW_NODE_LDG256
+  ldg256(p, lx, ly); ldg256(p + 2, lz, hx); ldg256(p + 4, hy, hz); ldg256(p + 6, rf, pad_);
+#else
+  lx = __ldg(p); ly = __ldg(p + 1); lz = __ldg(p + 2); hx = __ldg(p + 3); hy = __ldg(p + 4); hz = __ldg(p + 5); rf = __ldg(p + 6);
+#endif
+  (void)pad_;
   const int r0 = __float_as_int(rf.x), r1 = __float_as_int(rf.y), r2 = __float_as_int(rf.z), r3 = __float_as_int(rf.w);
   float n0, n1, n2, n3;
   const bool h0 = slab(r, s.best_t, bvh.eps_len, lx.x, ly.x, lz.x, hx.x, hy.x, hz.x, n0) && (r0 != DW_REF_NONE);
@@ -562,7 +576,11 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
 // next query set up) or is being traced by a lane (BUSY).  Lanes keep only the ray and the traversal state of the
 // query they run; when a query ends the lane writes (best_t, best_slot) to the slot and fetches another TRACE slot,
 // so traversal does not wait for physics, and physics runs for 32 slots at a time with every lane enabled.
-constexpr int kSlots = 64;
+#ifndef DW_POOL_SLOTS
+#define DW_POOL_SLOTS 64
+#endif
+constexpr int kSlots = DW_POOL_SLOTS;      // 33..64: lane l looks after slots l and l + 32 (the latter if it exists)
+static_assert(kSlots > 32 && kSlots <= 64, "pool size");
 enum : int { W_X = 0, W_Y, W_Z, W_KX, W_KY, W_KZ, W_EX, W_EY, W_EZ, W_LAMBDA, W_T, W_MEDIUM, W_LAST, W_STEP, W_HIST, W_PI,
              W_DBULK, W_N1, W_US, W_UF, W_BEST_T, W_BEST_SLOT, kWords };
 enum : int { S_EMPTY = 0, S_PHYS = 1, S_TRACE = 2, S_BUSY = 3 };
@@ -591,8 +609,9 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
   int* const q = wbase + kWarpQ;
   int* const my_stack = wbase + kWarpStack + lane;
   constexpr int sstride = 32;
+  const bool has2 = lane + 32 < kSlots;            // this lane also looks after slot lane + 32
   st[lane] = S_EMPTY;
-  st[lane + 32] = S_EMPTY;
+  if (has2) st[lane + 32] = S_EMPTY;
   __syncthreads();
   int lstack[kStackLocal];
   const unsigned lt = (1u << lane) - 1u;
@@ -614,7 +633,7 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
 
   for (;;) {
     // ---------------------------------------------------------------- census of the warp's slots
-    const int s0 = st[lane], s1 = st[lane + 32];
+    const int s0 = st[lane], s1 = has2 ? st[lane + 32] : -1;
     const unsigned p0 = __ballot_sync(0xffffffffu, s0 == S_PHYS), p1 = __ballot_sync(0xffffffffu, s1 == S_PHYS);
     const unsigned e0 = __ballot_sync(0xffffffffu, s0 == S_EMPTY), e1 = __ballot_sync(0xffffffffu, s1 == S_EMPTY);
     const unsigned t0 = __ballot_sync(0xffffffffu, s0 == S_TRACE), t1 = __ballot_sync(0xffffffffu, s1 == S_TRACE);

@@ -561,3 +561,41 @@ def test_empty_space_skip_is_invisible(cfg, n):
     b = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=200, dt=2.0, flags=dw.PROP_NO_EMPTY_SKIP)
     for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
         assert np.array_equal(a[key], b[key]), f"C{cfg}: '{key}' changes when queries are skipped"
+
+
+def test_results_do_not_depend_on_how_the_tree_is_built():
+    """The BVH, the split references and the empty-space grid only change HOW the nearest hit is found.  Every corner of
+    dw_build_params must therefore give bit-identical per-photon outputs and reductions (C1, wires of C3 via test above),
+    and out-of-range parameters must be refused with DW_E_ARG."""
+    c = synth.config(1)
+    ph = c.make_photons(150_000 - 11)
+    ref = None
+    corners = [dict(), dict(max_leaf_tris=1), dict(max_leaf_tris=8), dict(split_div=-1), dict(split_div=4), dict(split_div=512),
+               dict(grid_res=-1), dict(grid_res=8), dict(grid_res=128), dict(ploc_radius=1), dict(ploc_radius=64),
+               dict(max_leaf_tris=3, split_div=64, grid_res=96, ploc_radius=7)]
+    for kw in corners:
+        ctx = dw.Context(0)
+        ctx.set_optics(c.optics)
+        ctx.set_geometry(c.geometry)
+        st = ctx.build_bvh(**kw)
+        assert st["n_tri"] == c.geometry.n_tri and st["n_refs"] >= st["n_tri"] and st["n_nodes"] >= 1
+        if kw.get("split_div") == -1:
+            assert st["n_refs"] == st["n_tri"] and st["split_div"] == 0
+        if kw.get("grid_res") == -1:
+            assert st["grid_res"] == 0 and st["grid_free_cells"] == 0
+        r = gpu_run(ctx, ph, c.seed, c.max_steps, n_bins=100, dt=4.0)
+        if ref is None:
+            ref = r
+            assert int(r["fate_count"].sum()) == ph.n
+        else:
+            for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
+                assert np.array_equal(r[key], ref[key]), f"build parameters {kw}: '{key}' differs from the default build"
+        ctx.close()
+    ctx = dw.Context(0)
+    ctx.set_optics(c.optics)
+    ctx.set_geometry(c.geometry)
+    for bad in (dict(max_leaf_tris=9), dict(ploc_radius=257), dict(grid_res=7), dict(grid_res=129), dict(split_div=-2), dict(split_div=5000)):
+        with pytest.raises(dw.DwError) as ei:
+            ctx.build_bvh(**bad)
+        assert ei.value.code == dw.DW_E_ARG, bad
+    ctx.close()
