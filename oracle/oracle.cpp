@@ -20,6 +20,9 @@
 //   Lambert        : P6  pdf 2cos, <cos>=2/3 ; specular P7 incl. normal incidence
 //   surfaces/fates : P8  integrating sphere f/(1-rho(1-f)); P9 conservation; P10 transmit sheet
 //   Philox4x32-10  : published known-answer vectors (tests/golden/philox4x32_10_kat.txt)
+//   emission (E1-E5): position laws (r^2, z, rho^3 uniform), isotropy, e.k = 0 and uniform azimuth of e, Gaussian spectrum with
+//                        mean 174.8 nm / FWHM 10.2 nm (Table 2), two-exponential time profile with tau_1, tau_3, f_s
+//                        (Table 2): closed-form CDFs by KS, moments (tests/test_oracle_emission.py)
 //   parity unpinned: trajectories beyond what the closed forms above fix, and the paper's own
 //                    absolute LCE / t90 numbers (need the DARWIN CAD model).
 //
@@ -379,7 +382,66 @@ int set_table(Table& tb, int rows, int nl, double l0, double dl, const float* a)
 }  // namespace
 
 // =================================================================== C interface for ctypes (tests / bench)
+// ---------------------------------------------------------------- emission
+// One scintillation photon per id, drawn from Philox blocks 0..2 of the reserved step 0xFFFFFFFF (propagation steps are
+// < 2^31, so the streams never meet).  P:144: "The emission spectrum is modeled as a Gaussian with a mean of 174.8 nm and a
+// full width at half maximum of 10.2 nm.  The scintillation time profile is modeled by a two-component exponential decay
+// function"; Table 2: tau_1 = 3.5 ns, tau_3 = 24 ns, f_s = 0.66 (NR) / 0.22 (ER).  P:191: photons "generated
+// isotropically and uniformly" in the active region.  [readings, DESIGN.md E-*]: random transverse polarisation = normalize(k x r)
+// for an independent isotropic r; the spectrum is not truncated (tables clamp); the singlet branch is taken when
+// u < (float)f_s, the comparison the fp32 kernel makes.
+struct Source {
+  int shape;            // 0 point, 1 cylinder (axis z), 2 ball
+  double c[3];          // point / centre of the cylinder axis at z0 / centre of the ball
+  double radius;        // cylinder or ball radius
+  double z0, z1;        // cylinder: z range
+  double lambda_mean, lambda_sigma;   // nm; sigma = FWHM / (2 sqrt(2 ln 2))
+  double t_start, tau1, tau3, f_singlet;
+};
+constexpr uint32_t kEmitStep = 0xFFFFFFFFu;
+inline V3 isotropic(double u_cos, double u_phi) {
+  double ct = 1.0 - 2.0 * u_cos, st = std::sqrt(std::max(0.0, 1.0 - ct * ct)), ph = 2.0 * M_PI * u_phi;
+  return {st * std::cos(ph), st * std::sin(ph), ct};
+}
+inline void emit(const Source& s, uint64_t seed, uint64_t pid, V3& x, V3& k, V3& e, double& lambda, double& t) {
+  const Rand4 a = draw(seed, pid, kEmitStep, 0), b = draw(seed, pid, kEmitStep, 1), c = draw(seed, pid, kEmitStep, 2);
+  // E1 position
+  if (s.shape == 1) {
+    double r = s.radius * std::sqrt(a.u[0]), ph = 2.0 * M_PI * a.u[1];
+    x = {s.c[0] + r * std::cos(ph), s.c[1] + r * std::sin(ph), s.z0 + (s.z1 - s.z0) * a.u[2]};
+  } else if (s.shape == 2) {
+    V3 d = isotropic(a.u[1], a.u[2]);
+    double r = s.radius * std::cbrt(a.u[0]);
+    x = {s.c[0] + r * d.x, s.c[1] + r * d.y, s.c[2] + r * d.z};
+  } else {
+    x = {s.c[0], s.c[1], s.c[2]};
+  }
+  // E2 direction, E3 polarisation
+  k = isotropic(b.u[0], b.u[1]);
+  V3 r = isotropic(b.u[2], b.u[3]);
+  V3 kr = cross(k, r);
+  if (dot(kr, kr) < 1e-12) { V3 a2, b2; frame(k, a2, b2); e = a2; }
+  else e = unit(kr);
+  // E4 wavelength (Box-Muller), E5 time
+  lambda = s.lambda_mean + s.lambda_sigma * std::sqrt(-2.0 * std::log(c.u[0])) * std::cos(2.0 * M_PI * c.u[1]);
+  const double tau = (c.u[2] < (double)(float)s.f_singlet) ? s.tau1 : s.tau3;
+  t = s.t_start - tau * std::log(c.u[3]);
+}
+
 extern "C" {
+
+// out: 11 arrays of n doubles in the order of dw_photons (px py pz kx ky kz ex ey ez wavelength t0)
+void orc_emit(int shape, const double* c3, double radius, double z0, double z1, double lambda_mean, double lambda_sigma,
+              double t_start, double tau1, double tau3, double f_singlet, uint64_t seed, uint64_t id_base, int64_t n, double* out) {
+  Source s{shape, {c3[0], c3[1], c3[2]}, radius, z0, z1, lambda_mean, lambda_sigma, t_start, tau1, tau3, f_singlet};
+  for (int64_t i = 0; i < n; ++i) {
+    V3 x, k, e;
+    double lambda, t;
+    emit(s, seed, id_base + (uint64_t)i, x, k, e, lambda, t);
+    const double v[11] = {x.x, x.y, x.z, k.x, k.y, k.z, e.x, e.y, e.z, lambda, t};
+    for (int f = 0; f < 11; ++f) out[(size_t)f * n + i] = v[f];
+  }
+}
 
 void* orc_create() { return new Scene(); }
 void orc_destroy(void* h) { delete (Scene*)h; }

@@ -51,6 +51,7 @@ def lib():
         L.orc_first_hit.argtypes = [vp, i64] + [vp] * 7 + [C.c_int, vp, vp, C.c_int]
         L.orc_propagate.argtypes = ([vp, i64] + [vp] * 11 + [u64, u64, i32, C.c_int] + [vp] * 8 +
                                     [i64, vp, i64, f64, f64, vp, vp, vp, C.c_int])
+        L.orc_emit.argtypes = [C.c_int, vp, f64, f64, f64, f64, f64, f64, f64, f64, f64, u64, u64, i64, vp]
         L.orc_philox4x32_10.argtypes = [vp, vp, vp]
         L.orc_uniforms.argtypes = [u64, u64, u32, u32, vp]
         L.orc_rayleigh.argtypes = [vp, vp, u64, u64, u32]
@@ -199,3 +200,14 @@ def fresnel(n1, n2, nhat, k, e, u):
     R = C.c_double(0.0)
     oc = lib().orc_fresnel(float(n1), float(n2), _p(n), _p(k), _p(e), float(u), C.byref(R))
     return oc, R.value, k, e
+
+
+def emit(source: dict, seed: int, id_base: int, n: int):
+    """Emission: n photons of `source` (keys of paper_2203_14354_b200.synth.source()), fp64.
+    Returns a dict of arrays: pos [3,n], dir [3,n], pol [3,n], wavelength [n], t0 [n]."""
+    out = np.empty((11, n), np.float64)
+    c3 = np.ascontiguousarray(source["centre"], np.float64)
+    lib().orc_emit(int(source["shape"]), _p(c3), float(source["radius"]), float(source["z0"]), float(source["z1"]),
+                   float(source["lambda_mean"]), float(source["lambda_sigma"]), float(source["t_start"]), float(source["tau1"]),
+                   float(source["tau3"]), float(source["f_singlet"]), int(seed), int(id_base), int(n), _p(out))
+    return dict(pos=out[0:3], dir=out[3:6], pol=out[6:9], wavelength=out[9], t0=out[10])

@@ -404,3 +404,30 @@ def config(i: int, ptfe_reflectivity: float = 0.95) -> Config:
                       lambda n, base=0: photons_s2_spot(5, n, (400.0, 200.0, 2600.0 + 1.25), 1.0, 27.0, base),
                       "batches of 1e7, photon_id_base = b*1e7; PTFE reflectivity in {0.90,0.95,0.99}")
     raise ValueError(f"no config {i}")
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Emission sources.  Plain parameter sets: no arithmetic of the method lives here.
+FWHM_TO_SIGMA = 1.0 / 2.3548200450309493        # 1 / (2 sqrt(2 ln 2))
+SHAPE_POINT, SHAPE_CYLINDER, SHAPE_BALL = 0, 1, 2
+
+
+def source(shape=SHAPE_CYLINDER, centre=(0.0, 0.0, 0.0), radius=0.0, z0=0.0, z1=0.0, lambda_mean=174.8, lambda_fwhm=10.2,
+           t_start=0.0, tau1=3.5, tau3=24.0, f_singlet=0.66) -> dict:
+    """PAPER.md line 144 and Table 2 (lines 155-160): Gaussian spectrum 174.8 nm / FWHM 10.2 nm, two-exponential time profile with
+    tau_1 = 3.5 ns, tau_3 = 24 ns, singlet fraction 0.66 (nuclear recoils) or 0.22 (electronic recoils)."""
+    return dict(shape=int(shape), centre=tuple(float(v) for v in centre), radius=float(radius), z0=float(z0), z1=float(z1),
+                lambda_mean=float(lambda_mean), lambda_sigma=float(lambda_fwhm) * FWHM_TO_SIGMA, t_start=float(t_start),
+                tau1=float(tau1), tau3=float(tau3), f_singlet=float(f_singlet))
+
+
+def source_for(i: int, recoil: str = "NR") -> dict:
+    """The liquid volume of config i (1..3) as a cylinder source, or the S2 spot of config 4 as a ball source."""
+    fs = 0.66 if recoil == "NR" else 0.22
+    if i == 1:
+        return source(SHAPE_CYLINDER, (0, 0, 0), 249.0, 2.0, 494.0, f_singlet=fs)
+    if i in (2, 3):
+        return source(SHAPE_CYLINDER, (0, 0, 0), 1299.0, 2.0, 2599.0, f_singlet=fs)
+    if i == 4:
+        return source(SHAPE_BALL, (400.0, 200.0, 2601.25), 1.0, tau1=27.0, tau3=27.0, f_singlet=1.0)
+    raise ValueError(i)
