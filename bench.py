@@ -123,6 +123,19 @@ def workload(args):
     return c, n
 
 
+def synth_source(cfg):
+    from paper_2203_14354_b200 import synth
+    return synth.source_for(cfg)
+
+
+def emit_args(dw, source):
+    import ctypes
+    src = dw.Source(shape=int(source["shape"]), centre=(ctypes.c_float * 3)(*source["centre"]), radius=source["radius"], z0=source["z0"],
+                    z1=source["z1"], lambda_mean=source["lambda_mean"], lambda_sigma=source["lambda_sigma"], t_start=source["t_start"],
+                    tau1=source["tau1"], tau3=source["tau3"], f_singlet=source["f_singlet"])
+    return (ctypes.byref(src),)
+
+
 def cpu_baseline(c, n_sample, id_base=0, threads=None):
     """The oracle, as it stands, on the first n_sample photons of the workload's batch."""
     from oracle import oracle as orc
@@ -188,6 +201,8 @@ def main():
     ap.add_argument("--split-div", type=int, default=0, help="split triangles longer than scene extent / this (0 = default, -1 = never)")
     ap.add_argument("--grid-res", type=int, default=0, help="cells per axis of the empty-space grid (0 = default, -1 = none)")
     ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
+    ap.add_argument("--emit", action="store_true", help="generate each step's photons on the device with dw_emit inside the timed step "
+                    "(SURVEY 8(f) f1; C1-C4 only) instead of propagating a resident batch")
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
@@ -219,8 +234,14 @@ def main():
     stream = torch.cuda.current_stream()
     flags = (dw.PROP_UNBOUNDED_QUERY if args.literal else 0) | (dw.PROP_LEGACY_SCHEDULER if args.legacy else 0) | (dw.PROP_NO_EMPTY_SKIP if args.no_skip else 0)
 
+    source = synth_source(args.config) if args.emit else None
+    state = dict(d_ph=d_ph, k=0)
+
     def step():
-        ctx.propagate(d_ph, c.seed, c.max_steps, out, hist, flags=flags, stream=stream, th_phys=args.th_phys,
+        if source is not None:                  # a new batch of ids every step, written by dw_emit on the same stream
+            state["d_ph"] = ctx.emit(source, c.seed, n, id_base=id_base + state["k"] * n * world, device=dev, stream=stream)
+            state["k"] += 1
+        ctx.propagate(state["d_ph"], c.seed, c.max_steps, out, hist, flags=flags, stream=stream, th_phys=args.th_phys,
                       th_leaf=args.th_leaf, block_threads=args.block, blocks_per_sm=args.blocks_per_sm)
         if world > 1:
             dwdist.merge_hists(hist)        # the only exchange: tens of kB of integer histograms
@@ -253,9 +274,25 @@ def main():
     n_all = n * world
     value = n_all * args.steps / (total_ms * 1e-3)
 
+    emit_info = None
+    if args.emit:
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        keep = ctx.emit(source, c.seed, n, device=dev, stream=stream)          # warm-up and allocation
+        reps = 20
+        evs[0].record(stream)
+        for r in range(reps):
+            ctx.L.dw_emit(ctx.h, *emit_args(dw, source), int(c.seed), __import__("ctypes").byref(keep.c), dw._stream_ptr(stream))
+        evs[1].record(stream)
+        torch.cuda.synchronize()
+        ems = evs[0].elapsed_time(evs[1]) / reps
+        peaks0 = measured_peaks()
+        emit_info = dict(kernel="emit_kernel", ms=ems, photons_per_s=n / (ems * 1e-3), bytes_per_photon=44,
+                         achieved_gbs=44.0 * n / (ems * 1e-3) / 1e9, hbm_peak_gbs=peaks0["hbm_gbs"],
+                         frac_of_hbm=44.0 * n / (ems * 1e-3) / 1e9 / peaks0["hbm_gbs"])
+
     # ---- end to end through the host-buffer entry (pinned host memory, H2D + D2H inside the timed region)
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.emit:
         hp = dw.HostPhotons(ph)
         hout = dw.HostResults(n, ("flags", "channel", "t"))
         hh = dw.HostHists(ctx.n_chan, 2000, 0.0, 1.0)
@@ -309,13 +346,14 @@ def main():
                 config=dict(workload=c.name, photons_per_step_per_gpu=n, triangles=c.geometry.n_tri, max_steps=c.max_steps,
                             seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
                             mode="literal" if args.literal else "bounded rays",
+                            inputs="dw_emit on the device, a new batch of photon ids every step" if args.emit else "resident batch, same photons every step",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
                             bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch()),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
-                clocks=clocks, e2e=e2e, gpu_launches=int(launches), roofline=roofline, cpu_baseline=cpu)
+                clocks=clocks, e2e=e2e, emission=emit_info, gpu_launches=int(launches) * (2 if args.emit else 1), roofline=roofline, cpu_baseline=cpu)
     print(json.dumps(line))
     dwdist.finalize()
     return 0

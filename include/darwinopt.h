@@ -204,6 +204,34 @@ int dw_propagate(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_s
 int dw_propagate_host(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps,
                       const dw_results* out, const dw_hists* hist, const dw_propagate_params* params);
 
+
+/* Emission of scintillation photons on the device.
+ * "The emission spectrum is modeled as a Gaussian with a mean of 174.8 nm and a full width at half maximum of
+ * 10.2 nm.  The scintillation time profile is modeled by a two-component exponential decay function"; Table 2 (lines 155-160):
+ * tau_1 = 3.5 ns, tau_3 = 24 ns, singlet fraction 0.66 (nuclear recoils) / 0.22 (electronic recoils); line 191: photons are
+ * generated isotropically and uniformly in the active region.
+ * Photon photon_id_base + i takes Philox blocks 0..2 of the reserved step 0xFFFFFFFF (key = seed), so the result depends on
+ * (seed, photon id) only and any split of a batch gives the same photons:
+ *   position   shape 0: centre; 1: uniform in the cylinder of `radius` about the z axis through centre, z in [z0, z1];
+ *              2: uniform in the ball of `radius` about centre
+ *   direction  isotropic;  polarisation  normalize(k x r) for an independent isotropic r (random transverse)
+ *   wavelength lambda_mean + lambda_sigma * N(0,1) (Box-Muller; sigma = FWHM / (2 sqrt(2 ln 2)); not truncated)
+ *   time       t_start - tau ln u with tau = tau1 with probability f_singlet, else tau3 */
+typedef struct dw_source {
+  int32_t shape;                 /* DW_SOURCE_* */
+  float centre[3];               /* mm */
+  float radius, z0, z1;          /* mm; z0 <= z1 (cylinder only) */
+  float lambda_mean, lambda_sigma; /* nm; sigma >= 0 */
+  float t_start, tau1, tau3;     /* ns; tau >= 0 */
+  float f_singlet;               /* in [0, 1] */
+  int32_t reserved[3];
+} dw_source;
+enum { DW_SOURCE_POINT = 0, DW_SOURCE_CYLINDER = 1, DW_SOURCE_BALL = 2 };
+
+/* Writes out->n photons into the eleven DEVICE arrays of `out` (they are written although the struct declares them const:
+ * the same struct then goes to dw_propagate).  Asynchronous on the stream.  DW_E_ARG for a bad source or a null array. */
+int dw_emit(dw_ctx* ctx, const dw_source* source, uint64_t seed, const dw_photons* out, void* cuda_stream);
+
 /* Diagnostics / tests: raw Philox4x32-10 blocks and the uniforms the kernel derives from them, computed on the
  * device.  out_raw [n][4] uint32, out_u [n][4] float (either may be NULL), DEVICE pointers; entry i uses
  * photon id photon_id_base + i, the given step and block. */

@@ -25,7 +25,7 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch")
+           "dw_debug_philox", "dw_last_launch", "dw_emit")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -53,6 +53,11 @@ class Results(C.Structure):
 class Hists(C.Structure):
     _fields_ = [("n_chan", i64), ("chan_count", vp), ("n_bins", i64), ("t_min", f32), ("dt", f32),
                 ("time_hist", vp), ("fate_count", vp), ("total_steps", vp)]
+
+
+class Source(C.Structure):
+    _fields_ = [("shape", i32), ("centre", f32 * 3), ("radius", f32), ("z0", f32), ("z1", f32), ("lambda_mean", f32),
+                ("lambda_sigma", f32), ("t_start", f32), ("tau1", f32), ("tau3", f32), ("f_singlet", f32), ("reserved", i32 * 3)]
 
 
 class PropagateParams(C.Structure):
@@ -88,6 +93,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     L.dw_propagate_host.argtypes = [vp, C.POINTER(Photons), u64, i32, C.POINTER(Results), C.POINTER(Hists),
                                     C.POINTER(PropagateParams)]
     L.dw_debug_philox.argtypes = [vp, u64, u64, u32, u32, i64, vp, vp, vp]
+    L.dw_emit.argtypes = [vp, C.POINTER(Source), u64, C.POINTER(Photons), vp]
     L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
     for name in EXPORTS:
         if name not in ("dw_last_error",):
@@ -185,6 +191,16 @@ class Context:
         self.stats = {k: (list(getattr(st, k)) if k.startswith("scene") else getattr(st, k)) for k, _ in BuildStats._fields_}
         return self.stats
 
+    # ---- emission -------------------------------------------------------------------
+    def emit(self, source: dict, seed: int, n: int, id_base: int = 0, device="cuda:0", stream=None) -> "EmittedPhotons":
+        """n scintillation photons of `source` (see synth.source) generated on the device; the result goes to propagate()."""
+        out = EmittedPhotons(n, id_base, device)
+        src = Source(shape=int(source["shape"]), centre=(f32 * 3)(*source["centre"]), radius=source["radius"], z0=source["z0"],
+                     z1=source["z1"], lambda_mean=source["lambda_mean"], lambda_sigma=source["lambda_sigma"],
+                     t_start=source["t_start"], tau1=source["tau1"], tau3=source["tau3"], f_singlet=source["f_singlet"])
+        self._check(self.L.dw_emit(self.h, C.byref(src), int(seed), C.byref(out.c), _stream_ptr(stream)))
+        return out
+
     # ---- queries -------------------------------------------------------------------------------------
     def first_hit(self, origin, direction, exclude=None, stream=None):
         """origin, direction: torch CUDA float32 [3,n] (rows contiguous).  Returns (tri int32[n], dist float32[n])."""
@@ -247,6 +263,19 @@ class DevicePhotons(_PhotonsBase):
         rows = dict(px=ph.pos[0], py=ph.pos[1], pz=ph.pos[2], kx=ph.dir[0], ky=ph.dir[1], kz=ph.dir[2],
                     ex=ph.pol[0], ey=ph.pol[1], ez=ph.pol[2], wavelength=ph.wavelength, t0=ph.t0)
         self._fill({k: torch.from_numpy(_np(v, np.float32)).to(device) for k, v in rows.items()}, ph.n, ph.id_base)
+
+
+class EmittedPhotons(_PhotonsBase):
+    """Eleven uninitialised device arrays for Context.emit to fill."""
+
+    def __init__(self, n, id_base=0, device="cuda:0"):
+        import torch
+        self._fill({k: torch.empty(max(n, 1), dtype=torch.float32, device=device) for k in _IN}, n, id_base)
+
+    def numpy(self):
+        g = lambda k: self.t[k][: self.n].cpu().numpy()
+        return dict(pos=np.stack([g("px"), g("py"), g("pz")]), dir=np.stack([g("kx"), g("ky"), g("kz")]),
+                    pol=np.stack([g("ex"), g("ey"), g("ez")]), wavelength=g("wavelength"), t0=g("t0"))
 
 
 class HostPhotons(_PhotonsBase):

@@ -240,6 +240,23 @@ extern "C" int dw_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   return dw_propagate_impl(c, in, seed, max_steps, out, hist, params, (cudaStream_t)stream);
 }
 
+extern "C" int dw_emit(dw_ctx* c, const dw_source* src, uint64_t seed, const dw_photons* out, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!src || !out) return dw_fail(c, DW_E_ARG, "dw_emit: null source or output");
+  if (out->n < 0) return dw_fail(c, DW_E_ARG, "dw_emit: n < 0");
+  if (src->shape < DW_SOURCE_POINT || src->shape > DW_SOURCE_BALL) return dw_fail(c, DW_E_ARG, "dw_emit: unknown shape %d", src->shape);
+  const float chk[] = {src->centre[0], src->centre[1], src->centre[2], src->radius, src->z0, src->z1, src->lambda_mean, src->lambda_sigma,
+                       src->t_start, src->tau1, src->tau3, src->f_singlet};
+  for (float v : chk) if (!std::isfinite(v)) return dw_fail(c, DW_E_ARG, "dw_emit: non-finite source parameter");
+  if (src->radius < 0.f || src->lambda_sigma < 0.f || src->tau1 < 0.f || src->tau3 < 0.f || src->z1 < src->z0 ||
+      src->f_singlet < 0.f || src->f_singlet > 1.f)
+    return dw_fail(c, DW_E_ARG, "dw_emit: radius, sigma, tau must be >= 0, z0 <= z1, 0 <= f_singlet <= 1");
+  const float* const arr[11] = {out->px, out->py, out->pz, out->kx, out->ky, out->kz, out->ex, out->ey, out->ez, out->wavelength, out->t0};
+  if (out->n > 0) for (const float* a : arr) if (!a) return dw_fail(c, DW_E_ARG, "dw_emit: null output array");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_emit_impl(c, src, seed, out, (cudaStream_t)stream);
+}
+
 extern "C" int dw_debug_philox(dw_ctx* c, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
                                uint32_t* out_raw, float* out_u, void* stream) {
   if (!c) return DW_E_ARG;

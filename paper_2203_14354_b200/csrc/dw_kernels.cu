@@ -2,6 +2,7 @@
 // propagation kernel (S1..S13 of DESIGN.md; "photon propagation code", P:175 surface models,
 // P:185-187 Fresnel/TIR checks, P:436-444 appendix fixes).  fp32 arithmetic throughout.
 #include <float.h>
+#include <stddef.h>
 #include <math.h>
 
 #include "dw_internal.cuh"
@@ -936,6 +937,40 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
   if (threadIdx.x == 0 && A.hist.total_steps && s_steps) atomicAdd((unsigned long long*)A.hist.total_steps, s_steps);
 }
 
+// ------------------------------------------------------------------------------------------------ emission (f1)
+// One photon per thread; the steps and draws of include/darwinopt.h "dw_emit" (Table 2).
+constexpr uint32_t kEmitStep = 0xFFFFFFFFu;
+__device__ __forceinline__ V3 isotropic(float u_cos, float u_phi) {
+  float ct = 1.0f - 2.0f * u_cos, st = sqrtf(fmaxf(0.f, 1.0f - ct * ct)), sp, cp;
+  sincospif(2.0f * u_phi, &sp, &cp);
+  return mk(st * cp, st * sp, ct);
+}
+__global__ void emit_kernel(dw_source S, uint64_t seed, dw_photons P) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const uint64_t pid = P.photon_id_base + (uint64_t)i;
+  const float4 a = draw4(seed, pid, kEmitStep, 0u), b = draw4(seed, pid, kEmitStep, 1u), c = draw4(seed, pid, kEmitStep, 2u);
+  V3 x = mk(S.centre[0], S.centre[1], S.centre[2]);
+  if (S.shape == DW_SOURCE_CYLINDER) {
+    float r = S.radius * sqrtf(a.x), sp, cp;
+    sincospif(2.0f * a.y, &sp, &cp);
+    x = mk(fmaf(r, cp, S.centre[0]), fmaf(r, sp, S.centre[1]), fmaf(S.z1 - S.z0, a.z, S.z0));
+  } else if (S.shape == DW_SOURCE_BALL) {
+    x = fma3(S.radius * cbrtf(a.x), isotropic(a.y, a.z), x);
+  }
+  const V3 k = isotropic(b.x, b.y);
+  const V3 kr = cross(k, isotropic(b.z, b.w));
+  V3 e, e2;
+  if (dot(kr, kr) < 1e-12f) frame(k, e, e2);
+  else e = unit(kr);
+  const float lambda = fmaf(S.lambda_sigma * sqrtf(-2.0f * logf(c.x)), cospif(2.0f * c.y), S.lambda_mean);
+  const float tau = (c.z < S.f_singlet) ? S.tau1 : S.tau3;
+  const float t = fmaf(-tau, logf(c.w), S.t_start);
+  float* const* o = (float* const*)&P.px;          // the eleven arrays follow each other in dw_photons
+  o[0][i] = x.x; o[1][i] = x.y; o[2][i] = x.z; o[3][i] = k.x; o[4][i] = k.y; o[5][i] = k.z;
+  o[6][i] = e.x; o[7][i] = e.y; o[8][i] = e.z; o[9][i] = lambda; o[10][i] = t;
+}
+
 __global__ void philox_debug_kernel(uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
                                     uint32_t* __restrict__ out_raw, float* __restrict__ out_u) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -1020,6 +1055,14 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
     int rc = launch_propagate(c, &pi, seed, max_steps, out ? &po : nullptr, hist, params, stream);
     if (rc != DW_OK) return rc;
   }
+  return DW_OK;
+}
+
+int dw_emit_impl(dw_ctx* c, const dw_source* src, uint64_t seed, const dw_photons* out, cudaStream_t stream) {
+  static_assert(offsetof(dw_photons, t0) - offsetof(dw_photons, px) == 10 * sizeof(float*), "dw_photons: eleven consecutive arrays");
+  if (out->n == 0) return DW_OK;
+  emit_kernel<<<(unsigned)((out->n + 255) / 256), 256, 0, stream>>>(*src, seed, *out);
+  DW_CUDA(c, cudaGetLastError());
   return DW_OK;
 }
 
