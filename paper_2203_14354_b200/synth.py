@@ -431,3 +431,39 @@ def source_for(i: int, recoil: str = "NR") -> dict:
     if i == 4:
         return source(SHAPE_BALL, (400.0, 200.0, 2601.25), 1.0, tau1=27.0, tau3=27.0, f_singlet=1.0)
     raise ValueError(i)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Dispersive tables: five wavelength nodes, so that the linear interpolation of S3 is a live path once photons carry the
+# emission spectrum.  SYNTHETIC dispersion (the paper tabulates values at 175 nm only, Table 2): chosen to pass through the
+# config values at 175 nm and to vary by amounts of the order of the paper's quoted spreads.
+DISPERSIVE_GRID = (165.0, 5.0, 5)        # lambda0, dlambda, nodes: 165, 170, 175, 180, 185 nm
+
+
+def dispersive_optics(ptfe_reflectivity: float = 0.95, qe: float = 0.3) -> Optics:
+    l0, dl, nl = DISPERSIVE_GRID
+    lam = l0 + dl * np.arange(nl)
+    rows = lambda *r: np.asarray(r, np.float32)
+    flat = lambda v: np.full(nl, v, np.float32)
+    n = rows(1.69 - 0.008 * (lam - 175.0), flat(1.0), flat(1.0), flat(1.0))                       # LXe 1.77 .. 1.61
+    la = rows(50000.0 * (1.0 + 0.02 * (lam - 175.0)), flat(5.0e5), flat(INF), 2000.0 + 40.0 * (lam - 175.0))
+    ls = rows(400.0 * (lam / 175.0) ** 4, flat(2.0e5), flat(INF), flat(INF))                      # Rayleigh ~ lambda^4
+    det = rows(flat(0.0), qe + 0.005 * (lam - 175.0), flat(0.0), flat(1.0))
+    rd = rows(ptfe_reflectivity + 0.002 * (lam - 175.0), flat(0.0), flat(0.0), flat(0.0))
+    rs = rows(flat(0.0), flat(0.0), flat(0.5), flat(0.0))
+    tr = rows(flat(0.0), flat(0.0), flat(0.0), flat(0.0))
+    return Optics(nl, l0, dl, n, la, ls, det, rd, rs, tr)
+
+
+def config_dispersive(i: int = 1) -> Config:
+    """Config i (1 or 2) with the dispersive tables and photons that carry the emission spectrum (174.8 nm, FWHM 10.2 nm,
+    drawn by the harness, so that some wavelengths fall outside the table and exercise the clamping)."""
+    base = config(i)
+
+    def make(n, id_base=0):
+        ph = base.make_photons(n, id_base)
+        rng = np.random.Generator(np.random.PCG64([base.seed, id_base, 77]))
+        lam = rng.normal(174.8, 10.2 * FWHM_TO_SIGMA, ph.n).astype(np.float32)
+        return Photons(ph.pos, ph.dir, ph.pol, lam, ph.t0, ph.id_base)
+    return Config(base.name + " (dispersive tables)", base.geometry, dispersive_optics(), base.n_photons, base.seed, base.max_steps, make,
+                  "synthetic dispersion on five wavelength nodes")

@@ -599,3 +599,51 @@ def test_results_do_not_depend_on_how_the_tree_is_built():
             ctx.build_bvh(**bad)
         assert ei.value.code == dw.DW_E_ARG, bad
     ctx.close()
+
+
+# ------------------------------------------------------------------------------------------- S3 on more than one wavelength node
+_DISP = {}
+
+
+def dispersive(i=1):
+    if i not in _DISP:
+        conf = synth.config_dispersive(i)
+        _DISP[i] = (conf, dw.make_context(conf.geometry, conf.optics))
+    return _DISP[i]
+
+
+def test_table_interpolation_on_device():
+    """Same case as the oracle pin test_table_interpolation_and_clamping: nodes, points between nodes, wavelengths beyond both
+    ends of a five-node table; the device must reproduce the oracle photon by photon (same draws, max_steps 1)."""
+    R = 1000.0
+    op = synth.dispersive_optics()
+    lams = np.array([150.0, 165.0, 166.25, 172.5, 175.0, 178.0, 185.0, 199.0])
+    n_each = 40_000
+    base = synth.photons_point(5, n_each * len(lams))
+    ph = synth.Photons(base.pos, base.dir, base.pol, np.repeat(lams, n_each).astype(np.float32), base.t0, base.id_base)
+    for material, seed in ((synth.MAT_C0GAS, 5), (synth.MAT_LXE, 6)):
+        g = synth.sphere_detector(R, 4, material=material)
+        ctx = dw.make_context(g, op)
+        r = gpu_run(ctx, ph, seed, 1)
+        ref = orc.Oracle(g, op, bvh=True).propagate(ph, seed, 1)
+        same = (r["flags"] == ref["flags"]) & (r["channel"] == ref["channel"])
+        assert same.mean() >= 0.9995, f"material {material}: identical on {same.mean():.5f}"
+        assert np.allclose(r["t"][same], ref["t"][same], rtol=2e-6, atol=1e-6)       # t = d n(lambda) / c with the interpolated n
+        ctx.close()
+
+
+def test_step_locked_parity_with_dispersive_tables():
+    conf, ctx = dispersive(1)
+    n = 200_000
+    ph = conf.make_photons(n)
+    assert ph.wavelength.min() < 165.0 and ph.wavelength.max() > 185.0 and len(np.unique(ph.wavelength)) > 1000
+    ref = orc.Oracle(conf.geometry, conf.optics, bvh=True).propagate(ph, conf.seed, 3)
+    r = gpu_run(ctx, ph, conf.seed, 3)
+    same = (r["flags"] == ref["flags"]) & (r["steps"] == ref["steps"]) & (r["channel"] == ref["channel"]) & (r["last_tri"] == ref["last_tri"])
+    assert same.mean() >= 0.999, f"identical on {same.mean():.5f}"
+    assert np.allclose(r["t"][same], ref["t"][same], rtol=1e-4, atol=1e-4)
+
+
+def test_c1_statistical_parity_with_dispersive_tables():
+    conf, ctx = dispersive(1)
+    check_statistical_parity(1, 1_000_000, 1_000_000, ctx=ctx, conf=conf)

@@ -583,3 +583,48 @@ def test_transmitting_sheet_and_wire_shadow():
     frac = 1 - fates(out2)["detected"] / N
     assert abs(frac - shadow) < 4 * math.sqrt(shadow * (1 - shadow) / N)
     assert shadow == pytest.approx(0.04, abs=1e-3)          # the paper's 0.2 mm / 5 mm <-> 95-96% transparency
+
+
+# ----------------------------------------------------------------------------- S3 tables on more than one wavelength node
+def test_table_interpolation_and_clamping():
+    """S3 / G13: linear interpolation on the uniform wavelength grid, clamped at both ends.  From the centre of a detector
+    sphere the time of flight is exactly d n(lambda) / c (S5) and the detected fraction is exp(-d / L_abs(lambda)) (P2), so
+    both tabulated quantities are pinned against numpy's own interpolation routine: nodes, points between nodes, and
+    wavelengths beyond either end of the table."""
+    R = 1000.0
+    g = synth.sphere_detector(R, 4)
+    op = synth.dispersive_optics()
+    l0, dl, nl = synth.DISPERSIVE_GRID
+    grid = l0 + dl * np.arange(nl)
+    lams = np.array([150.0, 165.0, 166.25, 172.5, 175.0, 178.0, 185.0, 199.0])
+    n_each = 40_000
+    ph = synth.photons_point(5, n_each * len(lams))
+    lam = np.repeat(lams, n_each).astype(np.float32)
+    ph = synth.Photons(ph.pos, ph.dir, ph.pol, lam, ph.t0, ph.id_base)
+    out = orc.Oracle(g, op, bvh=True).propagate(ph, 5, 10)
+    det = out["fate"] == orc.FATE_DETECTED
+    d = np.sqrt((out["pos"] ** 2).sum(0))
+    # material 3 (the sphere's gas): n = 1 flat, L_abs = 2000 + 40 (lambda - 175), no scattering
+    L_tab = op.abs_len[synth.MAT_C0GAS].astype(np.float64)
+    assert L_tab[0] != L_tab[-1]
+    for k, l in enumerate(lams):
+        sel = slice(k * n_each, (k + 1) * n_each)
+        L = np.interp(l, grid, L_tab)                      # numpy clamps outside the grid
+        expect = np.exp(-d[sel][det[sel]] / L).mean() if det[sel].any() else 0.0
+        frac = det[sel].mean()
+        p = math.exp(-R / L)
+        assert abs(frac - p) < 4 * math.sqrt(p * (1 - p) / n_each) + 3e-4, (l, frac, p)   # + faceting bias (d <= R)
+        assert abs(expect - p) < 2e-3
+    # the index of refraction through the time of flight: put the dispersive LXe inside the sphere
+    g2 = synth.sphere_detector(R, 4, material=synth.MAT_LXE)
+    out2 = orc.Oracle(g2, op, bvh=True).propagate(ph, 6, 1)
+    direct = (out2["fate"] == orc.FATE_DETECTED) & ((out2["flags"] & orc.H_RAYLEIGH) == 0)
+    assert direct.sum() > 1000
+    d2 = np.sqrt((out2["pos"] ** 2).sum(0))
+    n_expect = np.interp(lam.astype(np.float64), grid, op.refr_index[synth.MAT_LXE].astype(np.float64))
+    # S5 advances by the ray parameter along k; the float32 input directions are unit vectors only to ~6e-8, so the parameter is
+    # the geometric distance divided by |k|
+    knorm = np.sqrt((ph.dir.astype(np.float64) ** 2).sum(0))
+    n_seen = out2["t"] * 299.792458 / (d2 / knorm)
+    assert np.abs(n_seen[direct] - n_expect[direct]).max() < 1e-9
+    assert n_expect.min() < 1.62 and n_expect.max() > 1.76          # the ends of the table were reached (clamped beyond)
