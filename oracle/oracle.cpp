@@ -23,12 +23,18 @@
 //   emission (E1-E5): position laws (r^2, z, rho^3 uniform), isotropy, e.k = 0 and uniform azimuth of e, Gaussian spectrum with
 //                        mean 174.8 nm / FWHM 10.2 nm (Table 2), two-exponential time profile with tau_1, tau_3, f_s
 //                        (Table 2): closed-form CDFs by KS, moments (tests/test_oracle_emission.py)
+//   thin film (F1-F6)  : surface "calculated using Fresnel equations from the specified complex index of refraction and surface
+//                        thickness": d -> 0 equals the bare interface, lossless film R + T = 1, quarter- and half-wave
+//                        layers, thick absorbing film -> |r12|^2 (silicon n = 0.81, k = 1.86 of Table 8 seen from LXe: 0.436),
+//                        evanescent exit -> T = 0, against an independent characteristic-matrix computation
+//                        (tests/test_oracle_film.py).  NOT yet part of orc_propagate: coefficients and the single event only.
 //   parity unpinned: trajectories beyond what the closed forms above fix, and the paper's own
 //                    absolute LCE / t90 numbers (need the DARWIN CAD model).
 //
 // Units: mm, ns, nm.  c = 299.792458 mm/ns.
 #include <algorithm>
 #include <cmath>
+#include <complex>
 #include <cstdint>
 #include <cstring>
 #include <limits>
@@ -382,6 +388,64 @@ int set_table(Table& tb, int rows, int nl, double l0, double dl, const float* a)
 }  // namespace
 
 // =================================================================== C interface for ctypes (tests / bench)
+// ---------------------------------------------------------------- thin-film surface
+// "Surface reflectivity in Chroma can either be explicitly specified ..., or calculated using Fresnel equations from the
+// specified complex index of refraction and surface thickness."  Textbook single-film (Airy) summation: a film of complex index
+// n2 = nf + i kf and thickness d between the photon's medium n1 (real) and the material behind the triangle n3 (real).
+// [readings F-*]: amplitudes per polarisation r = (r12 + r23 E^2) / (1 + r12 r23 E^2), t = t12 t23 E / (1 + r12 r23 E^2),
+// E = exp(i 2 pi d n2 cos(theta2) / lambda), cos(theta2) = sqrt(1 - (n1 sin(theta1) / n2)^2) with the root that decays into
+// the film; T = |t|^2 n3 cos(theta3) / (n1 cos(theta1)), zero when the wave in medium 3 is evanescent; A = 1 - R - T is
+// absorbed in the film.  Mixed polarisation by intensities, as in S8.
+typedef std::complex<double> Cx;
+struct FilmCoef { double Rs, Rp, Ts, Tp, abs_rs, abs_rp, abs_ts, abs_tp; };
+inline FilmCoef film_coefficients(double n1, double nf, double kf, double d_nm, double n3, double lambda_nm, double c1) {
+  const Cx n2(nf, kf);
+  const double s1 = std::sqrt(std::max(0.0, 1.0 - c1 * c1));
+  Cx c2 = std::sqrt(Cx(1.0, 0.0) - (n1 * s1 / n2) * (n1 * s1 / n2));
+  if ((n2 * c2).imag() < 0.0 || ((n2 * c2).imag() == 0.0 && (n2 * c2).real() < 0.0)) c2 = -c2;   // decays / propagates into the film
+  const double s3 = n1 * s1 / n3;
+  const bool evanescent = s3 >= 1.0;
+  const Cx c3 = evanescent ? Cx(0.0, std::sqrt(s3 * s3 - 1.0)) : Cx(std::sqrt(1.0 - s3 * s3), 0.0);
+  const Cx E = std::exp(Cx(0.0, 1.0) * (2.0 * M_PI * d_nm / lambda_nm) * n2 * c2), E2 = E * E;
+  // s: electric field normal to the plane of incidence
+  const Cx rs12 = (n1 * c1 - n2 * c2) / (n1 * c1 + n2 * c2), rs23 = (n2 * c2 - n3 * c3) / (n2 * c2 + n3 * c3);
+  const Cx ts12 = 2.0 * n1 * c1 / (n1 * c1 + n2 * c2), ts23 = 2.0 * n2 * c2 / (n2 * c2 + n3 * c3);
+  // p: electric field in the plane of incidence
+  const Cx rp12 = (n2 * c1 - n1 * c2) / (n2 * c1 + n1 * c2), rp23 = (n3 * c2 - n2 * c3) / (n3 * c2 + n2 * c3);
+  const Cx tp12 = 2.0 * n1 * c1 / (n2 * c1 + n1 * c2), tp23 = 2.0 * n2 * c2 / (n3 * c2 + n2 * c3);
+  const Cx rs = (rs12 + rs23 * E2) / (1.0 + rs12 * rs23 * E2), rp = (rp12 + rp23 * E2) / (1.0 + rp12 * rp23 * E2);
+  const Cx ts = ts12 * ts23 * E / (1.0 + rs12 * rs23 * E2), tp = tp12 * tp23 * E / (1.0 + rp12 * rp23 * E2);
+  const double flux = evanescent ? 0.0 : n3 * c3.real() / (n1 * c1);
+  return {std::norm(rs), std::norm(rp), std::norm(ts) * flux, std::norm(tp) * flux, std::abs(rs), std::abs(rp), std::abs(ts), std::abs(tp)};
+}
+// The surface event: 0 reflected (specular), 1 transmitted into medium 3, 2 absorbed in the film.  nhat faces the photon.
+inline int film(double n1, double nf, double kf, double d_nm, double n3, double lambda_nm, V3 nhat, V3& k, V3& e, double u,
+                double& R_out, double& T_out) {
+  double ci = -dot(k, nhat);
+  V3 sv = cross(k, nhat);
+  double si = norm(sv);
+  V3 s; double Es, Ep;
+  if (si < 1e-9) { s = e; Es = 1.0; Ep = 0.0; }            // normal incidence: whole amplitude tangential
+  else { s = (1.0 / si) * sv; V3 p = cross(s, k); Es = dot(e, s); Ep = dot(e, p); }
+  const FilmCoef f = film_coefficients(n1, nf, kf, d_nm, n3, lambda_nm, ci);
+  const double R = Es * Es * f.Rs + Ep * Ep * f.Rp, T = Es * Es * f.Ts + Ep * Ep * f.Tp;
+  R_out = R; T_out = T;
+  if (u < R) {
+    V3 kr = unit(k + (2.0 * ci) * nhat);
+    e = unit((f.abs_rs * Es) * s + (f.abs_rp * Ep) * cross(s, kr));   // magnitudes kept, phases ignored (G9)
+    k = kr;
+    return 0;
+  }
+  if (u < R + T) {
+    double eta = n1 / n3, ct = std::sqrt(std::max(0.0, 1.0 - eta * eta * si * si));
+    V3 kt = unit(eta * k + (eta * ci - ct) * nhat);
+    e = unit((f.abs_ts * Es) * s + (f.abs_tp * Ep) * cross(s, kt));
+    k = kt;
+    return 1;
+  }
+  return 2;
+}
+
 // ---------------------------------------------------------------- emission
 // One scintillation photon per id, drawn from Philox blocks 0..2 of the reserved step 0xFFFFFFFF (propagation steps are
 // < 2^31, so the streams never meet).  P:144: "The emission spectrum is modeled as a Gaussian with a mean of 174.8 nm and a
@@ -441,6 +505,19 @@ void orc_emit(int shape, const double* c3, double radius, double z0, double z1, 
     const double v[11] = {x.x, x.y, x.z, k.x, k.y, k.z, e.x, e.y, e.z, lambda, t};
     for (int f = 0; f < 11; ++f) out[(size_t)f * n + i] = v[f];
   }
+}
+
+// out: Rs Rp Ts Tp
+void orc_film_coefficients(double n1, double nf, double kf, double d_nm, double n3, double lambda_nm, double cos1, double out[4]) {
+  FilmCoef f = film_coefficients(n1, nf, kf, d_nm, n3, lambda_nm, cos1);
+  out[0] = f.Rs; out[1] = f.Rp; out[2] = f.Ts; out[3] = f.Tp;
+}
+int orc_film(double n1, double nf, double kf, double d_nm, double n3, double lambda_nm, const double nhat[3], double k[3], double e[3],
+             double u, double RT[2]) {
+  V3 kk{k[0], k[1], k[2]}, ee{e[0], e[1], e[2]};
+  int oc = film(n1, nf, kf, d_nm, n3, lambda_nm, {nhat[0], nhat[1], nhat[2]}, kk, ee, u, RT[0], RT[1]);
+  k[0] = kk.x; k[1] = kk.y; k[2] = kk.z; e[0] = ee.x; e[1] = ee.y; e[2] = ee.z;
+  return oc;
 }
 
 void* orc_create() { return new Scene(); }

@@ -52,6 +52,9 @@ def lib():
         L.orc_propagate.argtypes = ([vp, i64] + [vp] * 11 + [u64, u64, i32, C.c_int] + [vp] * 8 +
                                     [i64, vp, i64, f64, f64, vp, vp, vp, C.c_int])
         L.orc_emit.argtypes = [C.c_int, vp, f64, f64, f64, f64, f64, f64, f64, f64, f64, u64, u64, i64, vp]
+        L.orc_film_coefficients.argtypes = [f64] * 7 + [vp]
+        L.orc_film.argtypes = [f64] * 6 + [vp, vp, vp, f64, vp]
+        L.orc_film.restype = C.c_int
         L.orc_philox4x32_10.argtypes = [vp, vp, vp]
         L.orc_uniforms.argtypes = [u64, u64, u32, u32, vp]
         L.orc_rayleigh.argtypes = [vp, vp, u64, u64, u32]
@@ -211,3 +214,18 @@ def emit(source: dict, seed: int, id_base: int, n: int):
                    float(source["lambda_mean"]), float(source["lambda_sigma"]), float(source["t_start"]), float(source["tau1"]),
                    float(source["tau3"]), float(source["f_singlet"]), int(seed), int(id_base), int(n), _p(out))
     return dict(pos=out[0:3], dir=out[3:6], pol=out[6:9], wavelength=out[9], t0=out[10])
+
+
+def film_coefficients(n1, nf, kf, d_nm, n3, lambda_nm, cos1):
+    """Thin-film surface: (Rs, Rp, Ts, Tp) for a film nf + i kf of thickness d between n1 and n3."""
+    out = np.zeros(4)
+    lib().orc_film_coefficients(float(n1), float(nf), float(kf), float(d_nm), float(n3), float(lambda_nm), float(cos1), _p(out))
+    return tuple(out)
+
+
+def film(n1, nf, kf, d_nm, n3, lambda_nm, nhat, k, e, u):
+    """One surface event on a film: returns (outcome 0 reflect / 1 transmit / 2 absorbed, k', e', R, T)."""
+    kk, ee, rt = np.array(k, np.float64), np.array(e, np.float64), np.zeros(2)
+    oc = lib().orc_film(float(n1), float(nf), float(kf), float(d_nm), float(n3), float(lambda_nm),
+                        _p(np.ascontiguousarray(nhat, np.float64)), _p(kk), _p(ee), float(u), _p(rt))
+    return oc, kk, ee, rt[0], rt[1]
