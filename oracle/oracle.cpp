@@ -53,7 +53,7 @@ enum : uint32_t {
   FATE_DETECTED = 0, FATE_BULK_ABSORBED = 1, FATE_SURFACE_ABSORBED = 2, FATE_ESCAPED = 3,
   FATE_TRUNCATED = 4, FATE_NAN_ABORT = 5,
   H_RAYLEIGH = 0x10, H_REFLECT_DIFFUSE = 0x20, H_REFLECT_SPECULAR = 0x40, H_SURFACE_TRANSMIT = 0x80,
-  H_FRESNEL_REFLECT = 0x100, H_FRESNEL_REFRACT = 0x200, H_TIR = 0x400
+  H_FRESNEL_REFLECT = 0x100, H_FRESNEL_REFRACT = 0x200, H_TIR = 0x400, H_FILM = 0x1000
 };
 
 struct V3 { double x, y, z; };
@@ -121,6 +121,8 @@ struct Scene {
   int64_t nt = 0;
   Table n_idx, l_abs, l_sca;           // materials
   Table p_det, p_rd, p_rs, p_tr;       // surfaces
+  Table f_n, f_k, f_d;                 // thin-film surfaces: index, extinction, thickness (nm); same grid as the surfaces
+  std::vector<int32_t> film_on;        // per surface: 1 = the surface is a film (F-model), empty = none
   std::vector<BvhNode> nodes;          // own binary BVH (optional)
   std::vector<int32_t> order;          // triangle ids in leaf order
 };
@@ -312,82 +314,6 @@ inline int fresnel(double n1, double n2, V3 nhat, V3& k, V3& e, double u, double
   return 1;
 }
 
-struct PhotonOut { uint32_t flags, steps; int32_t channel, last_tri; double t; V3 x, k, e; };
-
-// ---------------------------------------------------------------- the loop S1..S11 for one photon
-PhotonOut propagate_one(const Scene& s, V3 x, V3 k, V3 e, double lambda, double t, uint64_t seed, uint64_t pid,
-                        int32_t max_steps, bool use_bvh) {
-  PhotonOut o{};
-  uint32_t hist = 0, step = 0;
-  int32_t last_tri = -1, channel = -1;
-  uint32_t fate = FATE_TRUNCATED;                            // S10: loop exit by count
-  while ((int32_t)step < max_steps) {
-    if (!(finite3(x) && finite3(k) && finite3(e) && std::isfinite(t))) { fate = FATE_NAN_ABORT; break; }  // S11
-    Rand4 r0 = draw(seed, pid, step, 0);                     // [u_a, u_s, u_surface, u_fresnel]
-    Hit h = first_hit(s, x, k, last_tri, use_bvh);           // S1
-    if (h.tri < 0) { fate = FATE_ESCAPED; ++step; break; }   // G3
-    int64_t T = h.tri;
-    V3 v0 = s.vert[s.idx[3 * T]], v1 = s.vert[s.idx[3 * T + 1]], v2 = s.vert[s.idx[3 * T + 2]];
-    V3 ng = unit(cross(v1 - v0, v2 - v0));
-    int m1, m2; V3 nhat;                                     // S2
-    if (dot(k, ng) > 0) { m1 = s.mat_in[T]; m2 = s.mat_out[T]; nhat = (-1.0) * ng; }
-    else { m1 = s.mat_out[T]; m2 = s.mat_in[T]; nhat = ng; }
-    double n1 = s.n_idx.at(m1, lambda), La = s.l_abs.at(m1, lambda), Ls = s.l_sca.at(m1, lambda);  // S3
-    double da = std::isinf(La) ? kInf : -La * std::log(r0.u[0]);  // S4
-    double ds = std::isinf(Ls) ? kInf : -Ls * std::log(r0.u[1]);
-    if (da < ds && da < h.d) {
-      x = x + da * k; t += da * n1 / kC; fate = FATE_BULK_ABSORBED; ++step; break;
-    }
-    if (ds < h.d) {
-      x = x + ds * k; t += ds * n1 / kC;
-      if (rayleigh(k, e, seed, pid, step) < 0) { fate = FATE_NAN_ABORT; ++step; break; }
-      hist |= H_RAYLEIGH; last_tri = -1; ++step; continue;
-    }
-    x = x + h.d * k; t += h.d * n1 / kC; last_tri = h.tri;   // S4 third branch, S5
-    int sf = s.surf[T];
-    if (sf >= 0) {                                           // S7 explicit surface
-      double pd = s.p_det.at(sf, lambda), prd = s.p_rd.at(sf, lambda), prs = s.p_rs.at(sf, lambda),
-             ptr = s.p_tr.at(sf, lambda);
-      double u = r0.u[2];
-      if (u < pd) { fate = FATE_DETECTED; channel = s.chan[T]; ++step; break; }
-      else if (u < pd + prd) { lambert(nhat, k, e, draw(seed, pid, step, 1)); hist |= H_REFLECT_DIFFUSE; }
-      else if (u < pd + prd + prs) { specular(nhat, k, e); hist |= H_REFLECT_SPECULAR; }
-      else if (u < pd + prd + prs + ptr) { hist |= H_SURFACE_TRANSMIT; }
-      else { fate = FATE_SURFACE_ABSORBED; ++step; break; }
-    } else {                                                 // S8 Fresnel (P:175, P:185-187)
-      double n2 = s.n_idx.at(m2, lambda), R;
-      int oc = fresnel(n1, n2, nhat, k, e, r0.u[3], R);
-      hist |= (oc == 1) ? H_FRESNEL_REFRACT : (oc == 2 ? (H_FRESNEL_REFLECT | H_TIR) : H_FRESNEL_REFLECT);
-    }
-    ++step;                                                  // S9
-  }
-  if (fate == FATE_TRUNCATED && !(finite3(x) && finite3(k) && finite3(e) && std::isfinite(t))) fate = FATE_NAN_ABORT;
-  o.flags = fate | hist; o.steps = step; o.channel = channel; o.last_tri = last_tri; o.t = t; o.x = x; o.k = k; o.e = e;
-  return o;
-}
-
-template <class F>
-void parallel_for(int64_t n, int nthreads, F f) {
-  if (nthreads <= 1 || n < 2) { f(0, 0, n); return; }
-  nthreads = (int)std::min<int64_t>(nthreads, n);
-  std::vector<std::thread> th;
-  for (int i = 0; i < nthreads; ++i) {
-    int64_t a = n * i / nthreads, b = n * (i + 1) / nthreads;
-    th.emplace_back([=] { f(i, a, b); });
-  }
-  for (auto& t : th) t.join();
-}
-
-int set_table(Table& tb, int rows, int nl, double l0, double dl, const float* a) {
-  tb.rows = rows; tb.nl = nl; tb.l0 = l0; tb.dl = dl;
-  tb.a.assign((size_t)rows * nl, 0.0);
-  for (size_t i = 0; i < tb.a.size(); ++i) tb.a[i] = (double)a[i];
-  return 0;
-}
-
-}  // namespace
-
-// =================================================================== C interface for ctypes (tests / bench)
 // ---------------------------------------------------------------- thin-film surface
 // "Surface reflectivity in Chroma can either be explicitly specified ..., or calculated using Fresnel equations from the
 // specified complex index of refraction and surface thickness."  Textbook single-film (Airy) summation: a film of complex index
@@ -446,6 +372,94 @@ inline int film(double n1, double nf, double kf, double d_nm, double n3, double 
   return 2;
 }
 
+
+struct PhotonOut { uint32_t flags, steps; int32_t channel, last_tri; double t; V3 x, k, e; };
+
+// ---------------------------------------------------------------- the loop S1..S11 for one photon
+PhotonOut propagate_one(const Scene& s, V3 x, V3 k, V3 e, double lambda, double t, uint64_t seed, uint64_t pid,
+                        int32_t max_steps, bool use_bvh) {
+  PhotonOut o{};
+  uint32_t hist = 0, step = 0;
+  int32_t last_tri = -1, channel = -1;
+  uint32_t fate = FATE_TRUNCATED;                            // S10: loop exit by count
+  while ((int32_t)step < max_steps) {
+    if (!(finite3(x) && finite3(k) && finite3(e) && std::isfinite(t))) { fate = FATE_NAN_ABORT; break; }  // S11
+    Rand4 r0 = draw(seed, pid, step, 0);                     // [u_a, u_s, u_surface, u_fresnel]
+    Hit h = first_hit(s, x, k, last_tri, use_bvh);           // S1
+    if (h.tri < 0) { fate = FATE_ESCAPED; ++step; break; }   // G3
+    int64_t T = h.tri;
+    V3 v0 = s.vert[s.idx[3 * T]], v1 = s.vert[s.idx[3 * T + 1]], v2 = s.vert[s.idx[3 * T + 2]];
+    V3 ng = unit(cross(v1 - v0, v2 - v0));
+    int m1, m2; V3 nhat;                                     // S2
+    if (dot(k, ng) > 0) { m1 = s.mat_in[T]; m2 = s.mat_out[T]; nhat = (-1.0) * ng; }
+    else { m1 = s.mat_out[T]; m2 = s.mat_in[T]; nhat = ng; }
+    double n1 = s.n_idx.at(m1, lambda), La = s.l_abs.at(m1, lambda), Ls = s.l_sca.at(m1, lambda);  // S3
+    double da = std::isinf(La) ? kInf : -La * std::log(r0.u[0]);  // S4
+    double ds = std::isinf(Ls) ? kInf : -Ls * std::log(r0.u[1]);
+    if (da < ds && da < h.d) {
+      x = x + da * k; t += da * n1 / kC; fate = FATE_BULK_ABSORBED; ++step; break;
+    }
+    if (ds < h.d) {
+      x = x + ds * k; t += ds * n1 / kC;
+      if (rayleigh(k, e, seed, pid, step) < 0) { fate = FATE_NAN_ABORT; ++step; break; }
+      hist |= H_RAYLEIGH; last_tri = -1; ++step; continue;
+    }
+    x = x + h.d * k; t += h.d * n1 / kC; last_tri = h.tri;   // S4 third branch, S5
+    int sf = s.surf[T];
+    if (sf >= 0 && !s.film_on.empty() && s.film_on[sf]) {    // thin-film surface (second mode)
+      double n3 = s.n_idx.at(m2, lambda), R, Tt;
+      int oc = film(n1, s.f_n.at(sf, lambda), s.f_k.at(sf, lambda), s.f_d.at(sf, lambda), n3, lambda, nhat, k, e, r0.u[3], R, Tt);
+      hist |= H_FILM;
+      if (oc == 0) hist |= H_REFLECT_SPECULAR;
+      else if (oc == 1) hist |= H_SURFACE_TRANSMIT;
+      else {                                                 // absorbed in the film: detected with the surface's detect probability
+        if (r0.u[2] < s.p_det.at(sf, lambda)) { fate = FATE_DETECTED; channel = s.chan[T]; }
+        else fate = FATE_SURFACE_ABSORBED;
+        ++step; break;
+      }
+    } else if (sf >= 0) {                                    // S7 explicit surface
+      double pd = s.p_det.at(sf, lambda), prd = s.p_rd.at(sf, lambda), prs = s.p_rs.at(sf, lambda),
+             ptr = s.p_tr.at(sf, lambda);
+      double u = r0.u[2];
+      if (u < pd) { fate = FATE_DETECTED; channel = s.chan[T]; ++step; break; }
+      else if (u < pd + prd) { lambert(nhat, k, e, draw(seed, pid, step, 1)); hist |= H_REFLECT_DIFFUSE; }
+      else if (u < pd + prd + prs) { specular(nhat, k, e); hist |= H_REFLECT_SPECULAR; }
+      else if (u < pd + prd + prs + ptr) { hist |= H_SURFACE_TRANSMIT; }
+      else { fate = FATE_SURFACE_ABSORBED; ++step; break; }
+    } else {                                                 // S8 Fresnel (P:175, P:185-187)
+      double n2 = s.n_idx.at(m2, lambda), R;
+      int oc = fresnel(n1, n2, nhat, k, e, r0.u[3], R);
+      hist |= (oc == 1) ? H_FRESNEL_REFRACT : (oc == 2 ? (H_FRESNEL_REFLECT | H_TIR) : H_FRESNEL_REFLECT);
+    }
+    ++step;                                                  // S9
+  }
+  if (fate == FATE_TRUNCATED && !(finite3(x) && finite3(k) && finite3(e) && std::isfinite(t))) fate = FATE_NAN_ABORT;
+  o.flags = fate | hist; o.steps = step; o.channel = channel; o.last_tri = last_tri; o.t = t; o.x = x; o.k = k; o.e = e;
+  return o;
+}
+
+template <class F>
+void parallel_for(int64_t n, int nthreads, F f) {
+  if (nthreads <= 1 || n < 2) { f(0, 0, n); return; }
+  nthreads = (int)std::min<int64_t>(nthreads, n);
+  std::vector<std::thread> th;
+  for (int i = 0; i < nthreads; ++i) {
+    int64_t a = n * i / nthreads, b = n * (i + 1) / nthreads;
+    th.emplace_back([=] { f(i, a, b); });
+  }
+  for (auto& t : th) t.join();
+}
+
+int set_table(Table& tb, int rows, int nl, double l0, double dl, const float* a) {
+  tb.rows = rows; tb.nl = nl; tb.l0 = l0; tb.dl = dl;
+  tb.a.assign((size_t)rows * nl, 0.0);
+  for (size_t i = 0; i < tb.a.size(); ++i) tb.a[i] = (double)a[i];
+  return 0;
+}
+
+}  // namespace
+
+// =================================================================== C interface for ctypes (tests / bench)
 // ---------------------------------------------------------------- emission
 // One scintillation photon per id, drawn from Philox blocks 0..2 of the reserved step 0xFFFFFFFF (propagation steps are
 // < 2^31, so the streams never meet).  P:144: "The emission spectrum is modeled as a Gaussian with a mean of 174.8 nm and a
@@ -539,6 +553,15 @@ int orc_set_surfaces(void* h, int n_surf, int n_lambda, double lambda0, double d
   set_table(s.p_rd, n_surf, n_lambda, lambda0, dlambda, rd);
   set_table(s.p_rs, n_surf, n_lambda, lambda0, dlambda, rs);
   set_table(s.p_tr, n_surf, n_lambda, lambda0, dlambda, tr);
+  return 0;
+}
+int orc_set_films(void* h, int n_surf, int n_lambda, double lambda0, double dlambda, const int32_t* film_on, const float* nf,
+                  const float* kf, const float* d_nm) {
+  Scene& s = *(Scene*)h;
+  s.film_on.assign(film_on, film_on + n_surf);
+  set_table(s.f_n, n_surf, n_lambda, lambda0, dlambda, nf);
+  set_table(s.f_k, n_surf, n_lambda, lambda0, dlambda, kf);
+  set_table(s.f_d, n_surf, n_lambda, lambda0, dlambda, d_nm);
   return 0;
 }
 int orc_set_geometry(void* h, int64_t nv, const float* xyz, int64_t nt, const int32_t* idx, const int32_t* mat_in,

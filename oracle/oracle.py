@@ -21,6 +21,7 @@ FATE_NAMES = ("detected", "bulk_absorbed", "surface_absorbed", "escaped", "trunc
 FATE_DETECTED, FATE_BULK_ABSORBED, FATE_SURFACE_ABSORBED, FATE_ESCAPED, FATE_TRUNCATED, FATE_NAN_ABORT = range(6)
 H_RAYLEIGH, H_REFLECT_DIFFUSE, H_REFLECT_SPECULAR, H_SURFACE_TRANSMIT = 0x10, 0x20, 0x40, 0x80
 H_FRESNEL_REFLECT, H_FRESNEL_REFRACT, H_TIR = 0x100, 0x200, 0x400
+H_FILM = 0x1000
 
 
 def build(force: bool = False) -> Path:
@@ -46,6 +47,7 @@ def lib():
         L.orc_hardware_threads.restype = C.c_int
         L.orc_set_materials.argtypes = [vp, C.c_int, C.c_int, f64, f64, vp, vp, vp]
         L.orc_set_surfaces.argtypes = [vp, C.c_int, C.c_int, f64, f64, vp, vp, vp, vp]
+        L.orc_set_films.argtypes = [vp, C.c_int, C.c_int, f64, f64, vp, vp, vp, vp]
         L.orc_set_geometry.argtypes = [vp, i64, vp, i64, vp, vp, vp, vp, vp]
         L.orc_build_bvh.argtypes = [vp]
         L.orc_first_hit.argtypes = [vp, i64] + [vp] * 7 + [C.c_int, vp, vp, C.c_int]
@@ -111,6 +113,9 @@ class Oracle:
                                  _p(_f32(o.refr_index)), _p(_f32(o.abs_len)), _p(_f32(o.scat_len)))
         self.L.orc_set_surfaces(self.h, o.detect.shape[0], o.n_lambda, o.lambda0, o.dlambda, _p(_f32(o.detect)),
                                 _p(_f32(o.reflect_diffuse)), _p(_f32(o.reflect_specular)), _p(_f32(o.transmit)))
+        if getattr(o, "film_on", None) is not None:            # thin-film surfaces, on the surfaces' grid
+            self.L.orc_set_films(self.h, o.detect.shape[0], o.n_lambda, o.lambda0, o.dlambda, _p(_i32(o.film_on)),
+                                 _p(_f32(o.film_n)), _p(_f32(o.film_k)), _p(_f32(o.film_d)))
 
     def set_geometry(self, g):
         self.n_chan = int(g.n_channels)

@@ -65,6 +65,12 @@ class Optics:
     reflect_diffuse: np.ndarray
     reflect_specular: np.ndarray
     transmit: np.ndarray
+    # thin-film surfaces (optional): film_on [S] int32 (1 = the surface is a film), film_n / film_k / film_d [S,n_lambda] float32
+    # (index, extinction, thickness in nm); for a film surface `detect` is the probability that a photon absorbed in it is detected
+    film_on: np.ndarray | None = None
+    film_n: np.ndarray | None = None
+    film_k: np.ndarray | None = None
+    film_d: np.ndarray | None = None
 
 
 @dataclasses.dataclass
@@ -467,3 +473,18 @@ def config_dispersive(i: int = 1) -> Config:
         return Photons(ph.pos, ph.dir, ph.pol, lam, ph.t0, ph.id_base)
     return Config(base.name + " (dispersive tables)", base.geometry, dispersive_optics(), base.n_photons, base.seed, base.max_steps, make,
                   "synthetic dispersion on five wavelength nodes")
+
+
+def with_film(op: Optics, surface: int, nf: float, kf: float, d_nm: float, detect: float | None = None) -> Optics:
+    """Copy of `op` in which `surface` is a thin film (index nf + i kf, thickness d_nm, flat in wavelength).
+    Table 8 of the paper (PAPER.md 356-357): silicon 0.81 + 1.86 i."""
+    S, nl = op.detect.shape
+    on = np.zeros(S, np.int32) if op.film_on is None else op.film_on.copy()
+    fn = np.ones((S, nl), np.float32) if op.film_n is None else op.film_n.copy()
+    fk = np.zeros((S, nl), np.float32) if op.film_k is None else op.film_k.copy()
+    fd = np.zeros((S, nl), np.float32) if op.film_d is None else op.film_d.copy()
+    on[surface] = 1; fn[surface] = nf; fk[surface] = kf; fd[surface] = d_nm
+    det = op.detect.copy()
+    if detect is not None:
+        det[surface] = detect
+    return dataclasses.replace(op, detect=det, film_on=on, film_n=fn, film_k=fk, film_d=fd)

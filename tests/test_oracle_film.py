@@ -135,3 +135,69 @@ def test_film_event_outcomes_and_state():
     assert abs(R - 0.5 * (Rs + Rp)) < 1e-12 and abs(T - 0.5 * (Ts + Tp)) < 1e-12
     oc, k2, e2, R, _ = orc.film(N_LXE, 0.81, 1.86, 3000.0, 1.0, 175.0, nhat, np.array([0.0, 0.0, 1.0]), e, 0.1)
     assert oc == 0 and np.allclose(k2, [0, 0, -1]) and abs(R - 0.43606) < 1e-5                         # normal incidence never aborts
+
+
+# ----------------------------------------------------------------------------- the film inside the propagation loop
+from paper_2203_14354_b200 import synth          # noqa: E402
+
+
+def film_column(n_behind, nf, kf, d_nm, detect):
+    """Column: perfect detector ch 0 at z = 0, film sheet (ch 2) at z = 100 between LXe below and material 3 above, perfect detector
+    ch 1 at z = 110.  Materials: 0 LXe 1.69, 1 GXe 1.0, 2 solid, 3 'behind' (index n_behind).  No bulk processes."""
+    A = (-50.0, 50.0)
+
+    def sheet(z, mi, mo, surf, ch):
+        xyz = np.array([[A[0], A[0], z], [A[1], A[0], z], [A[1], A[1], z], [A[0], A[1], z]], np.float32)
+        return synth.Geometry(xyz, np.array([[0, 1, 2], [0, 2, 3]], np.int32), np.full(2, mi, np.int32), np.full(2, mo, np.int32),
+                              np.full(2, surf, np.int32), np.full(2, ch, np.int32), max(ch + 1, 0))
+    g = synth.merge(sheet(0.0, 2, 0, 0, 0), sheet(100.0, 0, 3, 1, 2), sheet(110.0, 3, 2, 0, 1))   # normals +z: inner below, outer above
+    g.n_channels = 3
+    f = lambda v: np.asarray(v, np.float32)[:, None].copy()
+    inf = np.inf
+    op = synth.Optics(1, 175.0, 1.0, f([1.69, 1.0, 1.0, n_behind]), f([inf] * 4), f([inf] * 4),
+                      f([1.0, detect]), f([0, 0]), f([0, 0]), f([0, 0]))                           # surface 0 perfect detector, 1 the film
+    return g, synth.with_film(op, 1, nf, kf, d_nm)
+
+
+def shoot(g, op, n, theta_deg=0.0, seed=1, x0=0.0):
+    th = math.radians(theta_deg)
+    pos = np.repeat(np.array([[x0], [0.0], [50.0]]), n, 1)
+    k = np.repeat(np.array([[math.sin(th)], [0.0], [math.cos(th)]]), n, 1)
+    e = np.repeat(np.array([[0.0], [1.0], [0.0]]), n, 1)                                          # s-polarised
+    ph = synth.Photons(pos.astype(np.float32), k.astype(np.float32), e.astype(np.float32), np.full(n, 175.0, np.float32),
+                       np.zeros(n, np.float32))
+    return orc.Oracle(g, op, bvh=False).propagate(ph, seed, 20)
+
+
+def test_film_in_the_propagation_loop_against_closed_forms():
+    n = 200_000
+    sig = lambda p: 4 * math.sqrt(max(p * (1 - p), 1e-9) / n) + 1e-12
+    # thick silicon (Table 8) seen from LXe: R = 0.43606, T = 0, the rest is absorbed and detected with probability 0.25
+    out = shoot(*film_column(1.6, 0.81, 1.86, 3000.0, 0.25), n)
+    c = out["chan_count"].astype(float) / n
+    R = ((1.69 - 0.81) ** 2 + 1.86 ** 2) / ((1.69 + 0.81) ** 2 + 1.86 ** 2)
+    assert abs(c[0] - R) < sig(R) and c[1] == 0
+    assert abs(c[2] - 0.25 * (1 - R)) < sig(0.25 * (1 - R))
+    assert int(out["fate_count"][orc.FATE_SURFACE_ABSORBED]) == n - int(out["chan_count"].sum())
+    assert np.all((out["flags"] & orc.H_FILM) != 0)
+    assert np.all(((out["flags"] & orc.H_REFLECT_SPECULAR) != 0) == (out["channel"] == 0))
+    # zero thickness between LXe and GXe: the bare interface, 6.5795 % reflected (paper: 6.5 %, P:185), nothing absorbed
+    out = shoot(*film_column(1.0, 1.3, 0.7, 0.0, 1.0), n, seed=2)
+    c = out["chan_count"].astype(float) / n
+    R = ((1.69 - 1.0) / (1.69 + 1.0)) ** 2
+    assert abs(R - 0.065795) < 1e-6 and abs(c[0] - R) < sig(R) and c[2] == 0 and abs(c[0] + c[1] - 1) < 1e-12
+    # perfect anti-reflection layer (n2^2 = n1 n3, a quarter wave): everything goes through
+    n3 = 1.2
+    nf = math.sqrt(1.69 * n3)
+    out = shoot(*film_column(n3, nf, 0.0, 175.0 / (4 * nf), 1.0), n, seed=3)
+    assert int(out["chan_count"][1]) == n
+    # oblique: transmitted photons obey Snell into medium 3 and arrive at the top detector; the reflected ones return to the bottom
+    # (start at x = -35 mm: the reflected photon is 70 mm further in x when it is back at z = 0, the sheets reach to +-50 mm)
+    out = shoot(*film_column(1.6, 0.81, 1.86, 15.0, 0.0), n, theta_deg=25.0, seed=4, x0=-35.0)
+    assert int(out["fate_count"][orc.FATE_ESCAPED]) == 0
+    Rs, _, Ts, _ = orc.film_coefficients(1.69, 0.81, 1.86, 15.0, 1.6, 175.0, math.cos(math.radians(25.0)))
+    c = out["chan_count"].astype(float) / n
+    assert abs(c[0] - Rs) < sig(Rs) and abs(c[1] - Ts) < sig(Ts) and c[2] == 0
+    top = out["channel"] == 1
+    sin3 = np.hypot(out["dir"][0][top], out["dir"][1][top])
+    assert np.abs(1.6 * sin3 - 1.69 * math.sin(math.radians(25.0))).max() < 1e-6
