@@ -11,6 +11,7 @@
  *   dw_create / dw_destroy            context on one CUDA device; owns every device copy it makes
  *   dw_set_materials                  n, L_abs, L_Rayleigh per material vs wavelength        (Table 2)
  *   dw_set_surfaces                   detect / diffuse / specular / transmit probabilities
+ *   dw_set_films                      surfaces from a complex index and a film thickness    (Table 8)
  *   dw_set_geometry                   triangle mesh + per-triangle inner/outer material, surface, channel
  *   dw_build_bvh                      device LBVH build (one-off per geometry)
  *   dw_first_hit                      nearest triangle along rays (S1) -- the parity entry of the query
@@ -63,7 +64,8 @@ enum {
   DW_H_RAYLEIGH = 0x10, DW_H_REFLECT_DIFFUSE = 0x20, DW_H_REFLECT_SPECULAR = 0x40,
   DW_H_SURFACE_TRANSMIT = 0x80, DW_H_FRESNEL_REFLECT = 0x100, DW_H_FRESNEL_REFRACT = 0x200,
   DW_H_TIR = 0x400,
-  DW_H_MEDIUM_MISMATCH = 0x800  /* carried medium != medium seen from the hit triangle (ill-formed mesh) */
+  DW_H_MEDIUM_MISMATCH = 0x800, /* carried medium != medium seen from the hit triangle (ill-formed mesh) */
+  DW_H_FILM = 0x1000            /* the last surface event was on a thin-film surface (with REFLECT_SPECULAR / SURFACE_TRANSMIT) */
 };
 
 int dw_create(int cuda_device, dw_ctx** out);
@@ -86,6 +88,19 @@ int dw_set_materials(dw_ctx* ctx, int n_mat, int n_lambda, float lambda0, float 
 int dw_set_surfaces(dw_ctx* ctx, int n_surf, int n_lambda, float lambda0, float dlambda,
                     const float* detect, const float* reflect_diffuse, const float* reflect_specular,
                     const float* transmit);
+
+/* Thin-film surfaces.  PAPER.md line 175: surface reflectivity "calculated using Fresnel equations from the
+ * specified complex index of refraction and surface thickness"; Table 8 (lines 356-357): silicon n = 0.81, k = 1.86.
+ * For every surface s with film_on[s] != 0 the explicit probabilities are not used; instead a film of index n_film + i k_film
+ * and thickness thickness_nm lies between the photon's medium (n1) and the material on the other side of the triangle (n3):
+ * amplitudes by the single-film Airy summation per polarisation, R and T mixed by intensities as in S8; one uniform number
+ * (u_fresnel) decides reflect (specular) / transmit (refracted into n3, the photon changes medium) / absorbed in the film, and an
+ * absorbed photon is DETECTED with the surface's `detect` probability (u_surface), else SURFACE_ABSORBED.  History bit DW_H_FILM.
+ * HOST pointers: film_on [n_surf], the three tables [n_surf][n_lambda] on the SAME grid as the last dw_set_surfaces (n_surf,
+ * n_lambda, lambda0, dlambda must match it: DW_E_ARG otherwise; DW_E_STATE before dw_set_surfaces).  A later dw_set_surfaces with a
+ * different shape drops the films.  k_film >= 0, thickness_nm >= 0, n_film > 0 (DW_E_RANGE).  film_on == NULL removes all films. */
+int dw_set_films(dw_ctx* ctx, int n_surf, int n_lambda, float lambda0, float dlambda, const int32_t* film_on,
+                 const float* n_film, const float* k_film, const float* thickness_nm);
 
 /* Geometry: xyz [n_vert][3] fp32, idx [n_tri][3] int32, and per triangle the inner / outer material id,
  * the surface id (-1 = none: Fresnel between the two materials, S8) and the sensor channel (-1 = none).

@@ -19,13 +19,14 @@ FATE_NAMES = ("detected", "bulk_absorbed", "surface_absorbed", "escaped", "trunc
 FATE_DETECTED, FATE_BULK_ABSORBED, FATE_SURFACE_ABSORBED, FATE_ESCAPED, FATE_TRUNCATED, FATE_NAN_ABORT = range(6)
 H_RAYLEIGH, H_REFLECT_DIFFUSE, H_REFLECT_SPECULAR, H_SURFACE_TRANSMIT = 0x10, 0x20, 0x40, 0x80
 H_FRESNEL_REFLECT, H_FRESNEL_REFRACT, H_TIR, H_MEDIUM_MISMATCH = 0x100, 0x200, 0x400, 0x800
+H_FILM = 0x1000
 PROP_UNBOUNDED_QUERY = 1
 PROP_LEGACY_SCHEDULER = 2
 PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -85,6 +86,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     L.dw_version.restype = C.c_int
     L.dw_set_materials.argtypes = [vp, C.c_int, C.c_int, f32, f32, vp, vp, vp]
     L.dw_set_surfaces.argtypes = [vp, C.c_int, C.c_int, f32, f32, vp, vp, vp, vp]
+    L.dw_set_films.argtypes = [vp, C.c_int, C.c_int, f32, f32, vp, vp, vp, vp]
     L.dw_set_geometry.argtypes = [vp, i64, vp, i64, vp, vp, vp, vp, vp, C.c_int]
     L.dw_build_bvh.argtypes = [vp, C.POINTER(BuildParams), C.POINTER(BuildStats), vp]
     L.dw_first_hit.argtypes = [vp, i64] + [vp] * 9 + [vp]
@@ -170,6 +172,17 @@ class Context:
     def set_optics(self, o):
         self.set_materials(o.refr_index, o.abs_len, o.scat_len, o.lambda0, o.dlambda)
         self.set_surfaces(o.detect, o.reflect_diffuse, o.reflect_specular, o.transmit, o.lambda0, o.dlambda)
+        if getattr(o, "film_on", None) is not None:
+            self.set_films(o.film_on, o.film_n, o.film_k, o.film_d, o.lambda0, o.dlambda)
+
+    def set_films(self, film_on, film_n, film_k, film_d, lambda0, dlambda):
+        """Thin-film surfaces: film_on int32 [S]; index, extinction, thickness (nm) float32 [S, n_lambda] on the
+        surfaces' grid.  film_on=None removes all films."""
+        if film_on is None:
+            self._check(self.L.dw_set_films(self.h, 0, 0, 0.0, 1.0, None, None, None, None))
+            return
+        on, fn, fk, fd = _np(film_on, np.int32), _np(film_n, np.float32), _np(film_k, np.float32), _np(film_d, np.float32)
+        self._check(self.L.dw_set_films(self.h, fn.shape[0], fn.shape[1], lambda0, dlambda, _hp(on), _hp(fn), _hp(fk), _hp(fd)))
 
     def set_geometry(self, g):
         xyz, idx = _np(g.xyz, np.float32), _np(g.idx, np.int32)

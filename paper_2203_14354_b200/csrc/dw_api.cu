@@ -56,7 +56,7 @@ extern "C" int dw_destroy(dw_ctx* c) {
   if (!c) return DW_OK;
   cudaSetDevice(c->device);
   free_geometry(c);
-  cudaFree(c->d_mat); cudaFree(c->d_surf);
+  cudaFree(c->d_mat); cudaFree(c->d_surf); cudaFree(c->d_film); cudaFree(c->d_film_on);
   if (c->stage) cudaFree(c->stage);
   for (int i = 0; i < 2; ++i) {
     if (c->stage_streams[i]) cudaStreamDestroy(c->stage_streams[i]);
@@ -113,9 +113,40 @@ extern "C" int dw_set_surfaces(dw_ctx* c, int n_surf, int nl, float l0, float dl
   cudaFree(c->d_surf); c->d_surf = nullptr;
   DW_CUDA(c, cudaMalloc(&c->d_surf, h.size() * sizeof(float)));
   DW_CUDA(c, cudaMemcpy(c->d_surf, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+  if (c->d_film && (n_surf != c->tables.n_surf || nl != c->tables.nl_surf || l0 != c->tables.surf_l0 || 1.0f / dl != c->tables.surf_inv_dl)) {
+    cudaFree(c->d_film); cudaFree(c->d_film_on);        // films belong to the grid they were uploaded on
+    c->d_film = nullptr; c->d_film_on = nullptr; c->tables.film = nullptr; c->tables.film_on = nullptr;
+  }
   c->tables.surf = c->d_surf; c->tables.n_surf = n_surf; c->tables.nl_surf = nl;
   c->tables.surf_l0 = l0; c->tables.surf_inv_dl = 1.0f / dl;
   c->have_surf = true;
+  return DW_OK;
+}
+
+extern "C" int dw_set_films(dw_ctx* c, int n_surf, int nl, float l0, float dl, const int32_t* film_on, const float* nf,
+                            const float* kf, const float* d_nm) {
+  if (!c) return DW_E_ARG;
+  if (!c->have_surf) return dw_fail(c, DW_E_STATE, "dw_set_films: call dw_set_surfaces first");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  DW_CUDA(c, cudaDeviceSynchronize());
+  cudaFree(c->d_film); cudaFree(c->d_film_on);
+  c->d_film = nullptr; c->d_film_on = nullptr; c->tables.film = nullptr; c->tables.film_on = nullptr;
+  if (!film_on) return DW_OK;
+  if (!nf || !kf || !d_nm) return dw_fail(c, DW_E_ARG, "dw_set_films: null table");
+  if (n_surf != c->tables.n_surf || nl != c->tables.nl_surf || l0 != c->tables.surf_l0 || !(dl > 0.f) || 1.0f / dl != c->tables.surf_inv_dl)
+    return dw_fail(c, DW_E_ARG, "dw_set_films: the grid must be the one of dw_set_surfaces (%d surfaces x %d nodes)", c->tables.n_surf, c->tables.nl_surf);
+  const size_t m = (size_t)n_surf * nl;
+  std::vector<float> h(3 * m);
+  for (size_t i = 0; i < m; ++i) {
+    if (film_on[i / nl] && (!(nf[i] > 0.f) || !(kf[i] >= 0.f) || !(d_nm[i] >= 0.f) || !isfinite(nf[i]) || !isfinite(kf[i]) || !isfinite(d_nm[i])))
+      return dw_fail(c, DW_E_RANGE, "dw_set_films: entry %zu: n = %g, k = %g, thickness = %g", i, nf[i], kf[i], d_nm[i]);
+    h[i] = nf[i]; h[m + i] = kf[i]; h[2 * m + i] = d_nm[i];
+  }
+  DW_CUDA(c, cudaMalloc(&c->d_film, h.size() * sizeof(float)));
+  DW_CUDA(c, cudaMalloc(&c->d_film_on, sizeof(int32_t) * n_surf));
+  DW_CUDA(c, cudaMemcpy(c->d_film, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+  DW_CUDA(c, cudaMemcpy(c->d_film_on, film_on, sizeof(int32_t) * n_surf, cudaMemcpyHostToDevice));
+  c->tables.film = c->d_film; c->tables.film_on = c->d_film_on;
   return DW_OK;
 }
 

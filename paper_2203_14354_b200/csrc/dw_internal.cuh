@@ -8,7 +8,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 104
+#define DW_VERSION 105
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
@@ -21,6 +21,9 @@ struct DwTables {
   const float* surf;
   int n_mat, nl_mat, n_surf, nl_surf;
   float mat_l0, mat_inv_dl, surf_l0, surf_inv_dl;
+  // thin films on the surfaces' grid: film [3][n_surf][nl_surf] = index, extinction, thickness (nm); nullptr = none
+  const float* film;
+  const int32_t* film_on;
 };
 
 // 4-wide BVH node, 128 B, read as seven float4 (SoA over the four children; the eighth float4 is padding):
@@ -59,6 +62,8 @@ struct dw_ctx {
   // tables
   float* d_mat = nullptr;
   float* d_surf = nullptr;
+  float* d_film = nullptr;
+  int32_t* d_film_on = nullptr;
   DwTables tables{};
   bool have_mat = false, have_surf = false;
   // geometry, caller order

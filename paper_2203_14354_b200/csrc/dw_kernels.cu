@@ -309,6 +309,76 @@ __device__ DW_INL_PHYS uint32_t fresnel(float n1, float n2, V3 nh, V3& k, V3& e,
   return DW_H_FRESNEL_REFRACT;
 }
 
+// ------------------------------------------------------------------------------------------------ thin-film surface (f2)
+// include/darwinopt.h "dw_set_films" (Table 8): single-film Airy summation in fp32 complex arithmetic.  Out of line on
+// purpose: it is cold code, and the propagation kernels are sensitive to their instruction footprint.
+struct Cf { float re, im; };
+__device__ __forceinline__ Cf cf(float a, float b) { Cf z; z.re = a; z.im = b; return z; }
+__device__ __forceinline__ Cf operator+(Cf a, Cf b) { return cf(a.re + b.re, a.im + b.im); }
+__device__ __forceinline__ Cf operator-(Cf a, Cf b) { return cf(a.re - b.re, a.im - b.im); }
+__device__ __forceinline__ Cf operator*(Cf a, Cf b) { return cf(fmaf(a.re, b.re, -a.im * b.im), fmaf(a.re, b.im, a.im * b.re)); }
+__device__ __forceinline__ Cf operator*(float s, Cf a) { return cf(s * a.re, s * a.im); }
+__device__ __forceinline__ Cf operator/(Cf a, Cf b) {
+  float d = 1.0f / fmaf(b.re, b.re, b.im * b.im);
+  return cf(fmaf(a.re, b.re, a.im * b.im) * d, fmaf(a.im, b.re, -a.re * b.im) * d);
+}
+__device__ __forceinline__ float cabs2(Cf a) { return fmaf(a.re, a.re, a.im * a.im); }
+__device__ __forceinline__ Cf csqrtf_(Cf a) {               // principal square root
+  float m = sqrtf(cabs2(a));
+  float re = sqrtf(fmaxf(0.f, 0.5f * (m + a.re))), im = sqrtf(fmaxf(0.f, 0.5f * (m - a.re)));
+  return cf(re, a.im < 0.f ? -im : im);
+}
+// Returns 0 reflected, 1 transmitted (crossed into the other medium), 2 absorbed in the film.  nh faces the photon.
+__device__ __noinline__ int film_event(float n1, float nf, float kf, float d_nm, float n3, float lambda, V3 nh, V3& k, V3& e, float u) {
+  const float ci = -dot(k, nh);
+  const V3 sv = cross(k, nh);
+  const float si2 = dot(sv, sv), si = sqrtf(si2);
+  V3 s; float Es, Ep;
+  if (si < 1e-5f) { s = e; Es = 1.f; Ep = 0.f; }             // normal incidence must never abort
+  else { s = (1.0f / si) * sv; V3 p = cross(s, k); Es = dot(e, s); Ep = dot(e, p); }
+  const Cf n2 = cf(nf, kf);
+  const Cf q = cf(n1 * si, 0.f) / n2;
+  Cf c2 = csqrtf_(cf(1.f, 0.f) - q * q);
+  Cf n2c2 = n2 * c2;
+  if (n2c2.im < 0.f || (n2c2.im == 0.f && n2c2.re < 0.f)) { c2 = cf(-c2.re, -c2.im); n2c2 = cf(-n2c2.re, -n2c2.im); }
+  const float s3 = n1 * si / n3;
+  const bool evan = s3 >= 1.0f;
+  const Cf c3 = evan ? cf(0.f, sqrtf(s3 * s3 - 1.0f)) : cf(sqrtf(1.0f - s3 * s3), 0.f);
+  // E = exp(i phi n2 c2), phi = 2 pi d / lambda
+  const float phi = 6.283185307179586f * d_nm / lambda;
+  float sn, cs;
+  sincosf(phi * n2c2.re, &sn, &cs);
+  const float mag = expf(-phi * n2c2.im);
+  const Cf E = cf(mag * cs, mag * sn), E2 = E * E;
+  const Cf a1 = cf(n1 * ci, 0.f), a3 = n3 * c3;             // n cos(theta) of media 1 and 3
+  const Cf rs12 = (a1 - n2c2) / (a1 + n2c2), rs23 = (n2c2 - a3) / (n2c2 + a3);
+  const Cf ts12 = (2.0f * a1) / (a1 + n2c2), ts23 = (2.0f * n2c2) / (n2c2 + a3);
+  const Cf b1 = ci * n2, b2 = n1 * c2, b3 = n3 * c2, b4 = n2 * c3;
+  const Cf rp12 = (b1 - b2) / (b1 + b2), rp23 = (b3 - b4) / (b3 + b4);
+  const Cf tp12 = (2.0f * a1) / (b1 + b2), tp23 = (2.0f * n2c2) / (b3 + b4);
+  const Cf one = cf(1.f, 0.f);
+  const Cf ds = one + rs12 * rs23 * E2, dp = one + rp12 * rp23 * E2;
+  const Cf rs = (rs12 + rs23 * E2) / ds, rp = (rp12 + rp23 * E2) / dp;
+  const Cf ts = (ts12 * ts23 * E) / ds, tp = (tp12 * tp23 * E) / dp;
+  const float flux = evan ? 0.f : n3 * c3.re / (n1 * ci);
+  const float Rs = cabs2(rs), Rp = cabs2(rp), Ts = cabs2(ts) * flux, Tp = cabs2(tp) * flux;
+  const float R = Es * Es * Rs + Ep * Ep * Rp, T = Es * Es * Ts + Ep * Ep * Tp;
+  if (u < R) {
+    V3 kr = unit(fma3(2.0f * ci, nh, k));
+    e = unit(fma3(sqrtf(Rs) * Es, s, (sqrtf(Rp) * Ep) * cross(s, kr)));   // magnitudes kept, phases ignored (G9)
+    k = kr;
+    return 0;
+  }
+  if (u < R + T) {
+    const float eta = n1 / n3, ct = sqrtf(fmaxf(0.f, 1.0f - eta * eta * si2));
+    V3 kt = unit(fma3(eta, k, (eta * ci - ct) * nh));
+    e = unit(fma3(sqrtf(cabs2(ts)) * Es, s, (sqrtf(cabs2(tp)) * Ep) * cross(s, kt)));
+    k = kt;
+    return 1;
+  }
+  return 2;
+}
+
 // ------------------------------------------------------------------------------------------------ propagation
 struct PropArgs {
   DwBvh bvh;
@@ -334,6 +404,9 @@ constexpr int kChunk = 8;   // photons claimed per lane per queue transaction (x
 // have very different lengths (short bounded scatter segments next to long surface-to-surface rays).
 enum : int { LANE_IDLE = 0, LANE_PHYS = 1, LANE_TRACE = 2 };
 
+// kFilm: thin-film surfaces are compiled in.  Two instantiations, chosen at launch by whether dw_set_films was called: merely
+// containing the (never executed) film call costs the film-free workload 21 % (C2 157 vs 199 M photons/s: spills at the call site).
+template <bool kFilm>
 __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_stack[];
   __shared__ unsigned int s_fate[8];
@@ -479,7 +552,22 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
             V3 nh = toward_outer ? mk(-ng.x, -ng.y, -ng.z) : ng;
             uint32_t cw = __float_as_uint(tc.z);
             int sf = (int)((cw >> 16) & 0xFF);
-            if (sf != 0xFF) {                                         // S7 explicit surface
+            bool is_film = false;
+            if constexpr (kFilm) is_film = sf != 0xFF && __ldg(&A.tab.film_on[sf]) != 0;
+            if (is_film) {                                            // thin-film surface (second mode)
+              const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
+              const float n3 = table_at(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+              const float fnf = table_at(A.tab.film, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fkf = table_at(A.tab.film + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fd = table_at(A.tab.film + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              int oc = 2;
+              if constexpr (kFilm) oc = film_event(n1, fnf, fkf, fd, n3, lambda, nh, k, e, r0.w);
+              hist |= DW_H_FILM;
+              if (oc == 0) hist |= DW_H_REFLECT_SPECULAR;
+              else if (oc == 1) { hist |= DW_H_SURFACE_TRANSMIT; medium = m2; }
+              else if (r0.z < table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda)) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
+              else fate = DW_FATE_SURFACE_ABSORBED;
+            } else if (sf != 0xFF) {                                  // S7 explicit surface
               const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
               float c0 = table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               float c1 = table_at(A.tab.surf + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
@@ -596,6 +684,7 @@ constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 #ifndef DW_POOL_MIN_BLOCKS
 #define DW_POOL_MIN_BLOCKS 6
 #endif
+template <bool kFilm>
 __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
   __shared__ unsigned int s_fate[8];
@@ -765,7 +854,22 @@ __global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel
             V3 nh = toward_outer ? mk(-ng.x, -ng.y, -ng.z) : ng;
             uint32_t cw = __float_as_uint(tc.z);
             int sf = (int)((cw >> 16) & 0xFF);
-            if (sf != 0xFF) {                                         // S7 explicit surface
+            bool is_film = false;
+            if constexpr (kFilm) is_film = sf != 0xFF && __ldg(&A.tab.film_on[sf]) != 0;
+            if (is_film) {                                            // thin-film surface (second mode)
+              const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
+              const float n3 = table_at(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+              const float fnf = table_at(A.tab.film, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fkf = table_at(A.tab.film + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fd = table_at(A.tab.film + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              int oc = 2;
+              if constexpr (kFilm) oc = film_event(n1, fnf, fkf, fd, n3, lambda, nh, k, e, uf);
+              hist |= DW_H_FILM;
+              if (oc == 0) hist |= DW_H_REFLECT_SPECULAR;
+              else if (oc == 1) { hist |= DW_H_SURFACE_TRANSMIT; medium = m2; }
+              else if (us < table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda)) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
+              else fate = DW_FATE_SURFACE_ABSORBED;
+            } else if (sf != 0xFF) {                                  // S7 explicit surface
               const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
               float c0 = table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               float c1 = table_at(A.tab.surf + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
@@ -1008,8 +1112,10 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   if (B < 32 || B > 128 || (B & 31)) return dw_fail(c, DW_E_ARG, "dw_propagate: block_threads must be 32, 64, 96 or 128");
   size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)kWarpInts * (B / 32);
   int per_sm = 0;
-  if (legacy) DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, propagate_kernel, B, smem));
-  else DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, propagate_pool_kernel, B, smem));
+  const bool films = c->tables.film != nullptr && c->tables.film_on != nullptr;
+  void (*kern)(PropArgs) = legacy ? (films ? propagate_kernel<true> : propagate_kernel<false>)
+                                  : (films ? propagate_pool_kernel<true> : propagate_pool_kernel<false>);
+  DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, B, smem));
   if (params && params->blocks_per_sm > 0) per_sm = std::min(per_sm, params->blocks_per_sm);
   if (per_sm < 1) return dw_fail(c, DW_E_CUDA, "dw_propagate: kernel does not fit on an SM");
   const int64_t per_warp = legacy ? 32 : kSlots;
@@ -1021,8 +1127,7 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   DW_CUDA(c, cudaMallocAsync((void**)&head, sizeof(unsigned long long), stream));
   DW_CUDA(c, cudaMemsetAsync(head, 0, sizeof(unsigned long long), stream));
   A.queue_head = head;
-  if (legacy) propagate_kernel<<<grid, B, smem, stream>>>(A);
-  else propagate_pool_kernel<<<grid, B, smem, stream>>>(A);
+  kern<<<grid, B, smem, stream>>>(A);
   cudaError_t e = cudaGetLastError();
   cudaFreeAsync(head, stream);
   if (e != cudaSuccess) return dw_fail(c, DW_E_CUDA, "propagate kernel launch failed: %s", cudaGetErrorString(e));
