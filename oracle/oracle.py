@@ -234,3 +234,45 @@ def film(n1, nf, kf, d_nm, n3, lambda_nm, nhat, k, e, u):
     oc = lib().orc_film(float(n1), float(nf), float(kf), float(d_nm), float(n3), float(lambda_nm),
                         _p(np.ascontiguousarray(nhat, np.float64)), _p(kk), _p(ee), float(u), _p(rt))
     return oc, kk, ee, rt[0], rt[1]
+
+
+# ---- design-study reductions: plain counting, which is their definition
+def tally(flags, channel, t, last_tri, photons_per_source, channel_group, n_groups, tri_component, n_components,
+          n_bins=0, t_min=0.0, dt=1.0):
+    """LCE = photons hitting the photosensitive area / photons generated, per source position and per sensor
+    array (group); line 211: arrival times of the detected photons (for t90); lines 267-271, Table 6: absorbed photons by the
+    component that absorbed them.  Photon i belongs to source i // photons_per_source."""
+    flags, channel, last_tri = np.asarray(flags), np.asarray(channel), np.asarray(last_tri)
+    n = flags.shape[0]
+    ns = -(-n // photons_per_source) if n else 0
+    out = dict(detected=np.zeros((ns, n_groups), np.uint64), time_hist=np.zeros((ns, n_bins), np.uint64),
+               fate_by_source=np.zeros((ns, 8), np.uint64), absorbed_by_component=np.zeros(n_components, np.uint64))
+    fate = flags & 0xF
+    for i in range(n):
+        s = i // photons_per_source
+        out["fate_by_source"][s, fate[i] & 7] += 1
+        if fate[i] == FATE_DETECTED:
+            c = channel[i]
+            if 0 <= c < len(channel_group) and 0 <= channel_group[c] < n_groups:
+                out["detected"][s, channel_group[c]] += 1
+            if n_bins > 0:
+                b = int(np.floor((np.float32(t[i]) - np.float32(t_min)) / np.float32(dt)))
+                out["time_hist"][s, min(max(b, 0), n_bins - 1)] += 1
+        elif fate[i] == FATE_SURFACE_ABSORBED:
+            tr = last_tri[i]
+            if 0 <= tr < len(tri_component) and 0 <= tri_component[tr] < n_components:
+                out["absorbed_by_component"][tri_component[tr]] += 1
+    return out
+
+
+def t90_from_hist(hist, t_min, dt, q=0.9):
+    """Time by which the fraction q of the detected photons has arrived, from an arrival-time histogram:
+    linear interpolation inside the bin where the cumulative count crosses q of the total.  NaN if nothing was detected."""
+    h = np.asarray(hist, np.float64)
+    tot = h.sum()
+    if tot <= 0:
+        return float("nan")
+    cum = np.cumsum(h)
+    b = int(np.searchsorted(cum, q * tot, side="left"))
+    below = cum[b - 1] if b > 0 else 0.0
+    return float(t_min + dt * (b + (q * tot - below) / h[b]))
