@@ -17,6 +17,8 @@
  *   dw_first_hit                      nearest triangle along rays (S1) -- the parity entry of the query
  *   dw_propagate                      the Monte Carlo loop S1..S13 for a photon batch, device buffers
  *   dw_propagate_host                 same, host buffers (copies inside), for end-to-end timing
+ *   dw_emit                           scintillation photons generated on the device          (Table 2)
+ *   dw_tally                          LCE per source and array, arrival-time histograms, loss table (Table 6)
  *
  * Conventions
  *   - Units mm, ns, nm.  c = 299.792458 mm/ns.  All floating point is IEEE fp32.
@@ -246,6 +248,30 @@ enum { DW_SOURCE_POINT = 0, DW_SOURCE_CYLINDER = 1, DW_SOURCE_BALL = 2 };
 /* Writes out->n photons into the eleven DEVICE arrays of `out` (they are written although the struct declares them const:
  * the same struct then goes to dw_propagate).  Asynchronous on the stream.  DW_E_ARG for a bad source or a null array. */
 int dw_emit(dw_ctx* ctx, const dw_source* source, uint64_t seed, const dw_photons* out, void* cuda_stream);
+
+
+/* Design-study reductions over the per-photon results of dw_propagate.
+ * "LCE is defined here as the number of photons hitting the photosensitive area divided by the total number of
+ * generated photons", reported per source position and separately for the top and bottom arrays (lines 249-253: ~2500 point sources
+ * on a Z x R^2 grid); line 211: t90, "the time to collect 90% of detected photons"; lines 267-271 and Table 6: where the photons that
+ * are not detected get absorbed, by component.  Photon i belongs to source i / photons_per_source (the last source may be short).
+ *   detected[s][g]            photons of source s DETECTED on a channel c with channel_group[c] == g      (LCE = detected / generated)
+ *   time_hist[s][b]           arrival times of the DETECTED photons of source s, b = floor((t - t_min) / dt) clamped to [0, n_bins)
+ *   fate_by_source[s][f]      photons of source s with fate f (8 columns; bulk absorption is column DW_FATE_BULK_ABSORBED)
+ *   absorbed_by_component[k]  SURFACE_ABSORBED photons whose last triangle t has tri_component[t] == k
+ * Everything is ACCUMULATED (the caller zeroes) and integer, so sweeps add up and the result is bit-reproducible.  All pointers are
+ * DEVICE pointers; flags is required, channel / t / last_tri only for the tables that use them; any output may be NULL.  Channels or
+ * triangles outside [0, n_chan) / [0, n_tri_map), and groups or components outside their range, are not counted.  Asynchronous. */
+typedef struct dw_tally_tables {
+  const int32_t* channel_group;  int64_t n_chan;     int32_t n_groups;      /* [n_chan]     */
+  const int32_t* tri_component;  int64_t n_tri_map;  int32_t n_components;  /* [n_tri_map], indexed by the caller's triangle id */
+  uint64_t* detected;            /* [n_sources][n_groups] */
+  uint32_t* time_hist;  int64_t n_bins;  float t_min, dt;                    /* [n_sources][n_bins] */
+  uint64_t* fate_by_source;      /* [n_sources][8] */
+  uint64_t* absorbed_by_component; /* [n_components] */
+} dw_tally_tables;
+int dw_tally(dw_ctx* ctx, const dw_results* results, int64_t n, int64_t photons_per_source, const dw_tally_tables* tables,
+             void* cuda_stream);
 
 /* Diagnostics / tests: raw Philox4x32-10 blocks and the uniforms the kernel derives from them, computed on the
  * device.  out_raw [n][4] uint32, out_u [n][4] float (either may be NULL), DEVICE pointers; entry i uses

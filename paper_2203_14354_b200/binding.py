@@ -26,7 +26,7 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -59,6 +59,12 @@ class Hists(C.Structure):
 class Source(C.Structure):
     _fields_ = [("shape", i32), ("centre", f32 * 3), ("radius", f32), ("z0", f32), ("z1", f32), ("lambda_mean", f32),
                 ("lambda_sigma", f32), ("t_start", f32), ("tau1", f32), ("tau3", f32), ("f_singlet", f32), ("reserved", i32 * 3)]
+
+
+class TallyTables(C.Structure):
+    _fields_ = [("channel_group", vp), ("n_chan", i64), ("n_groups", i32), ("tri_component", vp), ("n_tri_map", i64), ("n_components", i32),
+                ("detected", vp), ("time_hist", vp), ("n_bins", i64), ("t_min", f32), ("dt", f32), ("fate_by_source", vp),
+                ("absorbed_by_component", vp)]
 
 
 class PropagateParams(C.Structure):
@@ -96,6 +102,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
                                     C.POINTER(PropagateParams)]
     L.dw_debug_philox.argtypes = [vp, u64, u64, u32, u32, i64, vp, vp, vp]
     L.dw_emit.argtypes = [vp, C.POINTER(Source), u64, C.POINTER(Photons), vp]
+    L.dw_tally.argtypes = [vp, C.POINTER(Results), i64, i64, C.POINTER(TallyTables), vp]
     L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
     for name in EXPORTS:
         if name not in ("dw_last_error",):
@@ -213,6 +220,39 @@ class Context:
                      t_start=source["t_start"], tau1=source["tau1"], tau3=source["tau3"], f_singlet=source["f_singlet"])
         self._check(self.L.dw_emit(self.h, C.byref(src), int(seed), C.byref(out.c), _stream_ptr(stream)))
         return out
+
+    # ---- design-study reductions ------------------------------------------------------
+    def tally(self, results, n, photons_per_source, acc: "Tally", stream=None):
+        """Accumulate the per-photon `results` (DeviceResults with flags, channel, t, last_tri) into the device tables of `acc`."""
+        acc.check_sources(n, photons_per_source)
+        self._check(self.L.dw_tally(self.h, C.byref(results.c), int(n), int(photons_per_source), C.byref(acc.c), _stream_ptr(stream)))
+
+    def design_study(self, sources, photons_per_source, seed, max_steps, channel_group, n_groups, tri_component, n_components,
+                     n_bins=2000, t_min=0.0, dt=1.0, sources_per_batch=32, device="cuda:0"):
+        """The paper's design-study loop on the device: for every source emit
+        photons_per_source photons, propagate, and reduce to LCE per source and sensor array, arrival-time histograms (t90) and the
+        table of absorbed photons by component.  Photon ids are source_index * photons_per_source + i, so a result does not
+        depend on sources_per_batch.  Returns a dict of numpy arrays."""
+        import torch
+        ns = len(sources)
+        acc = Tally(ns, channel_group, n_groups, tri_component, n_components, n_bins, t_min, dt, device)
+        pps = int(photons_per_source)
+        for b0 in range(0, ns, sources_per_batch):
+            b1 = min(ns, b0 + sources_per_batch)
+            nb = (b1 - b0) * pps
+            batch = EmittedPhotons(nb, b0 * pps, device)
+            for k, src in enumerate(sources[b0:b1]):            # one emission per source into its slice of the batch
+                part = _PhotonsBase()
+                part._fill({name: batch.t[name][k * pps:(k + 1) * pps] for name in _IN}, pps, (b0 + k) * pps)
+                s = Source(shape=int(src["shape"]), centre=(f32 * 3)(*src["centre"]), radius=src["radius"], z0=src["z0"], z1=src["z1"],
+                           lambda_mean=src["lambda_mean"], lambda_sigma=src["lambda_sigma"], t_start=src["t_start"], tau1=src["tau1"],
+                           tau3=src["tau3"], f_singlet=src["f_singlet"])
+                self._check(self.L.dw_emit(self.h, C.byref(s), int(seed), C.byref(part.c), _stream_ptr()))
+            out = DeviceResults(nb, ("flags", "channel", "t", "last_tri"), device)
+            self.propagate(batch, seed, max_steps, out, None)
+            self.tally(out, nb, pps, acc.view(b0, b1))
+        torch.cuda.synchronize()
+        return acc.numpy(pps)
 
     # ---- queries -------------------------------------------------------------------------------------
     def first_hit(self, origin, direction, exclude=None, stream=None):
@@ -378,3 +418,63 @@ def make_context(geometry, optics, device: int = 0, max_leaf_tris: int = 0) -> C
     ctx.set_geometry(geometry)
     ctx.build_bvh(max_leaf_tris)
     return ctx
+
+
+class Tally:
+    """Device tables of dw_tally for n_sources sources (zeroed here; dw_tally accumulates)."""
+
+    def __init__(self, n_sources, channel_group, n_groups, tri_component, n_components, n_bins=0, t_min=0.0, dt=1.0, device="cuda:0"):
+        import torch
+        self.ns, self.G, self.K, self.nb, self.t_min, self.dt = int(n_sources), int(n_groups), int(n_components), int(n_bins), float(t_min), float(dt)
+        self.channel_group = torch.from_numpy(_np(channel_group, np.int32)).to(device)
+        self.tri_component = torch.from_numpy(_np(tri_component, np.int32)).to(device)
+        z = lambda shape, dt_: torch.zeros(shape, dtype=dt_, device=device)
+        self.detected = z((max(self.ns, 1), self.G), torch.int64)
+        self.time_hist = z((max(self.ns, 1), max(self.nb, 1)), torch.int32)
+        self.fate_by_source = z((max(self.ns, 1), 8), torch.int64)
+        self.absorbed = z((self.K,), torch.int64)
+        self.c = self._tables(0)
+        self._limit = self.ns
+
+    def _tables(self, s0):
+        return TallyTables(channel_group=vp(self.channel_group.data_ptr()), n_chan=self.channel_group.numel(), n_groups=self.G,
+                           tri_component=vp(self.tri_component.data_ptr()), n_tri_map=self.tri_component.numel(), n_components=self.K,
+                           detected=vp(self.detected[s0:].data_ptr()), time_hist=vp(self.time_hist[s0:].data_ptr()) if self.nb > 0 else None,
+                           n_bins=self.nb, t_min=self.t_min, dt=self.dt, fate_by_source=vp(self.fate_by_source[s0:].data_ptr()),
+                           absorbed_by_component=vp(self.absorbed.data_ptr()))
+
+    def view(self, s0, s1):
+        """The same tables seen from source s0 on (for a batch that holds sources s0 .. s1 - 1)."""
+        v = object.__new__(Tally)
+        v.__dict__.update(self.__dict__)
+        v.c = self._tables(s0)
+        v._limit = s1 - s0
+        return v
+
+    def check_sources(self, n, pps):
+        if -(-int(n) // int(pps)) > self._limit:
+            raise ValueError(f"{n} photons at {pps} per source need more than the {self._limit} sources of these tables")
+
+    def numpy(self, photons_per_source=None):
+        det = self.detected[: self.ns].cpu().numpy().astype(np.uint64)
+        out = dict(detected=det, time_hist=self.time_hist[: self.ns, : self.nb].cpu().numpy().view(np.uint32).astype(np.uint64),
+                   fate_by_source=self.fate_by_source[: self.ns].cpu().numpy().astype(np.uint64),
+                   absorbed_by_component=self.absorbed.cpu().numpy().astype(np.uint64))
+        if photons_per_source:
+            gen = out["fate_by_source"].sum(1).astype(np.float64)
+            out["lce"] = det / np.maximum(gen, 1.0)[:, None]                 # PAPER.md line 189
+            out["t90"] = np.array([t90_from_hist(h, self.t_min, self.dt) for h in out["time_hist"]]) if self.nb > 0 else None
+        return out
+
+
+def t90_from_hist(hist, t_min, dt, q=0.9):
+    """Time by which the fraction q of the detected photons has arrived: linear interpolation inside the bin
+    where the cumulative count crosses q of the total; NaN if nothing was detected."""
+    h = np.asarray(hist, np.float64)
+    tot = h.sum()
+    if tot <= 0:
+        return float("nan")
+    cum = np.cumsum(h)
+    b = int(np.searchsorted(cum, q * tot, side="left"))
+    below = cum[b - 1] if b > 0 else 0.0
+    return float(t_min + dt * (b + (q * tot - below) / h[b]))

@@ -271,6 +271,59 @@ extern "C" int dw_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   return dw_propagate_impl(c, in, seed, max_steps, out, hist, params, (cudaStream_t)stream);
 }
 
+// Counting over the per-photon results (dw_tally).  Neighbouring photons share their source, so equal keys are merged inside the
+// warp first (__match_any_sync) and each distinct key costs one atomic.
+__device__ __forceinline__ void warp_count64(unsigned long long* base, long long key, bool on) {
+  const int lane = threadIdx.x & 31;
+  unsigned peers = __match_any_sync(0xffffffffu, on ? key : (long long)(-1 - lane));
+  if (on && lane == (__ffs(peers) - 1)) atomicAdd(base + key, (unsigned long long)__popc(peers));
+}
+__device__ __forceinline__ void warp_count32(unsigned* base, long long key, bool on) {
+  const int lane = threadIdx.x & 31;
+  unsigned peers = __match_any_sync(0xffffffffu, on ? key : (long long)(-1 - lane));
+  if (on && lane == (__ffs(peers) - 1)) atomicAdd(base + key, (unsigned)__popc(peers));
+}
+__global__ void tally_kernel(dw_results R, int64_t n, int64_t pps, dw_tally_tables T) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  const bool live = i < n;
+  const int64_t s = live ? i / pps : 0;
+  const uint32_t fate = live ? (R.flags[i] & 0xFu) : 0xFu;
+  if (T.fate_by_source) warp_count64((unsigned long long*)T.fate_by_source, s * 8 + (fate & 7u), live);
+  const bool det = live && fate == DW_FATE_DETECTED;
+  if (T.detected && R.channel && T.channel_group) {
+    int g = -1;
+    if (det) { const int c = R.channel[i]; if (c >= 0 && c < T.n_chan) g = T.channel_group[c]; }
+    warp_count64((unsigned long long*)T.detected, s * T.n_groups + g, det && g >= 0 && g < T.n_groups);
+  }
+  if (T.time_hist && R.t && T.n_bins > 0) {
+    long long b = 0;
+    if (det) {
+      const float fb = floorf((R.t[i] - T.t_min) / T.dt);
+      b = fb < 0.f ? 0 : (fb > (float)(T.n_bins - 1) ? T.n_bins - 1 : (long long)fb);
+    }
+    warp_count32(T.time_hist, s * T.n_bins + b, det);
+  }
+  if (T.absorbed_by_component && R.last_tri && T.tri_component) {
+    int k = -1;
+    if (live && fate == DW_FATE_SURFACE_ABSORBED) { const int t = R.last_tri[i]; if (t >= 0 && t < T.n_tri_map) k = T.tri_component[t]; }
+    warp_count64((unsigned long long*)T.absorbed_by_component, k, k >= 0 && k < T.n_components);
+  }
+}
+
+extern "C" int dw_tally(dw_ctx* c, const dw_results* res, int64_t n, int64_t pps, const dw_tally_tables* T, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!res || !T || n < 0 || pps < 1) return dw_fail(c, DW_E_ARG, "dw_tally: null argument, n < 0 or photons_per_source < 1");
+  if (n == 0) return DW_OK;
+  if (!res->flags) return dw_fail(c, DW_E_ARG, "dw_tally: results->flags is required");
+  if ((T->detected && (T->n_groups < 1 || T->n_chan < 0)) || (T->absorbed_by_component && (T->n_components < 1 || T->n_tri_map < 0)) ||
+      (T->time_hist && T->n_bins > 0 && !(T->dt > 0.f)))
+    return dw_fail(c, DW_E_ARG, "dw_tally: n_groups / n_components must be >= 1 and dt > 0 for the tables that are asked for");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  tally_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*res, n, pps, *T);
+  DW_CUDA(c, cudaGetLastError());
+  return DW_OK;
+}
+
 extern "C" int dw_emit(dw_ctx* c, const dw_source* src, uint64_t seed, const dw_photons* out, void* stream) {
   if (!c) return DW_E_ARG;
   if (!src || !out) return dw_fail(c, DW_E_ARG, "dw_emit: null source or output");

@@ -8,7 +8,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 105
+#define DW_VERSION 106
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
