@@ -684,8 +684,9 @@ constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 #ifndef DW_POOL_MIN_BLOCKS
 #define DW_POOL_MIN_BLOCKS 6
 #endif
+// The film-enabled instantiation gets one block fewer per SM: at 80 registers it spills 106 bytes around the film call.
 template <bool kFilm>
-__global__ void __launch_bounds__(128, DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
+__global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
   __shared__ unsigned int s_fate[8];
   __shared__ unsigned long long s_steps;
