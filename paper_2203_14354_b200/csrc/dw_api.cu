@@ -8,7 +8,13 @@
 #include <algorithm>
 #include <vector>
 
+#include <stdlib.h>
+
 #include "dw_internal.cuh"
+
+#ifndef DW_HOST_CHUNK_DEFAULT
+#define DW_HOST_CHUNK_DEFAULT (1 << 21)
+#endif
 
 static std::string g_create_err;
 
@@ -380,7 +386,10 @@ extern "C" int dw_propagate_host(dw_ctx* c, const dw_photons* in, uint64_t seed,
   DW_CUDA(c, cudaSetDevice(c->device));
   const int64_t n = in->n;
   if (n == 0) return DW_OK;
-  const int64_t chunk = std::min<int64_t>(n, 1 << 21);
+  // photons per staged chunk: DW_HOST_CHUNK in the environment overrides the default (a tuning knob for the end-to-end path)
+  int64_t chunk_max = DW_HOST_CHUNK_DEFAULT;
+  if (const char* ev = getenv("DW_HOST_CHUNK")) { long long v = atoll(ev); if (v >= 1024) chunk_max = v; }
+  const int64_t chunk = std::min<int64_t>(n, chunk_max);
   const int64_t n_chan = hist ? hist->n_chan : 0, n_bins = hist ? hist->n_bins : 0;
   // layout: 2 slots x (11 inputs + up to 14 outputs) + histograms
   size_t per_slot = 25 * align256(sizeof(float) * chunk);
