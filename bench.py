@@ -325,6 +325,15 @@ def main():
                     algorithmic_bytes_per_launch=alg_bytes,
                     memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
                     peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)")
+    # the derived ALU peak against what this device issues in register-only streams (dw_probe_peaks: ~0.1 s, outside the timed region)
+    try:
+        pk = ctx.probe_peaks()
+        roofline["issue_probe"] = dict(fma_tlane_instr_s=pk["fma_lane_instr_per_s"] / 1e12, alu_tlane_instr_s=pk["alu_lane_instr_per_s"] / 1e12,
+                                       mix_tlane_instr_s=pk["mix_lane_instr_per_s"] / 1e12, l2_read_gbs=pk["l2_read_bytes_per_s"] / 1e9,
+                                       note="pure FP32 FMA / pure integer ALU / even mix, lane-instructions per second; peak above is the derived "
+                                            "148 x 128 x clock, which the FMA stream reaches to within a few per cent")
+    except Exception as ex:                      # the probe is context, never a reason to lose the line
+        roofline["issue_probe"] = dict(error=str(ex))
     # measured DRAM traffic per launch of the dominant kernel, from the ncu capture named in the file (null if none for this workload)
     traffic_file = ROOT / "profiles" / "traffic.csv"
     if traffic_file.exists() and n == c.n_photons and not args.legacy:

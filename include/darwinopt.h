@@ -273,6 +273,15 @@ typedef struct dw_tally_tables {
 int dw_tally(dw_ctx* ctx, const dw_results* results, int64_t n, int64_t photons_per_source, const dw_tally_tables* tables,
              void* cuda_stream);
 
+
+/* Measured denominators for the roofline (SURVEY.md 8(d) "Peaks": the driver's peaks file holds HBM and
+ * tensor numbers only).  Runs four short register-only / L2-resident kernels on the default stream and waits for them:
+ *   out[0] FP32 FMA lane-instructions / s        out[1] integer ALU (LOP3) lane-instructions / s
+ *   out[2] lane-instructions / s of an even FMA + ALU mix (what the propagation kernel issues)
+ *   out[3] bytes / s read from a 32 MiB buffer that stays in L2
+ * About 0.1 s.  Not part of the hot path. */
+int dw_probe_peaks(dw_ctx* ctx, double out[4]);
+
 /* Diagnostics / tests: raw Philox4x32-10 blocks and the uniforms the kernel derives from them, computed on the
  * device.  out_raw [n][4] uint32, out_u [n][4] float (either may be NULL), DEVICE pointers; entry i uses
  * photon id photon_id_base + i, the given step and block. */

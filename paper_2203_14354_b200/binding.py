@@ -26,7 +26,7 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -102,6 +102,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
                                     C.POINTER(PropagateParams)]
     L.dw_debug_philox.argtypes = [vp, u64, u64, u32, u32, i64, vp, vp, vp]
     L.dw_emit.argtypes = [vp, C.POINTER(Source), u64, C.POINTER(Photons), vp]
+    L.dw_probe_peaks.argtypes = [vp, vp]
     L.dw_tally.argtypes = [vp, C.POINTER(Results), i64, i64, C.POINTER(TallyTables), vp]
     L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
     for name in EXPORTS:
@@ -253,6 +254,12 @@ class Context:
             self.tally(out, nb, pps, acc.view(b0, b1))
         torch.cuda.synchronize()
         return acc.numpy(pps)
+
+    def probe_peaks(self) -> dict:
+        """Measured issue rates and L2 read bandwidth of this device (include/darwinopt.h dw_probe_peaks)."""
+        out = (C.c_double * 4)()
+        self._check(self.L.dw_probe_peaks(self.h, out))
+        return dict(fma_lane_instr_per_s=out[0], alu_lane_instr_per_s=out[1], mix_lane_instr_per_s=out[2], l2_read_bytes_per_s=out[3])
 
     # ---- queries -------------------------------------------------------------------------------------
     def first_hit(self, origin, direction, exclude=None, stream=None):
