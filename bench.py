@@ -201,6 +201,9 @@ def main():
     ap.add_argument("--ploc-radius", type=int, default=0, help="search radius of the BVH clustering rounds (0 = library default)")
     ap.add_argument("--split-div", type=int, default=0, help="split triangles longer than scene extent / this (0 = default, -1 = never)")
     ap.add_argument("--grid-res", type=int, default=0, help="cells per axis of the empty-space grid (0 = default, -1 = none)")
+    ap.add_argument("--move", default="", choices=["", "affine", "component", "jitter"], help="run on synth.moved(geometry, KIND) (diagnostic)")
+    ap.add_argument("--refit", action="store_true", help="with --move: build the tree on the original geometry and move it with dw_refit_bvh "
+                    "instead of building on the moved one (diagnostic: cost and quality of a refit)")
     ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
     ap.add_argument("--emit", action="store_true", help="generate each step's photons on the device with dw_emit inside the timed step "
                     "(SURVEY 8(f) f1; C1-C4 only) instead of propagating a resident batch")
@@ -225,8 +228,14 @@ def main():
     c, n = workload(args)
     ctx = dw.Context(local)
     ctx.set_optics(c.optics)
-    ctx.set_geometry(c.geometry)
+    from paper_2203_14354_b200 import synth as _synth
+    geom = c.geometry if (not args.move or args.refit) else _synth.moved(c.geometry, args.move)
+    ctx.set_geometry(geom)
     stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res, split_div=args.split_div)
+    refit_info = None
+    if args.move and args.refit:
+        rs = ctx.refit(_synth.moved(c.geometry, args.move).xyz)
+        refit_info = dict(refit_ms=rs["refit_ms"], loose_tris=rs["n_loose_tris"], levels=rs["n_levels"], area_ratio=rs["area_ratio"])
     id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
     ph = c.make_photons(n, id_base)
     d_ph = dw.DevicePhotons(ph, dev)
@@ -359,7 +368,8 @@ def main():
                             inputs="dw_emit on the device, a new batch of photon ids every step" if args.emit else "resident batch, same photons every step",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
                             bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
-                            grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch()),
+                            grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch(),
+                            **({"moved": args.move, "refit": refit_info} if args.move else {})),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},

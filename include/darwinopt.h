@@ -14,6 +14,7 @@
  *   dw_set_films                      surfaces from a complex index and a film thickness    (Table 8)
  *   dw_set_geometry                   triangle mesh + per-triangle inner/outer material, surface, channel
  *   dw_build_bvh                      device LBVH build (one-off per geometry)
+ *   dw_refit_bvh                      same triangles at new vertex positions, tree kept       (P:305-412 design sweeps)
  *   dw_first_hit                      nearest triangle along rays (S1) -- the parity entry of the query
  *   dw_propagate                      the Monte Carlo loop S1..S13 for a photon batch, device buffers
  *   dw_propagate_host                 same, host buffers (copies inside), for end-to-end timing
@@ -141,6 +142,26 @@ typedef struct dw_build_stats {
  * binary radix tree -> bottom-up refit -> traversal nodes + triangles permuted to leaf order.
  * params NULL = defaults; stats may be NULL.  Synchronises the stream before returning (one-off call). */
 int dw_build_bvh(dw_ctx* ctx, const dw_build_params* params, dw_build_stats* stats, void* cuda_stream);
+
+typedef struct dw_refit_stats {
+  float refit_ms;          /* device time of the whole refit (upload of the vertices included) */
+  int32_t n_levels;        /* levels of the 4-wide tree whose boxes were recomputed */
+  int32_t n_loose_tris;    /* split triangles whose number of pieces changed (split more coarsely, or pieces shared by references) */
+  int32_t grid_free_cells; /* cells of the rebuilt empty-space grid that got a triangle-free box (0 without a grid) */
+  float scene_lo[3], scene_hi[3];
+  float area_ratio;        /* sum of the half-areas of all child boxes of the tree, relative to the same sum when the tree was built:
+                            * the expected box tests per ray grow with it; well above 1 means a rebuild pays */
+} dw_refit_stats;
+
+/* Geometry variants without a rebuild (the paper's design sweeps move or reshape components of one detector,
+ * P:305-412): new vertex positions xyz [n_vert][3] for the SAME triangles (indices, materials, surfaces and channels as set by
+ * dw_set_geometry; n_vert must match).  The tree keeps its shape; triangle records, reference boxes (long triangles are clipped
+ * again; a changed piece count is fitted to the references the tree has), the boxes of all 4-wide nodes bottom-up, the length
+ * tolerance and the empty-space grid are recomputed.  The tree only decides HOW the nearest hit is found: every query gives the
+ * result a fresh dw_build_bvh on the moved geometry gives, bit for bit; large motions cost speed, not correctness.
+ * pointers_are_device as in dw_set_geometry.  DW_E_STATE before dw_build_bvh; DW_E_ARG on a size mismatch; DW_E_RANGE on a
+ * non-finite vertex or a zero-area triangle (the context then has no BVH and no valid geometry: set it again).  Synchronises. */
+int dw_refit_bvh(dw_ctx* ctx, int64_t n_vert, const float* xyz, int pointers_are_device, dw_refit_stats* stats, void* cuda_stream);
 
 /* First hit (S1): for ray i the triangle with the smallest d > 0 along o + d*dir, ignoring triangle
  * exclude_tri[i] (caller id; pointer may be NULL); exact ties -> lowest caller id.  DEVICE pointers, length n.

@@ -26,7 +26,7 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -39,6 +39,11 @@ class BuildStats(C.Structure):
     _fields_ = [("n_tri", i64), ("n_nodes", i64), ("node_bytes", i64), ("tri_bytes", i64), ("max_depth", i32),
                 ("n_leaves", i32), ("scene_lo", f32 * 3), ("scene_hi", f32 * 3), ("build_ms", f32),
                 ("ploc_rounds", i32), ("binary_depth", i32), ("grid_res", i32), ("grid_free_cells", i32), ("n_refs", i32), ("split_div", i32)]
+
+
+class RefitStats(C.Structure):
+    _fields_ = [("refit_ms", f32), ("n_levels", i32), ("n_loose_tris", i32), ("grid_free_cells", i32), ("scene_lo", f32 * 3),
+                ("scene_hi", f32 * 3), ("area_ratio", f32)]
 
 
 class Photons(C.Structure):
@@ -211,6 +216,17 @@ class Context:
         self._check(self.L.dw_build_bvh(self.h, C.byref(p), C.byref(st), _stream_ptr(stream)))
         self.stats = {k: (list(getattr(st, k)) if k.startswith("scene") else getattr(st, k)) for k, _ in BuildStats._fields_}
         return self.stats
+
+    def refit(self, xyz, stream=None) -> dict:
+        """New vertex positions (numpy [V,3] or a torch CUDA tensor) for the same triangles, under the tree of the last build_bvh
+        (SURVEY.md 8(f) f4): results equal those of a fresh build on the moved geometry, bit for bit."""
+        st = RefitStats()
+        if hasattr(xyz, "is_cuda") and xyz.is_cuda:
+            self._check(self.L.dw_refit_bvh(self.h, xyz.shape[0], _dp(xyz), 1, C.byref(st), _stream_ptr(stream)))
+        else:
+            a = _np(xyz, np.float32)
+            self._check(self.L.dw_refit_bvh(self.h, a.shape[0], _hp(a), 0, C.byref(st), _stream_ptr(stream)))
+        return {k: (list(getattr(st, k)) if k.startswith("scene") else getattr(st, k)) for k, _ in RefitStats._fields_}
 
     # ---- emission (SURVEY.md 8(f) f1) -------------------------------------------------------------------
     def emit(self, source: dict, seed: int, n: int, id_base: int = 0, device="cuda:0", stream=None) -> "EmittedPhotons":

@@ -53,9 +53,8 @@ extern "C" int dw_create(int cuda_device, dw_ctx** out) {
 static void free_geometry(dw_ctx* c) {
   cudaFree(c->d_xyz); cudaFree(c->d_idx); cudaFree(c->d_code); cudaFree(c->d_chan);
   c->d_xyz = nullptr; c->d_idx = nullptr; c->d_code = nullptr; c->d_chan = nullptr;
-  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
-  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr;
-  c->have_geom = false; c->built = false;
+  dw_bvh_free(c);
+  c->have_geom = false;
 }
 
 extern "C" int dw_destroy(dw_ctx* c) {
@@ -240,6 +239,16 @@ extern "C" int dw_build_bvh(dw_ctx* c, const dw_build_params* p, dw_build_stats*
   if (!c->have_geom) return dw_fail(c, DW_E_STATE, "dw_build_bvh: no geometry");
   DW_CUDA(c, cudaSetDevice(c->device));
   return dw_bvh_build_impl(c, p, st, (cudaStream_t)stream);
+}
+
+extern "C" int dw_refit_bvh(dw_ctx* c, int64_t n_vert, const float* xyz, int on_dev, dw_refit_stats* st, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!c->built || !c->have_geom) return dw_fail(c, DW_E_STATE, "dw_refit_bvh: build the BVH first");
+  if (n_vert != c->n_vert) return dw_fail(c, DW_E_ARG, "dw_refit_bvh: %lld vertices, the geometry has %lld", (long long)n_vert, (long long)c->n_vert);
+  if (n_vert > 0 && !xyz) return dw_fail(c, DW_E_ARG, "dw_refit_bvh: NULL array");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  DW_CUDA(c, cudaDeviceSynchronize());                           // no query of the old tree may still be running
+  return dw_bvh_refit_impl(c, xyz, on_dev, st, (cudaStream_t)stream);
 }
 
 extern "C" int dw_first_hit(dw_ctx* c, int64_t n, const float* ox, const float* oy, const float* oz, const float* dx,

@@ -78,9 +78,10 @@ __device__ int clip_axis(const float (*in)[3], int n, int axis, float val, bool 
   return m;
 }
 
-// References of one triangle.  out_lo / out_hi == nullptr: count only.  Returns the number of references.
+// References of one triangle.  out_lo / out_hi == nullptr: count only.  Returns the number of references.  cap > 0: room for
+// cap boxes; pieces beyond it are merged into the last box (the refit must fill exactly as many references as the tree has).
 __device__ int split_triangle(const float v[3][3], const float tlo[3], const float thi[3], float smax, float pad,
-                              float* out_lo, float* out_hi) {
+                              float* out_lo, float* out_hi, int cap = 0) {
   float ext = fmaxf(thi[0] - tlo[0], fmaxf(thi[1] - tlo[1], thi[2] - tlo[2]));
   if (!(ext > smax)) {
     if (out_lo) for (int c = 0; c < 3; ++c) { out_lo[c] = tlo[c]; out_hi[c] = thi[c]; }
@@ -109,7 +110,16 @@ __device__ int split_triangle(const float v[3][3], const float tlo[3], const flo
     if (hi[1] - lo[1] > e) { e = hi[1] - lo[1]; ax = 1; }
     if (hi[2] - lo[2] > e) { e = hi[2] - lo[2]; ax = 2; }
     if (e <= smax || sp + 2 > kSplitStack) {
-      if (out_lo) for (int c = 0; c < 3; ++c) { out_lo[3 * cnt + c] = lo[c] - pad; out_hi[3 * cnt + c] = hi[c] + pad; }
+      if (out_lo) {
+        if (cap > 0 && cnt >= cap) {
+          for (int c = 0; c < 3; ++c) {
+            out_lo[3 * (cap - 1) + c] = fminf(out_lo[3 * (cap - 1) + c], lo[c] - pad);
+            out_hi[3 * (cap - 1) + c] = fmaxf(out_hi[3 * (cap - 1) + c], hi[c] + pad);
+          }
+        } else {
+          for (int c = 0; c < 3; ++c) { out_lo[3 * cnt + c] = lo[c] - pad; out_hi[3 * cnt + c] = hi[c] + pad; }
+        }
+      }
       ++cnt;
       continue;
     }
@@ -365,10 +375,11 @@ __global__ void wide_single_kernel(int n, const float4* __restrict__ blo, const 
 __global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const int* __restrict__ ref_tri, const int* __restrict__ slot,
                                  const float* __restrict__ xyz, const int32_t* __restrict__ idx,
                                  const uint32_t* __restrict__ code, const int32_t* __restrict__ chan,
-                                 float4* __restrict__ tris) {
+                                 float4* __restrict__ tris, int* __restrict__ slot_ref) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   int t = ref_tri[vals[j]];                  // reference -> triangle (several references may share one)
+  slot_ref[slot[j]] = (int)vals[j];
   int i0 = idx[3 * (int64_t)t], i1 = idx[3 * (int64_t)t + 1], i2 = idx[3 * (int64_t)t + 2];
   float v0[3], e1[3], e2[3];
   for (int a = 0; a < 3; ++a) {
@@ -382,6 +393,131 @@ __global__ void pack_tris_kernel(int n, const unsigned* __restrict__ vals, const
   o[2] = make_float4(e2[2], __int_as_float(t), __uint_as_float(code[t]), __int_as_float(chan[t]));
 }
 
+
+// ---- refit (dw_refit_bvh): same triangles, same tree, new vertex positions.
+// errs[0] triangles with a non-finite vertex, errs[1] with zero area (the tests of dw_set_geometry), errs[2] first bad triangle
+__global__ void refit_check_kernel(int n, const float* __restrict__ xyz, const int32_t* __restrict__ idx,
+                                   unsigned long long* __restrict__ errs) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  float v[3][3];
+  load_tri(xyz, idx, t, v);
+  bool fin = true;
+  for (int k = 0; k < 3; ++k) for (int a = 0; a < 3; ++a) fin = fin && isfinite(v[k][a]);
+  if (!fin) { atomicAdd(&errs[0], 1ull); atomicMin(&errs[2], (unsigned long long)t); return; }
+  double e1[3], e2[3];
+  for (int a = 0; a < 3; ++a) { e1[a] = (double)v[1][a] - v[0][a]; e2[a] = (double)v[2][a] - v[0][a]; }
+  double cx = e1[1] * e2[2] - e1[2] * e2[1], cy = e1[2] * e2[0] - e1[0] * e2[2], cz = e1[0] * e2[1] - e1[1] * e2[0];
+  if (!(cx * cx + cy * cy + cz * cz > 0.0)) { atomicAdd(&errs[1], 1ull); atomicMin(&errs[2], (unsigned long long)t); }
+}
+// Boxes of the references of triangle t at its new position.  A split triangle is clipped again; its pieces need not be the
+// old ones (any set of boxes whose union covers the triangle is valid: every leaf tests the whole triangle), but the tree has a
+// fixed number of references for it: with too many pieces the triangle is split more coarsely, with too few some pieces serve two references.
+__global__ void refit_refs_kernel(int n, const float* __restrict__ xyz, const int32_t* __restrict__ idx,
+                                  const float* __restrict__ tlo, const float* __restrict__ thi,
+                                  const unsigned* __restrict__ scene, int split_div, float pad, const int* __restrict__ offs,
+                                  const int* __restrict__ counts, float* __restrict__ rlo, float* __restrict__ rhi,
+                                  int* __restrict__ n_loose) {
+  int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const int o = offs[t], cnt = counts[t];
+  const float* lo = tlo + 3 * (int64_t)t;
+  const float* hi = thi + 3 * (int64_t)t;
+  float* olo = rlo + 3 * (int64_t)o;
+  float* ohi = rhi + 3 * (int64_t)o;
+  if (cnt == 1) {
+    for (int c = 0; c < 3; ++c) { olo[c] = lo[c]; ohi[c] = hi[c]; }
+    return;
+  }
+  float v[3][3];
+  load_tri(xyz, idx, t, v);
+  float smax = split_smax(scene, split_div);
+  const int want = split_triangle(v, lo, hi, smax, 0.f, nullptr, nullptr);
+  int made = want;
+  for (int it = 0; made > cnt && it < 16; ++it) {                // more pieces than references: split more coarsely
+    smax *= 1.19f;
+    made = split_triangle(v, lo, hi, smax, 0.f, nullptr, nullptr);
+  }
+  made = split_triangle(v, lo, hi, smax, pad, olo, ohi, cnt);    // cap: a last resort, pieces beyond it are merged
+  if (made == 1 && cnt > 1)                                      // no longer split: the one box is unpadded, pad it like the others
+    for (int c = 0; c < 3; ++c) { olo[c] -= pad; ohi[c] += pad; }
+  // fewer pieces than references: reference k takes piece k * made / cnt.  Every piece is used, and since old and new pieces
+  // come in the same order along the triangle, a reference keeps a box near the leaf it sits in.  Back to front, in place.
+  if (made < cnt)
+    for (int k = cnt - 1; k >= 0; --k) {
+      const int j = (int)((int64_t)k * made / cnt);
+      for (int c = 0; c < 3; ++c) { olo[3 * k + c] = olo[3 * j + c]; ohi[3 * k + c] = ohi[3 * j + c]; }
+    }
+  if (want != cnt) atomicAdd(n_loose, 1);
+}
+// Triangle records at the new positions; the triangle of a slot is the caller id its record carries.
+__global__ void refit_pack_kernel(int n, const float* __restrict__ xyz, const int32_t* __restrict__ idx, float4* __restrict__ tris) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  float4* o = tris + 3 * (int64_t)s;
+  const float4 c = o[2];
+  const int t = __float_as_int(c.y);
+  float v[3][3];
+  load_tri(xyz, idx, t, v);
+  float e1[3], e2[3];
+  for (int a = 0; a < 3; ++a) { e1[a] = v[1][a] - v[0][a]; e2[a] = v[2][a] - v[0][a]; }
+  o[0] = make_float4(v[0][0], v[0][1], v[0][2], e1[0]);
+  o[1] = make_float4(e1[1], e1[2], e2[0], e2[1]);
+  o[2] = make_float4(e2[2], c.y, c.z, c.w);
+}
+// One level of the wide tree, deepest first: the box of a leaf child is the union of the boxes of its references, the box
+// of an internal child the union of that node's child boxes (already recomputed: children have larger indices and lie deeper).
+__global__ void refit_level_kernel(int first, int count, float4* __restrict__ nodes, const int* __restrict__ slot_ref,
+                                   const float* __restrict__ rlo, const float* __restrict__ rhi) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  const int w = first + i;
+  const float4 rf = nodes[8 * (int64_t)w + 6];
+  const int ref[4] = {__float_as_int(rf.x), __float_as_int(rf.y), __float_as_int(rf.z), __float_as_int(rf.w)};
+  float4 lo[4], hi[4];
+  for (int k = 0; k < 4; ++k) {
+    lo[k] = make_float4(FLT_MAX, FLT_MAX, FLT_MAX, 0.f); hi[k] = make_float4(-FLT_MAX, -FLT_MAX, -FLT_MAX, 0.f);
+    if (ref[k] == DW_REF_NONE) continue;
+    if (ref[k] < 0) {
+      const int code = ~ref[k], s0 = code >> 3, cnt = (code & 7) + 1;
+      for (int s = s0; s < s0 + cnt; ++s) {
+        const int64_t r = slot_ref[s];
+        lo[k] = min4(lo[k], make_float4(rlo[3 * r], rlo[3 * r + 1], rlo[3 * r + 2], 0.f));
+        hi[k] = max4(hi[k], make_float4(rhi[3 * r], rhi[3 * r + 1], rhi[3 * r + 2], 0.f));
+      }
+    } else {
+      const float4* ch = nodes + 8 * (int64_t)ref[k];
+      const float4 cr = ch[6];
+      const int cref[4] = {__float_as_int(cr.x), __float_as_int(cr.y), __float_as_int(cr.z), __float_as_int(cr.w)};
+      const float4 q0 = ch[0], q1 = ch[1], q2 = ch[2], q3 = ch[3], q4 = ch[4], q5 = ch[5];
+      const float cl[4][3] = {{q0.x, q1.x, q2.x}, {q0.y, q1.y, q2.y}, {q0.z, q1.z, q2.z}, {q0.w, q1.w, q2.w}};
+      const float chh[4][3] = {{q3.x, q4.x, q5.x}, {q3.y, q4.y, q5.y}, {q3.z, q4.z, q5.z}, {q3.w, q4.w, q5.w}};
+      for (int j = 0; j < 4; ++j) {
+        if (cref[j] == DW_REF_NONE) continue;
+        lo[k] = min4(lo[k], make_float4(cl[j][0], cl[j][1], cl[j][2], 0.f));
+        hi[k] = max4(hi[k], make_float4(chh[j][0], chh[j][1], chh[j][2], 0.f));
+      }
+    }
+  }
+  write_wide(nodes, w, lo, hi, ref);
+}
+
+// Sum over all nodes of the half-areas of their child boxes: the surface-area measure of tree quality (the expected number of box
+// tests of a random ray is proportional to it).  dw_refit_bvh reports it relative to the build.
+__global__ void node_area_kernel(int n_nodes, const float4* __restrict__ nodes, double* __restrict__ sum) {
+  int w = blockIdx.x * blockDim.x + threadIdx.x;
+  double a = 0.0;
+  if (w < n_nodes) {
+    const float4* p = nodes + 8 * (int64_t)w;
+    const float4 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], rf = p[6];
+    if (__float_as_int(rf.x) != DW_REF_NONE) a += half_area(make_float4(q0.x, q1.x, q2.x, 0.f), make_float4(q3.x, q4.x, q5.x, 0.f));
+    if (__float_as_int(rf.y) != DW_REF_NONE) a += half_area(make_float4(q0.y, q1.y, q2.y, 0.f), make_float4(q3.y, q4.y, q5.y, 0.f));
+    if (__float_as_int(rf.z) != DW_REF_NONE) a += half_area(make_float4(q0.z, q1.z, q2.z, 0.f), make_float4(q3.z, q4.z, q5.z, 0.f));
+    if (__float_as_int(rf.w) != DW_REF_NONE) a += half_area(make_float4(q0.w, q1.w, q2.w, 0.f), make_float4(q3.w, q4.w, q5.w, 0.f));
+  }
+  for (int o = 16; o; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+  if ((threadIdx.x & 31) == 0 && a != 0.0) atomicAdd(sum, a);
+}
 
 // ---- empty-space grid.  G^3 cells over the scene box.  A cell is OCCUPIED if the box of any
 // triangle, grown by `margin`, overlaps it.  Every free cell gets one axis-aligned box of free cells that contains it
@@ -460,6 +596,79 @@ static inline unsigned G_blocks(int64_t n, int B) { return (unsigned)((n + B - 1
 #define DW_B(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = dw_fail(c, DW_E_CUDA, "%s failed: %s (%s:%d)", \
     #call, cudaGetErrorString(e__), __FILE__, __LINE__); goto done; } } while (0)
 
+
+// Empty-space grid over the scene box [lo, hi] from the reference boxes (rebuilt as a whole by a refit); nothing is built for an
+// empty or flat world.  c->d_cells is allocated here if it is not there yet (GR^3 cells; a refit keeps the resolution).
+static int grid_build(dw_ctx* c, int n, const float* tlo, const float* thi, const float lo[3], const float hi[3], float eps_len,
+                      int GR, cudaStream_t stream, int* grid_built, int* grid_free, float* grid_ms) {
+  int rc = DW_OK;
+  const int B = 256;
+  int *occ = nullptr, *sat = nullptr, *cnt = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  *grid_built = 0; *grid_free = 0; *grid_ms = 0.f;
+  c->bvh.cells = nullptr; c->bvh.grid_n = 0;
+  float ext[3] = {hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]};
+  const float emax = fmaxf(ext[0], fmaxf(ext[1], ext[2]));
+  if (n <= 0 || !(emax > 0.f)) return DW_OK;
+  {
+    for (int a = 0; a < 3; ++a) ext[a] = fmaxf(ext[a], 1e-3f * emax);           // a flat axis still gets cells of finite size
+    const float3 glo = make_float3(lo[0], lo[1], lo[2]);
+    const float3 cs = make_float3(ext[0] / GR, ext[1] / GR, ext[2] / GR);
+    const float3 ics = make_float3(GR / ext[0], GR / ext[1], GR / ext[2]);
+    // margin > edge slack (2e-6 x longest edge <= 15 eps_len) + eps_len of t_max + fp32 rounding of the segment end
+    const float margin = 32.0f * eps_len;
+    const int G3 = GR * GR * GR, P = GR + 1;
+    DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
+    DW_B(cudaMalloc(&occ, 4 * (size_t)G3)); DW_B(cudaMalloc(&sat, 4 * (size_t)P * P * P)); DW_B(cudaMalloc(&cnt, 4));
+    if (!c->d_cells) DW_B(cudaMalloc(&c->d_cells, sizeof(uint2) * (size_t)G3));
+    DW_B(cudaMemsetAsync(occ, 0, 4 * (size_t)G3, stream));
+    DW_B(cudaMemsetAsync(sat, 0, 4 * (size_t)P * P * P, stream));
+    DW_B(cudaMemsetAsync(cnt, 0, 4, stream));
+    DW_B(cudaEventRecord(ev0, stream));
+    grid_mark_kernel<<<G_blocks(n, B), B, 0, stream>>>(n, tlo, thi, glo, ics, margin, GR, occ);
+    sat_x_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, occ, sat);
+    sat_y_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
+    sat_z_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
+    grid_grow_kernel<<<G_blocks(G3, B), B, 0, stream>>>(GR, occ, sat, c->d_cells, cnt);
+    DW_B(cudaGetLastError());
+    DW_B(cudaEventRecord(ev1, stream));
+    DW_B(cudaMemcpyAsync(grid_free, cnt, 4, cudaMemcpyDeviceToHost, stream));
+    DW_B(cudaStreamSynchronize(stream));
+    cudaEventElapsedTime(grid_ms, ev0, ev1);
+    *grid_built = GR;
+    c->bvh.cells = c->d_cells; c->bvh.grid_n = GR; c->bvh.grid_lo = glo; c->bvh.grid_cs = cs; c->bvh.grid_inv_cs = ics;
+  }
+done:
+  cudaFree(occ); cudaFree(sat); cudaFree(cnt);
+  if (ev0) cudaEventDestroy(ev0);
+  if (ev1) cudaEventDestroy(ev1);
+  return rc;
+}
+
+static int nodes_area(dw_ctx* c, int n_nodes, cudaStream_t stream, double* out) {
+  int rc = DW_OK;
+  double* d = nullptr;
+  *out = 0.0;
+  DW_B(cudaMalloc(&d, 8));
+  DW_B(cudaMemsetAsync(d, 0, 8, stream));
+  node_area_kernel<<<G_blocks(n_nodes, 256), 256, 0, stream>>>(n_nodes, c->d_nodes, d);
+  DW_B(cudaGetLastError());
+  DW_B(cudaMemcpyAsync(out, d, 8, cudaMemcpyDeviceToHost, stream));
+  DW_B(cudaStreamSynchronize(stream));
+done:
+  cudaFree(d);
+  return rc;
+}
+
+void dw_bvh_free(dw_ctx* c) {
+  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
+  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
+  dw_ctx::Refit& r = c->rf;
+  cudaFree(r.counts); cudaFree(r.offs); cudaFree(r.slot_ref); cudaFree(r.tlo); cudaFree(r.thi); cudaFree(r.rlo); cudaFree(r.rhi);
+  cudaFree(r.scene);
+  r = dw_ctx::Refit{};
+}
+
 int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* stats, cudaStream_t stream) {
   int rc = DW_OK;
   const int nt = (int)c->n_tri;     // triangles
@@ -474,8 +683,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   const int split_div = split_req == 0 ? 32 : split_req;
   if (split_req != -1 && (split_div < 1 || split_div > 4096)) return dw_fail(c, DW_E_ARG, "dw_build_bvh: split_div must be -1, 0 or in 1..4096");
   if (grid_req != -1 && (GR < 8 || GR > 128)) return dw_fail(c, DW_E_ARG, "dw_build_bvh: grid_res must be -1, 0 or in 8..128");
-  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
-  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
+  dw_bvh_free(c);
   if (stats) memset(stats, 0, sizeof *stats);
 
   size_t N = 0, N2 = 0;             // set after stage 0
@@ -496,6 +704,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   unsigned h_scene[6] = {0, 0, 0, 0, 0, 0};
   int h_misc[4] = {0, 0, 0, 0};      // [0] next-level tasks, [1] wide nodes, [2] leaves, [3] binary depth
   int n_nodes = 1, wide_depth = 1, ploc_rounds = 0;
+  std::vector<int> levels{0, 1};     // wide-tree level k = nodes [levels[k], levels[k+1]) (kept for dw_refit_bvh)
   const int B = 256;
   unsigned G = 0;
   const unsigned GT = (unsigned)((NT + B - 1) / B);
@@ -556,6 +765,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   tmp_bytes = std::max(tmp_bytes, tmp2);
   DW_B(cudaMalloc(&tmp, tmp_bytes));
   DW_B(cudaMalloc(&c->d_tris, 48 * N));
+  DW_B(cudaMalloc(&c->rf.slot_ref, 4 * N));
 
   if (n > 0) {
     morton_kernel<<<G, B, 0, stream>>>(n, tlo, thi, scene, keys, vals);
@@ -584,7 +794,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     }
     if (base != 2 * n - 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: %d of %d nodes made", base - n, n - 1); goto done; }
     leaf_walk_kernel<<<G, B, 0, stream>>>(n, left, parent, size, slot, leftmost, misc + 3);
-    pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, ref_tri, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris);
+    pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, ref_tri, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris, c->rf.slot_ref);
   }
   if (n <= max_leaf) {
     DW_B(cudaMalloc(&c->d_nodes, 128));
@@ -605,6 +815,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
       DW_B(cudaMemcpyAsync(&count, misc, 4, cudaMemcpyDeviceToHost, stream));
       DW_B(cudaStreamSynchronize(stream));
       DW_B(cudaMemsetAsync(misc, 0, 4, stream));
+      if (count > 0) levels.push_back(levels.back() + count);      // the children made by this launch are the next level
       cur ^= 1;
       ++wide_depth;
     }
@@ -634,36 +845,20 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     cudaEventElapsedTime(&tree_ms, ev0, ev1);                                     // before the events are reused below
     c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len, nullptr, 0, make_float3(0, 0, 0), make_float3(0, 0, 0), make_float3(0, 0, 0)};
     // ---- empty-space grid over the scene box (skipped for an empty or flat world)
-    float ext[3] = {hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2]};
-    const float emax = fmaxf(ext[0], fmaxf(ext[1], ext[2]));
-    if (grid_req != -1 && n > 0 && emax > 0.f) {
-      for (int a = 0; a < 3; ++a) ext[a] = fmaxf(ext[a], 1e-3f * emax);           // a flat axis still gets cells of finite size
-      const float3 glo = make_float3(lo[0], lo[1], lo[2]);
-      const float3 cs = make_float3(ext[0] / GR, ext[1] / GR, ext[2] / GR);
-      const float3 ics = make_float3(GR / ext[0], GR / ext[1], GR / ext[2]);
-      // margin > edge slack (2e-6 x longest edge <= 15 eps_len) + eps_len of t_max + fp32 rounding of the segment end
-      const float margin = 32.0f * eps_len;
-      const int G3 = GR * GR * GR, P = GR + 1;
-      DW_B(cudaMalloc(&occ, 4 * (size_t)G3)); DW_B(cudaMalloc(&sat, 4 * (size_t)P * P * P));
-      DW_B(cudaMalloc(&c->d_cells, sizeof(uint2) * (size_t)G3));
-      DW_B(cudaMemsetAsync(occ, 0, 4 * (size_t)G3, stream));
-      DW_B(cudaMemsetAsync(sat, 0, 4 * (size_t)P * P * P, stream));
-      DW_B(cudaMemsetAsync(misc, 0, 4, stream));
-      DW_B(cudaEventRecord(ev0, stream));
-      grid_mark_kernel<<<G_blocks(n, B), B, 0, stream>>>(n, tlo, thi, glo, ics, margin, GR, occ);
-      sat_x_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, occ, sat);
-      sat_y_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
-      sat_z_kernel<<<G_blocks(GR * GR, B), B, 0, stream>>>(GR, sat);
-      grid_grow_kernel<<<G_blocks(G3, B), B, 0, stream>>>(GR, occ, sat, c->d_cells, misc);
-      DW_B(cudaGetLastError());
-      DW_B(cudaEventRecord(ev1, stream));
-      DW_B(cudaMemcpyAsync(&grid_free, misc, 4, cudaMemcpyDeviceToHost, stream));
-      DW_B(cudaStreamSynchronize(stream));
-      cudaEventElapsedTime(&grid_ms, ev0, ev1);
-      grid_built = GR;
-      c->bvh.cells = c->d_cells; c->bvh.grid_n = GR; c->bvh.grid_lo = glo; c->bvh.grid_cs = cs; c->bvh.grid_inv_cs = ics;
+    if (grid_req != -1) {
+      rc = grid_build(c, n, tlo, thi, lo, hi, eps_len, GR, stream, &grid_built, &grid_free, &grid_ms);
+      if (rc != DW_OK) goto done;
     }
     c->built = true;
+    {   // the refit state takes over the boxes, the reference layout and the scene bounds
+      dw_ctx::Refit& r = c->rf;
+      r.n_refs = n; r.split_div = split_used; r.grid_res = grid_built;
+      r.counts = counts; r.offs = offs; r.tlo = tlo_t; r.thi = thi_t; r.rlo = tlo; r.rhi = thi; r.scene = scene;
+      counts = nullptr; offs = nullptr; tlo_t = nullptr; thi_t = nullptr; tlo = nullptr; thi = nullptr; scene = nullptr;
+      r.level_start = levels;
+      rc = nodes_area(c, n_nodes, stream, &r.build_area);
+      if (rc != DW_OK) goto done;
+    }
     if (stats) {
       stats->n_tri = nt; stats->n_refs = n; stats->split_div = split_used; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
       stats->max_depth = wide_depth; stats->n_leaves = h_misc[2];
@@ -680,6 +875,77 @@ done:
   for (int k = 0; k < 2; ++k) { cudaFree(cl[k]); cudaFree(ch[k]); cudaFree(cn[k]); cudaFree(tasks[k]); }
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
-  if (rc != DW_OK) { cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells); c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false; }
+  if (rc != DW_OK) dw_bvh_free(c);
+  return rc;
+}
+
+// dw_refit_bvh: new vertex positions under the tree of the last build (include/darwinopt.h).
+int dw_bvh_refit_impl(dw_ctx* c, const float* xyz, int on_device, dw_refit_stats* stats, cudaStream_t stream) {
+  int rc = DW_OK;
+  const int nt = (int)c->n_tri, B = 256;
+  dw_ctx::Refit& r = c->rf;
+  const int n = r.n_refs;
+  unsigned long long* errs = nullptr;
+  int* loose = nullptr;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  unsigned long long h_err[3] = {0, 0, ~0ull};
+  unsigned h_scene[6] = {0, 0, 0, 0, 0, 0};
+  int h_loose = 0, grid_built = 0, grid_free = 0;
+  float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0}, mx = 0.f, eps_len = 0.f, ms = 0.f, grid_ms = 0.f;
+  double area = 0.0;
+  if (stats) { memset(stats, 0, sizeof *stats); stats->area_ratio = 1.0f; }
+  if (nt == 0) return DW_OK;                                     // an empty world stays empty
+  DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
+  DW_B(cudaMalloc(&errs, sizeof h_err)); DW_B(cudaMalloc(&loose, 4));
+  DW_B(cudaEventRecord(ev0, stream));
+  DW_B(cudaMemcpyAsync(c->d_xyz, xyz, sizeof(float) * 3 * (size_t)c->n_vert, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, stream));
+  DW_B(cudaMemcpyAsync(errs, h_err, sizeof h_err, cudaMemcpyHostToDevice, stream));
+  DW_B(cudaMemsetAsync(loose, 0, 4, stream));
+  {
+    const unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    DW_B(cudaMemcpyAsync(r.scene, init, sizeof init, cudaMemcpyHostToDevice, stream));
+  }
+  refit_check_kernel<<<G_blocks(nt, B), B, 0, stream>>>(nt, c->d_xyz, c->d_idx, errs);
+  tri_bounds_kernel<<<G_blocks(nt, B), B, 0, stream>>>(nt, c->d_xyz, c->d_idx, r.tlo, r.thi, r.scene);
+  DW_B(cudaMemcpyAsync(h_err, errs, sizeof h_err, cudaMemcpyDeviceToHost, stream));
+  DW_B(cudaMemcpyAsync(h_scene, r.scene, sizeof h_scene, cudaMemcpyDeviceToHost, stream));
+  DW_B(cudaStreamSynchronize(stream));
+  if (h_err[0] || h_err[1]) {
+    rc = dw_fail(c, DW_E_RANGE, "dw_refit_bvh: %llu triangles with non-finite vertices, %llu with zero area (first bad triangle %llu); "
+                 "the geometry is no longer valid, set it again", h_err[0], h_err[1], h_err[2]);
+    c->have_geom = false;
+    goto done;
+  }
+  for (int a = 0; a < 3; ++a) { lo[a] = o2f(h_scene[a]); hi[a] = o2f(h_scene[3 + a]); mx = fmaxf(mx, fmaxf(fabsf(lo[a]), fabsf(hi[a]))); }
+  eps_len = 4.0f * 1.1920929e-7f * mx;                           // as in the build: tolerance and padding follow the scene
+  refit_refs_kernel<<<G_blocks(nt, B), B, 0, stream>>>(nt, c->d_xyz, c->d_idx, r.tlo, r.thi, r.scene, r.split_div, eps_len, r.offs, r.counts,
+                                                       r.rlo, r.rhi, loose);
+  refit_pack_kernel<<<G_blocks(n, B), B, 0, stream>>>(n, c->d_xyz, c->d_idx, c->d_tris);
+  for (int k = (int)r.level_start.size() - 2; k >= 0; --k) {
+    const int first = r.level_start[k], count = r.level_start[k + 1] - first;
+    refit_level_kernel<<<G_blocks(count, B), B, 0, stream>>>(first, count, c->d_nodes, r.slot_ref, r.rlo, r.rhi);
+  }
+  DW_B(cudaGetLastError());
+  DW_B(cudaMemcpyAsync(&h_loose, loose, 4, cudaMemcpyDeviceToHost, stream));
+  c->bvh.eps_len = eps_len;
+  if (r.grid_res > 0) {
+    rc = grid_build(c, n, r.rlo, r.rhi, lo, hi, eps_len, r.grid_res, stream, &grid_built, &grid_free, &grid_ms);
+    if (rc != DW_OK) goto done;
+  }
+  rc = nodes_area(c, c->bvh.n_nodes, stream, &area);
+  if (rc != DW_OK) goto done;
+  DW_B(cudaEventRecord(ev1, stream));
+  DW_B(cudaStreamSynchronize(stream));
+  cudaEventElapsedTime(&ms, ev0, ev1);
+  if (stats) {
+    stats->area_ratio = r.build_area > 0.0 ? (float)(area / r.build_area) : 1.0f;
+    stats->refit_ms = ms; stats->n_levels = (int)r.level_start.size() - 1; stats->n_loose_tris = h_loose; stats->grid_free_cells = grid_free;
+    for (int a = 0; a < 3; ++a) { stats->scene_lo[a] = lo[a]; stats->scene_hi[a] = hi[a]; }
+  }
+done:
+  cudaFree(errs); cudaFree(loose);
+  if (ev0) cudaEventDestroy(ev0);
+  if (ev1) cudaEventDestroy(ev1);
+  if (rc != DW_OK) dw_bvh_free(c);
   return rc;
 }

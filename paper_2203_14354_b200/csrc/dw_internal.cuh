@@ -5,10 +5,11 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 106
+#define DW_VERSION 107
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)
@@ -79,6 +80,18 @@ struct dw_ctx {
   uint2* d_cells = nullptr;
   DwBvh bvh{};
   bool built = false;
+  // what dw_refit_bvh needs from the last build (dw_bvh.cu); the boxes are scratch that every refit rewrites
+  struct Refit {
+    int n_refs = 0, split_div = 0, grid_res = 0;
+    double build_area = 0.0;      // sum of the half-areas of all child boxes as built
+    int* counts = nullptr;        // [n_tri] references of the triangle
+    int* offs = nullptr;          // [n_tri] its first reference
+    int* slot_ref = nullptr;      // [n_refs] leaf-order slot -> reference
+    float *tlo = nullptr, *thi = nullptr;   // [n_tri][3] triangle boxes
+    float *rlo = nullptr, *rhi = nullptr;   // [n_refs][3] reference boxes
+    unsigned* scene = nullptr;    // [6] scene bounds, order-preserving uint encoding
+    std::vector<int> level_start; // wide-tree level k = nodes [level_start[k], level_start[k+1])
+  } rf;
   // launch record
   int last_grid = 0, last_block = 0, last_smem = 0;
   int64_t n_launches = 0;
@@ -101,6 +114,8 @@ int dw_fail(dw_ctx* ctx, int code, const char* fmt, ...);
 
 // implemented in dw_bvh.cu
 int dw_bvh_build_impl(dw_ctx* ctx, const dw_build_params* params, dw_build_stats* stats, cudaStream_t stream);
+int dw_bvh_refit_impl(dw_ctx* ctx, const float* xyz, int on_device, dw_refit_stats* stats, cudaStream_t stream);
+void dw_bvh_free(dw_ctx* ctx);   // nodes, triangle records, grid and the refit state
 // implemented in dw_kernels.cu
 int dw_first_hit_impl(dw_ctx* ctx, int64_t n, const float* ox, const float* oy, const float* oz, const float* dx,
                       const float* dy, const float* dz, const int32_t* exclude, int32_t* tri, float* dist,

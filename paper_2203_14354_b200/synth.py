@@ -298,6 +298,26 @@ def merge(*geoms: Geometry) -> Geometry:
 
 
 # --------------------------------------------------------------------------- photons
+def moved(g: Geometry, kind: str) -> Geometry:
+    """The same triangles at new vertex positions, of the kind a design sweep makes (inputs of dw_refit_bvh).
+    'affine': the whole detector stretched and shifted (every box changes, long triangles change their number of pieces);
+    'component': everything above 60 % of the height lifted by 2 % of it (one part moves, the triangles across the cut stretch);
+    'jitter': every vertex displaced by up to 0.2 % of the size (seeded)."""
+    xyz = g.xyz.astype(np.float64)
+    lo, hi = xyz.min(0), xyz.max(0)
+    size = float((hi - lo).max())
+    if kind == "affine":
+        out = (xyz - lo) * np.array([1.07, 0.94, 1.11]) + lo + np.array([3.0, -2.0, 5.0])
+    elif kind == "component":
+        out = xyz.copy()
+        out[xyz[:, 2] > lo[2] + 0.6 * (hi[2] - lo[2]), 2] += 0.02 * (hi[2] - lo[2])
+    elif kind == "jitter":
+        out = xyz + np.random.default_rng(5).uniform(-0.002 * size, 0.002 * size, xyz.shape)
+    else:
+        raise ValueError(f"unknown motion '{kind}'")
+    return dataclasses.replace(g, xyz=np.ascontiguousarray(out, dtype=np.float32))
+
+
 def isotropic(rng: np.random.Generator, n: int) -> np.ndarray:
     """[3,n] float64 unit vectors, cos(theta) uniform in [-1,1], phi uniform."""
     ct = rng.uniform(-1.0, 1.0, n)

@@ -33,6 +33,7 @@ def test_struct_layouts_match_header_sizes():
     assert C.sizeof(binding.Hists) == 8 + 8 + 8 + 4 + 4 + 8 + 8 + 8
     assert C.sizeof(binding.PropagateParams) == 32
     assert C.sizeof(binding.BuildParams) == 32
+    assert C.sizeof(binding.RefitStats) == 4 + 3 * 4 + 6 * 4 + 4
     assert C.sizeof(binding.BuildStats) == 4 * 8 + 2 * 4 + 6 * 4 + 4 + 6 * 4 + 4  # build_ms, ploc_rounds, binary_depth, grid_res, grid_free_cells, n_refs, split_div + tail padding to 8
 
 
