@@ -204,6 +204,8 @@ def main():
     ap.add_argument("--move", default="", choices=["", "affine", "component", "jitter"], help="run on synth.moved(geometry, KIND) (diagnostic)")
     ap.add_argument("--refit", action="store_true", help="with --move: build the tree on the original geometry and move it with dw_refit_bvh "
                     "instead of building on the moved one (diagnostic: cost and quality of a refit)")
+    ap.add_argument("--render", type=int, default=0, help="also time dw_render on an N x N image of the detector seen from outside and from "
+                    "inside (diagnostic: the first-hit query on coherent rays; reported in config.render)")
     ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
     ap.add_argument("--emit", action="store_true", help="generate each step's photons on the device with dw_emit inside the timed step "
                     "(SURVEY 8(f) f1; C1-C4 only) instead of propagating a resident batch")
@@ -236,6 +238,23 @@ def main():
     if args.move and args.refit:
         rs = ctx.refit(_synth.moved(c.geometry, args.move).xyz)
         refit_info = dict(refit_ms=rs["refit_ms"], loose_tris=rs["n_loose_tris"], levels=rs["n_levels"], area_ratio=rs["area_ratio"])
+    render_info = None
+    if args.render > 0:
+        import numpy as _np
+        lo, hi = geom.xyz.min(0).astype(float), geom.xyz.max(0).astype(float)
+        mid, size = (lo + hi) / 2, float((hi - lo).max())
+        render_info = {}
+        for name, v in (("outside", dict(eye=mid + _np.array([1.3, 0.8, 0.9]) * size, forward=[-1.3, -0.8, -0.9], up=[0, 0, 1], fov_y_deg=40.0)),
+                        ("inside", dict(eye=mid + _np.array([0.1, -0.05, -0.25]) * size, forward=[0.4, 0.3, 0.85], up=[0, 0, 1], fov_y_deg=80.0))):
+            best = float("inf")
+            for _ in range(5):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                tri_img, _, _ = ctx.render(width=args.render, height=args.render, device=dev, **v)
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1))
+            render_info[name] = dict(ms=best, mrays_per_s=args.render ** 2 / best / 1e3, hit_fraction=float((tri_img >= 0).float().mean()))
     id_base, _ = dwdist.shard_ids(n, rank, world, weak=True)
     ph = c.make_photons(n, id_base)
     d_ph = dw.DevicePhotons(ph, dev)
@@ -369,7 +388,8 @@ def main():
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
                             bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch(),
-                            **({"moved": args.move, "refit": refit_info} if args.move else {})),
+                            **({"moved": args.move, "refit": refit_info} if args.move else {}),
+                            **({"render": render_info} if render_info else {})),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},

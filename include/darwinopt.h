@@ -16,6 +16,7 @@
  *   dw_build_bvh                      device LBVH build (one-off per geometry)
  *   dw_refit_bvh                      same triangles at new vertex positions, tree kept       (P:305-412 design sweeps)
  *   dw_first_hit                      nearest triangle along rays (S1) -- the parity entry of the query
+ *   dw_render                         S1 for the rays of a pinhole camera: ids, depths, shaded image
  *   dw_propagate                      the Monte Carlo loop S1..S13 for a photon batch, device buffers
  *   dw_propagate_host                 same, host buffers (copies inside), for end-to-end timing
  *   dw_emit                           scintillation photons generated on the device          (Table 2)
@@ -169,6 +170,22 @@ int dw_refit_bvh(dw_ctx* ctx, int64_t n_vert, const float* xyz, int pointers_are
 int dw_first_hit(dw_ctx* ctx, int64_t n, const float* ox, const float* oy, const float* oz,
                  const float* dx, const float* dy, const float* dz, const int32_t* exclude_tri,
                  int32_t* tri_out, float* dist_out, void* cuda_stream);
+
+/* Ray cast of the mesh into device buffers (the "Chroma rendering" insert of Fig. 1, without
+ * a display): a pinhole camera at `eye` looking along `forward`, image `width` x `height` pixels, vertical field of view fov_y_deg.
+ * With f = unit(forward), r = unit(f x up), u = r x f, t = tan(fov_y / 2), the ray of pixel (i, j) -- i to the right, j downwards,
+ * stored at [j * width + i] -- has direction unit(f + x t (width / height) r + y t u), x = 2 (i + 0.5) / width - 1,
+ * y = 1 - 2 (j + 0.5) / height, and is answered by the first-hit query S1 (no excluded triangle). */
+typedef struct dw_camera {
+  float eye[3], forward[3], up[3];
+  float fov_y_deg;
+  int32_t width, height;
+} dw_camera;
+/* Outputs are DEVICE pointers of width * height elements, any may be NULL: tri_out = caller id of the nearest triangle or -1,
+ * depth_out = its distance or +inf, shade_out = round(255 |n . d|) with n the unit normal of that triangle, 0 on a miss.
+ * DW_E_STATE before dw_build_bvh; DW_E_ARG for a bad size (1..32768), field of view, or an up vector parallel to forward.
+ * Asynchronous on the stream. */
+int dw_render(dw_ctx* ctx, const dw_camera* camera, int32_t* tri_out, float* depth_out, uint8_t* shade_out, void* cuda_stream);
 
 /* Photon batch, structure of arrays, each of length n (52 B per photon).  Directions and polarisations are
  * unit vectors with pol . dir = 0.  photon_id_base + i is photon i's identity in the counter-based random

@@ -236,6 +236,43 @@ def film(n1, nf, kf, d_nm, n3, lambda_nm, nhat, k, e, u):
     return oc, kk, ee, rt[0], rt[1]
 
 
+# ---- ray cast of the mesh: the definition written out, the first-hit query S1 per pixel
+def camera_rays(eye, forward, up, fov_y_deg, width, height):
+    """PAPER.md line 138 ("Chroma rendering", insert of Fig. 1) names a rendering of the mesh and no camera model; the pinhole camera of
+    include/darwinopt.h (dw_camera) is the reading: f = unit(forward), r = unit(f x up), u = r x f, t = tan(fov_y / 2); pixel (i, j),
+    i to the right and j downwards, looks along unit(f + x t (width / height) r + y t u) with x = 2 (i + 0.5) / width - 1,
+    y = 1 - 2 (j + 0.5) / height.  Returns directions [3, height * width] float64, pixel (i, j) at column j * width + i."""
+    f = np.asarray(forward, np.float64)
+    f = f / np.linalg.norm(f)
+    r = np.cross(f, np.asarray(up, np.float64))
+    r = r / np.linalg.norm(r)
+    u = np.cross(r, f)
+    t = np.tan(np.radians(np.float64(fov_y_deg)) / 2.0)
+    i = np.arange(width, dtype=np.float64)[None, :]
+    j = np.arange(height, dtype=np.float64)[:, None]
+    x = np.broadcast_to(2.0 * (i + 0.5) / width - 1.0, (height, width)).reshape(-1)
+    y = np.broadcast_to(1.0 - 2.0 * (j + 0.5) / height, (height, width)).reshape(-1)
+    d = f[:, None] + (x * t * (width / height))[None, :] * r[:, None] + (y * t)[None, :] * u[:, None]
+    return d / np.linalg.norm(d, axis=0)
+
+
+def render(oracle, geometry, eye, forward, up, fov_y_deg, width, height, use_bvh=None):
+    """Per pixel the nearest triangle along the camera ray (id, distance) and shade = round(255 |n . d|), n the unit normal of that
+    triangle; (-1, inf, 0) where nothing is hit.  `oracle` is an Oracle holding `geometry`.  Arrays [height, width]."""
+    d = camera_rays(eye, forward, up, fov_y_deg, width, height)
+    n = d.shape[1]
+    o = np.repeat(np.asarray(eye, np.float32)[:, None], n, axis=1)
+    d32 = d.astype(np.float32)            # the query takes single-precision rays (as every first-hit comparison does) ...
+    tri, dist = oracle.first_hit(o, d32, exclude=None, use_bvh=use_bvh)
+    V = np.asarray(geometry.xyz, np.float64)
+    I = np.asarray(geometry.idx)[np.maximum(tri, 0)]
+    nrm = np.cross(V[I[:, 1]] - V[I[:, 0]], V[I[:, 2]] - V[I[:, 0]])
+    nrm /= np.linalg.norm(nrm, axis=1)[:, None]
+    cosang = np.abs(np.einsum("ij,ji->i", nrm, d32.astype(np.float64)))   # ... and shades with the direction it was given
+    shade = np.where(tri >= 0, np.floor(255.0 * cosang + 0.5), 0.0).astype(np.uint8)
+    return tri.reshape(height, width), dist.reshape(height, width), shade.reshape(height, width)
+
+
 # ---- design-study reductions (SURVEY.md 8(f) f3): plain counting, which is their definition
 def tally(flags, channel, t, last_tri, photons_per_source, channel_group, n_groups, tri_component, n_components,
           n_bins=0, t_min=0.0, dt=1.0):

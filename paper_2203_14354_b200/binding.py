@@ -26,7 +26,7 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh", "dw_render")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -44,6 +44,10 @@ class BuildStats(C.Structure):
 class RefitStats(C.Structure):
     _fields_ = [("refit_ms", f32), ("n_levels", i32), ("n_loose_tris", i32), ("grid_free_cells", i32), ("scene_lo", f32 * 3),
                 ("scene_hi", f32 * 3), ("area_ratio", f32)]
+
+
+class Camera(C.Structure):
+    _fields_ = [("eye", f32 * 3), ("forward", f32 * 3), ("up", f32 * 3), ("fov_y_deg", f32), ("width", i32), ("height", i32)]
 
 
 class Photons(C.Structure):
@@ -289,6 +293,17 @@ class Context:
                                         _stream_ptr(stream)))
         return tri, dist
 
+    def render(self, eye, forward, up, fov_y_deg: float, width: int, height: int, device="cuda:0", stream=None):
+        """Ray cast of the mesh (dw_render).  Returns torch CUDA tensors [height, width]: (tri int32, depth float32, shade uint8)."""
+        import torch
+        cam = Camera(eye=(f32 * 3)(*eye), forward=(f32 * 3)(*forward), up=(f32 * 3)(*up), fov_y_deg=fov_y_deg, width=width, height=height)
+        shape = (max(int(height), 0), max(int(width), 0))
+        tri = torch.empty(shape, dtype=torch.int32, device=device)
+        depth = torch.empty(shape, dtype=torch.float32, device=device)
+        shade = torch.empty(shape, dtype=torch.uint8, device=device)
+        self._check(self.L.dw_render(self.h, C.byref(cam), _dp(tri), _dp(depth), _dp(shade), _stream_ptr(stream)))
+        return tri, depth, shade
+
     def propagate(self, ph: "DevicePhotons", seed: int, max_steps: int, out: "DeviceResults | None" = None,
                   hist: "DeviceHists | None" = None, flags: int = 0, block_threads: int = 0, blocks_per_sm: int = 0,
                   th_phys: int = 0, th_leaf: int = 0, stream=None):
@@ -432,6 +447,15 @@ class DeviceHists(_HistsBase):
 class HostHists(_HistsBase):
     def __init__(self, n_chan, n_bins=0, t_min=0.0, dt=1.0):
         self._make(n_chan, n_bins, t_min, dt)
+
+
+def write_pgm(path, shade) -> None:
+    """An 8-bit image [height, width] (numpy or torch) as a binary PGM file: the headless stand-in for a display."""
+    a = shade.cpu().numpy() if hasattr(shade, "cpu") else np.asarray(shade)
+    a = np.ascontiguousarray(a, dtype=np.uint8)
+    with open(path, "wb") as fh:
+        fh.write(b"P5\n%d %d\n255\n" % (a.shape[1], a.shape[0]))
+        fh.write(a.tobytes())
 
 
 def make_context(geometry, optics, device: int = 0, max_leaf_tris: int = 0) -> Context:

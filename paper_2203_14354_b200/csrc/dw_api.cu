@@ -262,6 +262,19 @@ extern "C" int dw_first_hit(dw_ctx* c, int64_t n, const float* ox, const float* 
   return dw_first_hit_impl(c, n, ox, oy, oz, dx, dy, dz, ex, tri, dist, (cudaStream_t)stream);
 }
 
+extern "C" int dw_render(dw_ctx* c, const dw_camera* cam, int32_t* tri, float* depth, uint8_t* shade, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!c->built) return dw_fail(c, DW_E_STATE, "dw_render: build the BVH first");
+  if (!cam) return dw_fail(c, DW_E_ARG, "dw_render: NULL camera");
+  if (cam->width < 1 || cam->height < 1 || cam->width > 32768 || cam->height > 32768)
+    return dw_fail(c, DW_E_ARG, "dw_render: image size %d x %d out of range (1..32768)", cam->width, cam->height);
+  if (!(cam->fov_y_deg > 0.f && cam->fov_y_deg < 180.f)) return dw_fail(c, DW_E_ARG, "dw_render: fov_y_deg must be in (0, 180)");
+  for (int a = 0; a < 3; ++a)
+    if (!isfinite(cam->eye[a])) return dw_fail(c, DW_E_ARG, "dw_render: eye must be finite");
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_render_impl(c, cam, tri, depth, shade, (cudaStream_t)stream);
+}
+
 static int check_batch(dw_ctx* c, const char* who, const dw_photons* in, int32_t max_steps, const dw_hists* h) {
   if (!c->built) return dw_fail(c, DW_E_STATE, "%s: build the BVH first", who);
   if (!in || in->n < 0 || max_steps < 0) return dw_fail(c, DW_E_ARG, "%s: bad batch / max_steps", who);

@@ -1086,6 +1086,49 @@ __global__ void philox_debug_kernel(uint64_t seed, uint64_t base, uint32_t step,
   if (out_u) { out_u[4 * i] = u01(r.x); out_u[4 * i + 1] = u01(r.y); out_u[4 * i + 2] = u01(r.z); out_u[4 * i + 3] = u01(r.w); }
 }
 
+// ------------------------------------------------------------------------------------------------ ray cast of the mesh (dw_render)
+// One pinhole-camera ray per pixel through the first-hit query: the part of the paper's "Chroma rendering" (insert of
+// Fig. 1) that needs no display.  Pixel (i, j), i to the right, j downwards: d = unit(f + x r + y u) with x = 2 (i + 0.5) / w - 1,
+// y = 1 - 2 (j + 0.5) / h and r, u already scaled by tan(fov / 2) (and the aspect ratio) on the host.  A warp covers an 8 x 4 pixel
+// tile so that its rays stay together in the tree.  shade = round(255 |n . d|), 0 where nothing is hit.
+struct DwCameraDev { float eye[3], f[3], r[3], u[3]; int w, h; };
+__global__ void __launch_bounds__(128) render_kernel(DwBvh bvh, DwCameraDev cam, int32_t* __restrict__ tri, float* __restrict__ depth,
+                                                     uint8_t* __restrict__ shade) {
+  extern __shared__ int s_stack[];
+  int lstack[kStackLocal];
+  const int tiles_x = (cam.w + 15) / 16;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = (blockIdx.x % tiles_x) * 16 + (warp & 1) * 8 + (lane & 7);
+  const int j = (blockIdx.x / tiles_x) * 8 + (warp >> 1) * 4 + (lane >> 3);
+  if (i >= cam.w || j >= cam.h) return;
+  const float x = 2.0f * ((float)i + 0.5f) / (float)cam.w - 1.0f, y = 1.0f - 2.0f * ((float)j + 0.5f) / (float)cam.h;
+  const V3 d = unit(mk(fmaf(x, cam.r[0], fmaf(y, cam.u[0], cam.f[0])), fmaf(x, cam.r[1], fmaf(y, cam.u[1], cam.f[1])),
+                       fmaf(x, cam.r[2], fmaf(y, cam.u[2], cam.f[2]))));
+  Ray r;
+  ray_setup(r, mk(cam.eye[0], cam.eye[1], cam.eye[2]), d);
+  TraceState s;
+  ts_begin(s, INFINITY);
+  int* my = s_stack + threadIdx.x;
+  while (s.node != kDone) {
+    if (s.node >= 0) step_internal(bvh, r, s, my, blockDim.x, lstack);
+    else step_triangle(bvh, r, s, -1, -1, my, blockDim.x, lstack);
+  }
+  const int64_t px = (int64_t)j * cam.w + i;
+  const bool hit = s.best_slot >= 0;
+  if (tri) tri[px] = hit ? s.best_id : -1;
+  if (depth) depth[px] = hit ? s.best_t : INFINITY;
+  if (shade) {
+    float v = 0.f;
+    if (hit) {
+      const float4* p = bvh.tris + 3 * (size_t)s.best_slot;
+      const float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+      const V3 n = unit(cross(mk(a.w, b.x, b.y), mk(b.z, b.w, c.x)));
+      v = floorf(fmaf(255.0f, fabsf(dot(n, d)), 0.5f));
+    }
+    shade[px] = (uint8_t)fminf(v, 255.f);
+  }
+}
+
 }  // namespace
 
 int dw_first_hit_impl(dw_ctx* c, int64_t n, const float* ox, const float* oy, const float* oz, const float* dx,
@@ -1093,6 +1136,31 @@ int dw_first_hit_impl(dw_ctx* c, int64_t n, const float* ox, const float* oy, co
   const int B = 128;
   size_t smem = sizeof(int) * kStackShared * B;
   first_hit_kernel<<<(unsigned)((n + B - 1) / B), B, smem, stream>>>(c->bvh, n, ox, oy, oz, dx, dy, dz, exclude, tri, dist);
+  DW_CUDA(c, cudaGetLastError());
+  return DW_OK;
+}
+
+int dw_render_impl(dw_ctx* c, const dw_camera* cam, int32_t* tri, float* depth, uint8_t* shade, cudaStream_t stream) {
+  // camera basis in double precision: f = unit(forward), r = unit(f x up), u = r x f, then r and u scaled to the image half-sizes
+  double f[3] = {cam->forward[0], cam->forward[1], cam->forward[2]}, up[3] = {cam->up[0], cam->up[1], cam->up[2]};
+  const double fl = sqrt(f[0] * f[0] + f[1] * f[1] + f[2] * f[2]);
+  if (!(fl > 0.0) || !isfinite(fl)) return dw_fail(c, DW_E_ARG, "dw_render: forward must be a finite non-zero vector");
+  for (int a = 0; a < 3; ++a) f[a] /= fl;
+  double r[3] = {f[1] * up[2] - f[2] * up[1], f[2] * up[0] - f[0] * up[2], f[0] * up[1] - f[1] * up[0]};
+  const double rl = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+  const double ul = sqrt(up[0] * up[0] + up[1] * up[1] + up[2] * up[2]);
+  if (!(rl > 1e-6 * ul) || !isfinite(rl)) return dw_fail(c, DW_E_ARG, "dw_render: up must be finite and not parallel to forward");
+  for (int a = 0; a < 3; ++a) r[a] /= rl;
+  const double u[3] = {r[1] * f[2] - r[2] * f[1], r[2] * f[0] - r[0] * f[2], r[0] * f[1] - r[1] * f[0]};
+  const double th = tan(0.5 * (double)cam->fov_y_deg * 3.14159265358979323846 / 180.0), aspect = (double)cam->width / (double)cam->height;
+  DwCameraDev d;
+  for (int a = 0; a < 3; ++a) {
+    d.eye[a] = cam->eye[a]; d.f[a] = (float)f[a]; d.r[a] = (float)(r[a] * th * aspect); d.u[a] = (float)(u[a] * th);
+  }
+  d.w = cam->width; d.h = cam->height;
+  const int B = 128;
+  const unsigned tiles = (unsigned)(((cam->width + 15) / 16) * (int64_t)((cam->height + 7) / 8));
+  render_kernel<<<tiles, B, sizeof(int) * kStackShared * B, stream>>>(c->bvh, d, tri, depth, shade);
   DW_CUDA(c, cudaGetLastError());
   return DW_OK;
 }
