@@ -118,7 +118,7 @@ class ClockSampler:
 
 def workload(args):
     from paper_2203_14354_b200 import synth
-    c = synth.config(args.config)
+    c = synth.config_design(args.design, 2) if getattr(args, "design", "") else synth.config(args.config)
     n = args.photons or c.n_photons
     return c, n
 
@@ -201,6 +201,8 @@ def main():
     ap.add_argument("--ploc-radius", type=int, default=0, help="search radius of the BVH clustering rounds (0 = library default)")
     ap.add_argument("--split-div", type=int, default=0, help="split triangles longer than scene extent / this (0 = default, -1 = never)")
     ap.add_argument("--grid-res", type=int, default=0, help="cells per axis of the empty-space grid (0 = default, -1 = none)")
+    ap.add_argument("--design", default="", choices=["", "baseline", "detailed_pmt", "side_sensors", "both"],
+                    help="run on synth.config_design(VARIANT) at C2 size instead of a BASELINE.json config (SURVEY 8(f) f4, diagnostic)")
     ap.add_argument("--move", default="", choices=["", "affine", "component", "jitter"], help="run on synth.moved(geometry, KIND) (diagnostic)")
     ap.add_argument("--refit", action="store_true", help="with --move: build the tree on the original geometry and move it with dw_refit_bvh "
                     "instead of building on the moved one (diagnostic: cost and quality of a refit)")

@@ -27,6 +27,7 @@ import numpy as np
 
 MAT_LXE, MAT_GXE, MAT_SOLID, MAT_C0GAS = 0, 1, 2, 3
 SURF_PTFE, SURF_CATHODE, SURF_STEEL, SURF_PERFECT = 0, 1, 2, 3
+MAT_QUARTZ, SURF_BLACK, SURF_SIPM = 4, 4, 5        # design variants (design_optics / tpc_design)
 LAMBDA_NM = 175.0
 INF = float("inf")
 
@@ -267,6 +268,99 @@ def tpc(R: float, z_liq: float, height: float, n_seg: int = 256, pmt_pitch: floa
     return mb.build(n_channels=2 * n_pmt, info=info)
 
 
+def design_optics(ptfe_reflectivity: float = 0.95, qe: float = 0.3, sipm_pde: float = 0.24, quartz_n: float = 1.6) -> Optics:
+    """default_optics plus what the design variants need: material 4 = quartz window (index 1.6, absorption
+    length 1 m, no scattering), surface 4 = black (absorbs everything), surface 5 = SiPM (detects with the photon detection
+    efficiency, absorbs the rest).  Values are stand-ins of the right size; the paper tabulates none of them."""
+    o = default_optics(ptfe_reflectivity, qe)
+    col = lambda v: np.full((1, o.n_lambda), v, np.float32)   # noqa: E731
+    cat = np.concatenate
+    return dataclasses.replace(
+        o, refr_index=cat([o.refr_index, col(quartz_n)]), abs_len=cat([o.abs_len, col(1000.0)]), scat_len=cat([o.scat_len, col(INF)]),
+        detect=cat([o.detect, col(0.0), col(sipm_pde)]), reflect_diffuse=cat([o.reflect_diffuse, col(0.0), col(0.0)]),
+        reflect_specular=cat([o.reflect_specular, col(0.0), col(0.0)]), transmit=cat([o.transmit, col(0.0), col(0.0)]))
+
+
+def _frustum(cx, cy, r0, z0, r1, z1, n: int):
+    """Open cone frustum between the circle (r0, z0) and the circle (r1, z1), 2 triangles per segment."""
+    a, b = _ring(r0, n), _ring(r1, n)
+    xyz = np.concatenate([np.column_stack([a[:, 0] + cx, a[:, 1] + cy, np.full(n, z0)]),
+                          np.column_stack([b[:, 0] + cx, b[:, 1] + cy, np.full(n, z1)])])
+    j = np.arange(n)
+    jn = (j + 1) % n
+    idx = np.concatenate([np.stack([j, jn, n + jn], axis=1), np.stack([j, n + jn, n + j], axis=1)])
+    return xyz, idx
+
+
+def tpc_design(R: float, z_liq: float, height: float, n_seg: int = 256, pmt_pitch: float = 81.0, pmt_diam: float = 76.2,
+               pmt_tris: int = 32, detailed_pmt: bool = False, side_sensors: bool = False, window: float = 5.0, cone: float = 10.0,
+               tile_fill: float = 0.9) -> Geometry:
+    """Design variants of the synthetic TPC (the paper's section 5 studies).
+    detailed_pmt: every PMT is a quartz window (a closed cylinder `window` thick: front face quartz|xenon without a surface, i.e.
+      Fresnel; back face the photocathode, quartz|solid; rim black) standing on the cap on a closed black skirt, with a conical PTFE reflector opening from the
+      window's edge towards the xenon over `cone` mm.  Needs height - z_liq > window + cone + 2.
+    side_sensors: the liquid part of the wall carries one rectangular sensor per wall segment and row (rows as high as a segment is
+      wide), `tile_fill` of the cell in each direction, floating 1 mm in front of the PTFE: n_seg x rows channels after the PMTs'.
+    Materials and surfaces of design_optics()."""
+    mb = _MeshBuilder()
+    ring = _ring(R, n_seg)
+    mb.add(*_wall_band(ring, 0.0, z_liq), MAT_LXE, MAT_SOLID, SURF_PTFE, -1)
+    mb.add(*_wall_band(ring, z_liq, height), MAT_GXE, MAT_SOLID, SURF_PTFE, -1)
+    mb.add(*_fan(0, 0, 0.0, ring, up=False), MAT_LXE, MAT_SOLID, SURF_PTFE, -1)
+    mb.add(*_fan(0, 0, height, ring, up=True), MAT_GXE, MAT_SOLID, SURF_PTFE, -1)
+    mb.add(*_fan(0, 0, z_liq, ring, up=True), MAT_LXE, MAT_GXE, -1, -1)
+    r_pmt = pmt_diam / 2
+    r_cell = pmt_pitch / 2 - 0.5
+    centres = hex_centres(pmt_pitch, R - (pmt_pitch / 2 + 1.0))
+    disk = _ring(r_pmt, pmt_tris)
+    n_pmt = centres.shape[0]
+    if detailed_pmt and height - z_liq <= window + cone + 2.0:
+        raise ValueError("tpc_design: the gas gap is too small for the top PMTs")
+    for top in (False, True):
+        med = MAT_GXE if top else MAT_LXE
+        sgn = -1.0 if top else 1.0
+        z_back = height - 1.0 if top else 1.0
+        for i, (cx, cy) in enumerate(centres):
+            ch = (n_pmt if top else 0) + i
+            if not detailed_pmt:
+                mb.add(*_fan(cx, cy, z_back, disk, up=not top), med, med, SURF_CATHODE, ch)
+                continue
+            z_front = z_back + sgn * window
+            mb.add(*_fan(cx, cy, z_front, disk, up=not top), MAT_QUARTZ, med, -1, -1)                 # window face: Fresnel
+            mb.add(*_fan(cx, cy, z_back, disk, up=top), MAT_QUARTZ, MAT_SOLID, SURF_CATHODE, ch)      # photocathode behind the window
+            xyz, idx = _wall_band(disk + [cx, cy], min(z_back, z_front), max(z_back, z_front))
+            mb.add(xyz, idx, MAT_QUARTZ, med, SURF_BLACK, -1)                                         # rim
+            # skirt from the photocathode to the cap: nothing gets under the window (the space behind it is declared solid)
+            z_cap = height if top else 0.0
+            mb.add(*_wall_band(disk + [cx, cy], min(z_back, z_cap), max(z_back, z_cap)), MAT_SOLID, med, SURF_BLACK, -1)
+            mb.add(*_frustum(cx, cy, r_pmt + 0.05, z_front, r_cell, z_front + sgn * cone, pmt_tris), med, med, SURF_PTFE, -1)
+    n_chan = 2 * n_pmt
+    info = dict(R=R, z_liq=z_liq, height=height, n_pmt_per_array=n_pmt, pmt_centres=centres, grids=[], detailed_pmt=detailed_pmt,
+                n_side=0, z_min=(1.0 + window + cone + 1.0) if detailed_pmt else 2.0, r_margin=3.0 if side_sensors else 1.0)
+    if side_sensors:
+        dphi = 2 * np.pi / n_seg
+        cell = 2 * R * np.sin(dphi / 2)                               # width of a wall segment = height of a row
+        z_lo = info["z_min"] if detailed_pmt else 2.0
+        rows = int((z_liq - 1.0 - z_lo) // cell)
+        r_plane = R * np.cos(dphi / 2) - 1.0                          # 1 mm in front of the flat wall segment
+        j = np.arange(n_seg)[None, :]
+        k = np.arange(rows)[:, None]
+        a0, a1 = (j + 0.5 - tile_fill / 2) * dphi, (j + 0.5 + tile_fill / 2) * dphi
+        rr = r_plane / np.cos(tile_fill * dphi / 2)
+        z0, z1 = z_lo + (k + 0.5 - tile_fill / 2) * cell, z_lo + (k + 0.5 + tile_fill / 2) * cell
+        full = lambda v: np.broadcast_to(v, (rows, n_seg))   # noqa: E731
+        corners = [(a0, z0), (a1, z0), (a1, z1), (a0, z1)]
+        xyz = np.stack([np.stack([full(rr * np.cos(a)), full(rr * np.sin(a)), full(z)], axis=-1) for a, z in corners], axis=2)   # [rows, n_seg, 4, 3]
+        base = 4 * np.arange(rows * n_seg)[:, None]
+        idx = np.concatenate([base + [0, 1, 2], base + [0, 2, 3]], axis=1).reshape(-1, 3)
+        chan = np.repeat(n_chan + np.arange(rows * n_seg), 2)
+        mb.add(xyz.reshape(-1, 3), idx, MAT_LXE, MAT_LXE, SURF_SIPM, chan)
+        info["n_side"] = rows * n_seg
+        info["side_rows"] = rows
+        n_chan += rows * n_seg
+    return mb.build(n_channels=n_chan, info=info)
+
+
 def sphere_detector(radius: float = 1000.0, subdiv: int = 4, material: int = MAT_C0GAS,
                     surface: int = SURF_PERFECT) -> Geometry:
     """C0: every triangle of the icosphere is its own detector channel."""
@@ -356,19 +450,20 @@ def photons_point(seed: int, n: int, origin=(0.0, 0.0, 0.0), id_base: int = 0) -
     return _finish(rng, pos, None, id_base)
 
 
-def photons_in_liquid(seed: int, n: int, R: float, z_liq: float, exclude_z=(), id_base: int = 0) -> Photons:
-    """Uniform in the liquid: r = (R-1) sqrt(u), z in [2, z_liq-1]; slabs |z-zg|<0.5 excluded (C3)."""
+def photons_in_liquid(seed: int, n: int, R: float, z_liq: float, exclude_z=(), id_base: int = 0, z_min: float = 2.0,
+                      r_margin: float = 1.0) -> Photons:
+    """Uniform in the liquid: r = (R-r_margin) sqrt(u), z in [z_min, z_liq-1]; slabs |z-zg|<0.5 excluded (C3)."""
     rng = np.random.Generator(np.random.PCG64([seed, id_base]))
-    r = (R - 1.0) * np.sqrt(rng.uniform(0, 1, n))
+    r = (R - r_margin) * np.sqrt(rng.uniform(0, 1, n))
     ph = rng.uniform(0, 2 * np.pi, n)
-    z = rng.uniform(2.0, z_liq - 1.0, n)
+    z = rng.uniform(z_min, z_liq - 1.0, n)
     for _ in range(64):
         bad = np.zeros(n, bool)
         for zg in exclude_z:
             bad |= np.abs(z - zg) < 0.5
         if not bad.any():
             break
-        z[bad] = rng.uniform(2.0, z_liq - 1.0, int(bad.sum()))
+        z[bad] = rng.uniform(z_min, z_liq - 1.0, int(bad.sum()))
     pos = np.stack([r * np.cos(ph), r * np.sin(ph), z])
     return _finish(rng, pos, None, id_base)
 
@@ -430,6 +525,25 @@ def config(i: int, ptfe_reflectivity: float = 0.95) -> Config:
                       lambda n, base=0: photons_s2_spot(5, n, (400.0, 200.0, 2600.0 + 1.25), 1.0, 27.0, base),
                       "batches of 1e7, photon_id_base = b*1e7; PTFE reflectivity in {0.90,0.95,0.99}")
     raise ValueError(f"no config {i}")
+
+
+DESIGN_VARIANTS = ("baseline", "detailed_pmt", "side_sensors", "both")
+
+
+def config_design(variant: str = "both", scale: int = 1) -> Config:
+    """Design variants at the size of C1 (scale 1: R = 250 mm) or C2 (scale 2: R = 1300 mm).  The gas gap is
+    60 mm so that the detailed top PMTs fit.  'baseline' is the same detector with plain photocathode disks and a bare wall."""
+    if variant not in DESIGN_VARIANTS:
+        raise ValueError(f"unknown design variant '{variant}'")
+    R, z_liq = (250.0, 495.0) if scale == 1 else (1300.0, 2600.0)
+    kw = dict(detailed_pmt=variant in ("detailed_pmt", "both"), side_sensors=variant in ("side_sensors", "both"))
+    key = ("design", variant, scale)
+    if key not in _GEOM_CACHE:
+        _GEOM_CACHE[key] = tpc_design(R, z_liq, z_liq + 60.0, **kw)
+    g = _GEOM_CACHE[key]
+    seed = 40 + DESIGN_VARIANTS.index(variant)
+    return Config(f"design variant '{variant}' at C{scale} size", g, design_optics(), 1_000_000 if scale == 1 else 10_000_000, seed, 2000,
+                  lambda n, base=0: photons_in_liquid(seed, n, R, z_liq, (), base, z_min=g.info["z_min"], r_margin=g.info["r_margin"]))
 
 
 # ---------------------------------------------------------------------------------------------------------------------
