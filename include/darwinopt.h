@@ -255,7 +255,9 @@ int dw_propagate(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_s
 
 /* Same computation with HOST pointers in `in`, `out` and `hist` (pinned memory recommended): the call copies
  * the batch to the device in chunks overlapped with propagation, copies the requested results back and ADDS
- * the reductions into the host arrays.  Synchronous: returns when the host buffers are complete. */
+ * the reductions into the host arrays.  Synchronous: returns when the host buffers are complete.
+ * Chunks: 1 Mi photons first, then three times larger each time up to 6 Mi (environment: DW_HOST_FIRST, DW_HOST_CHUNK, in photons;
+ * DW_HOST_SLOTS = 2..4 staging buffers); the context keeps 2 x 100 B x chunk of device staging memory (1.26 GB at the default). */
 int dw_propagate_host(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps,
                       const dw_results* out, const dw_hists* hist, const dw_propagate_params* params);
 

@@ -12,8 +12,14 @@
 
 #include "dw_internal.cuh"
 
+#ifndef DW_HOST_SLOTS_DEFAULT
+#define DW_HOST_SLOTS_DEFAULT 2
+#endif
+#ifndef DW_HOST_FIRST_DEFAULT
+#define DW_HOST_FIRST_DEFAULT (1 << 20)
+#endif
 #ifndef DW_HOST_CHUNK_DEFAULT
-#define DW_HOST_CHUNK_DEFAULT (1 << 21)
+#define DW_HOST_CHUNK_DEFAULT (6 << 20)
 #endif
 
 static std::string g_create_err;
@@ -63,7 +69,7 @@ extern "C" int dw_destroy(dw_ctx* c) {
   free_geometry(c);
   cudaFree(c->d_mat); cudaFree(c->d_surf); cudaFree(c->d_film); cudaFree(c->d_film_on);
   if (c->stage) cudaFree(c->stage);
-  for (int i = 0; i < 2; ++i) {
+  for (int i = 0; i < dw_ctx::kStageSlotsMax; ++i) {
     if (c->stage_streams[i]) cudaStreamDestroy(c->stage_streams[i]);
     if (c->stage_events[i]) cudaEventDestroy(c->stage_events[i]);
   }
@@ -412,30 +418,33 @@ extern "C" int dw_propagate_host(dw_ctx* c, const dw_photons* in, uint64_t seed,
   int64_t chunk_max = DW_HOST_CHUNK_DEFAULT;
   if (const char* ev = getenv("DW_HOST_CHUNK")) { long long v = atoll(ev); if (v >= 1024) chunk_max = v; }
   const int64_t chunk = std::min<int64_t>(n, chunk_max);
+  // staging slots (= streams = chunks in flight): DW_HOST_SLOTS in the environment, 2..4
+  int n_slots = DW_HOST_SLOTS_DEFAULT;
+  if (const char* ev = getenv("DW_HOST_SLOTS")) { int v = atoi(ev); if (v >= 2 && v <= dw_ctx::kStageSlotsMax) n_slots = v; }
   const int64_t n_chan = hist ? hist->n_chan : 0, n_bins = hist ? hist->n_bins : 0;
-  // layout: 2 slots x (11 inputs + up to 14 outputs) + histograms
+  // layout: n_slots x (11 inputs + up to 14 outputs) + histograms
   size_t per_slot = 25 * align256(sizeof(float) * chunk);
   size_t hist_bytes = align256(8 * n_chan) + align256(4 * n_bins) + align256(64) + align256(8);
-  size_t need = 2 * per_slot + hist_bytes;
+  size_t need = n_slots * per_slot + hist_bytes;
   if (c->stage_bytes < need) {
     if (c->stage) cudaFree(c->stage);
     c->stage = nullptr; c->stage_bytes = 0;
     DW_CUDA(c, cudaMalloc(&c->stage, need));
     c->stage_bytes = need;
   }
-  for (int i = 0; i < 2; ++i) {
+  for (int i = 0; i < n_slots; ++i) {
     if (!c->stage_streams[i]) DW_CUDA(c, cudaStreamCreateWithFlags(&c->stage_streams[i], cudaStreamNonBlocking));
     if (!c->stage_events[i]) DW_CUDA(c, cudaEventCreateWithFlags(&c->stage_events[i], cudaEventDisableTiming));
   }
   char* base = (char*)c->stage;
-  char* hbase = base + 2 * per_slot;
+  char* hbase = base + n_slots * per_slot;
   uint64_t* d_chan = (uint64_t*)hbase;
   uint32_t* d_time = (uint32_t*)(hbase + align256(8 * n_chan));
   uint64_t* d_fate = (uint64_t*)(hbase + align256(8 * n_chan) + align256(4 * n_bins));
   uint64_t* d_steps = (uint64_t*)(hbase + align256(8 * n_chan) + align256(4 * n_bins) + align256(64));
   DW_CUDA(c, cudaMemsetAsync(hbase, 0, hist_bytes, c->stage_streams[0]));
   DW_CUDA(c, cudaEventRecord(c->stage_events[0], c->stage_streams[0]));
-  DW_CUDA(c, cudaStreamWaitEvent(c->stage_streams[1], c->stage_events[0], 0));
+  for (int i = 1; i < n_slots; ++i) DW_CUDA(c, cudaStreamWaitEvent(c->stage_streams[i], c->stage_events[0], 0));
   const float* src[11] = {in->px, in->py, in->pz, in->kx, in->ky, in->kz, in->ex, in->ey, in->ez, in->wavelength, in->t0};
   void* dst_host[14] = {nullptr};
   if (out) {
@@ -443,9 +452,15 @@ extern "C" int dw_propagate_host(dw_ctx* c, const dw_photons* in, uint64_t seed,
                      out->kx, out->ky, out->kz, out->ex, out->ey, out->ez};
     memcpy(dst_host, tmp, sizeof tmp);
   }
+  // Chunks grow: a small first one so that the device starts after a short copy, then three times larger each time up to `chunk`
+  // (every chunk is its own launch with its own tail, so few large chunks are better once the pipeline is running).
+  int64_t first = std::min<int64_t>(chunk, DW_HOST_FIRST_DEFAULT);
+  if (const char* ev = getenv("DW_HOST_FIRST")) { long long v = atoll(ev); if (v >= 1024) first = std::min<int64_t>(chunk, v); }
   int slot = 0;
-  for (int64_t a = 0; a < n; a += chunk, slot ^= 1) {
-    const int64_t m = std::min<int64_t>(chunk, n - a);
+  int64_t m_next = first;
+  for (int64_t a = 0, m = 0; a < n; a += m, slot = (slot + 1) % n_slots) {
+    m = std::min<int64_t>(m_next, n - a);
+    m_next = std::min<int64_t>(chunk, 3 * m_next);
     cudaStream_t s = c->stage_streams[slot];
     char* sb = base + slot * per_slot;
     float* din[11];
@@ -467,8 +482,7 @@ extern "C" int dw_propagate_host(dw_ctx* c, const dw_photons* in, uint64_t seed,
     for (int k = 0; k < 14; ++k)
       if (dst_host[k]) DW_CUDA(c, cudaMemcpyAsync((char*)dst_host[k] + 4 * a, dout[k], 4 * m, cudaMemcpyDeviceToHost, s));
   }
-  DW_CUDA(c, cudaStreamSynchronize(c->stage_streams[0]));
-  DW_CUDA(c, cudaStreamSynchronize(c->stage_streams[1]));
+  for (int i = 0; i < n_slots; ++i) DW_CUDA(c, cudaStreamSynchronize(c->stage_streams[i]));
   if (hist) {
     std::vector<uint64_t> hc((size_t)n_chan), hf(8), hs(1);
     std::vector<uint32_t> ht((size_t)n_bins);

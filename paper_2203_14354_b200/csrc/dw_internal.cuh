@@ -98,8 +98,9 @@ struct dw_ctx {
   // staging for dw_propagate_host
   void* stage = nullptr;
   size_t stage_bytes = 0;
-  cudaStream_t stage_streams[2] = {nullptr, nullptr};
-  cudaEvent_t stage_events[2] = {nullptr, nullptr};
+  static constexpr int kStageSlotsMax = 4;
+  cudaStream_t stage_streams[kStageSlotsMax] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t stage_events[kStageSlotsMax] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 // error helpers --------------------------------------------------------------------------------------------
