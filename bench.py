@@ -208,6 +208,9 @@ def main():
                     "instead of building on the moved one (diagnostic: cost and quality of a refit)")
     ap.add_argument("--render", type=int, default=0, help="also time dw_render on an N x N image of the detector seen from outside and from "
                     "inside (diagnostic: the first-hit query on coherent rays; reported in config.render)")
+    ap.add_argument("--pipeline", action="store_true", help="also time the same K steps issued alternately on two streams, so that the drain "
+                    "of one batch (its longest-lived photons) overlaps the start of the next (diagnostic, reported in config.pipelined; "
+                    "the headline value stays the serial one)")
     ap.add_argument("--no-skip", action="store_true", help="DW_PROP_NO_EMPTY_SKIP (traverse every query, diagnostic)")
     ap.add_argument("--emit", action="store_true", help="generate each step's photons on the device with dw_emit inside the timed step "
                     "(SURVEY 8(f) f1; C1-C4 only) instead of propagating a resident batch")
@@ -305,6 +308,28 @@ def main():
     n_all = n * world
     value = n_all * args.steps / (total_ms * 1e-3)
 
+    pipelined = None
+    if args.pipeline and not args.emit and world == 1:
+        out2 = dw.DeviceResults(n, ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), dev)
+        lanes = [(torch.cuda.Stream(device=dev), out), (torch.cuda.Stream(device=dev), out2)]
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for rep in range(2):                                   # first pass warms the second stream up
+            e0.record(lanes[0][0])
+            lanes[1][0].wait_event(e0)
+            for i in range(args.steps):
+                st_i, out_i = lanes[i % 2]
+                ctx.propagate(d_ph, c.seed, c.max_steps, out_i, hist, flags=flags, stream=st_i, th_phys=args.th_phys, th_leaf=args.th_leaf,
+                              block_threads=args.block, blocks_per_sm=args.blocks_per_sm)
+            done = torch.cuda.Event()
+            done.record(lanes[1][0])
+            lanes[0][0].wait_event(done)
+            e1.record(lanes[0][0])
+            torch.cuda.synchronize()
+        pms = e0.elapsed_time(e1)
+        pipelined = dict(value=n * args.steps / (pms * 1e-3), ms_per_step=pms / args.steps, streams=2,
+                         note="same K steps, alternating streams; results of the two lanes go to separate buffers")
+
     emit_info = None
     if args.emit:
         evs = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
@@ -391,7 +416,8 @@ def main():
                             bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch(),
                             **({"moved": args.move, "refit": refit_info} if args.move else {}),
-                            **({"render": render_info} if render_info else {})),
+                            **({"render": render_info} if render_info else {}),
+                            **({"pipelined": pipelined} if pipelined else {})),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
