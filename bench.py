@@ -280,6 +280,7 @@ def main():
         if world > 1:
             dwdist.merge_hists(hist)        # the only exchange: tens of kB of integer histograms
 
+    sampler = ClockSampler(local).start()            # NVML is initialised here, before the warm-up: its first calls take driver locks
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
@@ -287,7 +288,8 @@ def main():
     dwdist.barrier()
     torch.cuda.synchronize()
     launches0 = ctx.last_launch()["n_launches"]
-    sampler = ClockSampler(local).start()
+    sampler.samples.clear()                          # only the samples of the timed region count
+    sampler.reasons.clear()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     ev[0].record(stream)
     for i in range(args.steps):
@@ -356,12 +358,15 @@ def main():
         dwdist.barrier()
         t0 = time.perf_counter()
         reps = max(1, min(args.steps, 3))
+        each = []
         for _ in range(reps):
-            ctx.propagate_host(hp, c.seed, c.max_steps, hout, hh, flags=flags)
+            t1 = time.perf_counter()
+            ctx.propagate_host(hp, c.seed, c.max_steps, hout, hh, flags=flags)      # synchronous: returns when the host buffers are complete
+            each.append(1e3 * (time.perf_counter() - t1))
         torch.cuda.synchronize()
         dt = dwdist.max_over_ranks(time.perf_counter() - t0)
         e2e = dict(value=n_all * reps / dt, unit=UNIT, h2d_bytes_per_step=int(hp.nbytes), d2h_bytes_per_step=int(hout.nbytes + hh.nbytes),
-                   ms_per_step=1e3 * dt / reps, api="dw_propagate_host (pinned host buffers, chunked copies overlapped with propagation)")
+                   ms_per_step=1e3 * dt / reps, ms_each=each, api="dw_propagate_host (pinned host buffers, chunked copies overlapped with propagation)")
 
     if rank != 0:
         dwdist.finalize()
@@ -421,7 +426,7 @@ def main():
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
-                clocks=clocks, e2e=e2e, emission=emit_info, gpu_launches=int(launches) * (2 if args.emit else 1), roofline=roofline, cpu_baseline=cpu)
+                clocks=clocks, ms_each=[round(v, 3) for v in per_step_ms], e2e=e2e, emission=emit_info, gpu_launches=int(launches) * (2 if args.emit else 1), roofline=roofline, cpu_baseline=cpu)
     print(json.dumps(line))
     dwdist.finalize()
     return 0

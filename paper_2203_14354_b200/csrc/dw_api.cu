@@ -52,6 +52,22 @@ extern "C" int dw_create(int cuda_device, dw_ctx** out) {
   dw_ctx* c = new dw_ctx();
   c->device = cuda_device;
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, cuda_device);
+  // A pool of its own for the 8-byte queue heads of the launches, which keeps its memory: the default pool gives freed memory
+  // back to the system at every synchronisation (release threshold 0) and maps it again for the next launch.
+  {
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = cuda_device;
+    if (cudaMemPoolCreate(&c->pool, &props) == cudaSuccess) {
+      unsigned long long keep = ~0ull;
+      cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    } else {
+      c->pool = nullptr;
+      cudaGetLastError();
+    }
+  }
   *out = c;
   return DW_OK;
 }
@@ -69,6 +85,7 @@ extern "C" int dw_destroy(dw_ctx* c) {
   free_geometry(c);
   cudaFree(c->d_mat); cudaFree(c->d_surf); cudaFree(c->d_film); cudaFree(c->d_film_on);
   if (c->stage) cudaFree(c->stage);
+  if (c->pool) { cudaDeviceSynchronize(); cudaMemPoolDestroy(c->pool); }
   for (int i = 0; i < dw_ctx::kStageSlotsMax; ++i) {
     if (c->stage_streams[i]) cudaStreamDestroy(c->stage_streams[i]);
     if (c->stage_events[i]) cudaEventDestroy(c->stage_events[i]);

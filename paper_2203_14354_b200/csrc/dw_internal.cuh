@@ -92,6 +92,7 @@ struct dw_ctx {
     unsigned* scene = nullptr;    // [6] scene bounds, order-preserving uint encoding
     std::vector<int> level_start; // wide-tree level k = nodes [level_start[k], level_start[k+1])
   } rf;
+  cudaMemPool_t pool = nullptr;   // queue heads of the launches (stream-ordered, memory kept between launches)
   // launch record
   int last_grid = 0, last_block = 0, last_smem = 0;
   int64_t n_launches = 0;

@@ -1193,7 +1193,8 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   int grid = (int)std::min<int64_t>((int64_t)c->sm_count * per_sm, std::max<int64_t>(blocks_needed, 1));
   // queue head: a stream-ordered 8-byte allocation, so that launches on different streams never share one
   unsigned long long* head = nullptr;
-  DW_CUDA(c, cudaMallocAsync((void**)&head, sizeof(unsigned long long), stream));
+  if (c->pool) DW_CUDA(c, cudaMallocFromPoolAsync((void**)&head, sizeof(unsigned long long), c->pool, stream));
+  else DW_CUDA(c, cudaMallocAsync((void**)&head, sizeof(unsigned long long), stream));
   DW_CUDA(c, cudaMemsetAsync(head, 0, sizeof(unsigned long long), stream));
   A.queue_head = head;
   kern<<<grid, B, smem, stream>>>(A);
