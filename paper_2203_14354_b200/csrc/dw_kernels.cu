@@ -16,6 +16,9 @@ namespace {
 #ifndef DW_NODE_LDG256
 #define DW_NODE_LDG256 0
 #endif
+#ifndef DW_FLAT_TABLES
+#define DW_FLAT_TABLES 1
+#endif
 #ifndef DW_OUTLINE
 #define DW_OUTLINE 2
 #endif
@@ -685,9 +688,14 @@ constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 #define DW_POOL_MIN_BLOCKS 6
 #endif
 // The film-enabled instantiation gets one block fewer per SM: at 80 registers it spills 106 bytes around the film call.
-template <bool kFilm>
+// kFlat: all tables have one wavelength node (the BASELINE.json configs): a look-up is one load, no call.
+template <bool kFilm, bool kFlat>
 __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
+  auto TAB = [](const float* __restrict__ tab, int row, int nl, float l0, float inv_dl, float lam) -> float {
+    if constexpr (kFlat) return __ldg(tab + row);
+    else return table_at(tab, row, nl, l0, inv_dl, lam);
+  };
   __shared__ unsigned int s_fate[8];
   __shared__ unsigned long long s_steps;
   if (threadIdx.x < 8) s_fate[threadIdx.x] = 0;
@@ -823,9 +831,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
             us = r0.z; uf = r0.w;
             if (medium >= 0 && medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
             medium = m1;
-            n1 = table_at(A.tab.mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-            float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-            float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            n1 = TAB(A.tab.mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float La = TAB(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float Ls = TAB(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, m1, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
             float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
             absorb_first = da < ds;
             dbulk = fminf(da, ds);
@@ -859,23 +867,23 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
             if constexpr (kFilm) is_film = sf != 0xFF && __ldg(&A.tab.film_on[sf]) != 0;
             if (is_film) {                                            // thin-film surface (second mode)
               const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
-              const float n3 = table_at(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-              const float fnf = table_at(A.tab.film, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
-              const float fkf = table_at(A.tab.film + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
-              const float fd = table_at(A.tab.film + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float n3 = TAB(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+              const float fnf = TAB(A.tab.film, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fkf = TAB(A.tab.film + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              const float fd = TAB(A.tab.film + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               int oc = 2;
               if constexpr (kFilm) oc = film_event(n1, fnf, fkf, fd, n3, lambda, nh, k, e, uf);
               hist |= DW_H_FILM;
               if (oc == 0) hist |= DW_H_REFLECT_SPECULAR;
               else if (oc == 1) { hist |= DW_H_SURFACE_TRANSMIT; medium = m2; }
-              else if (us < table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda)) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
+              else if (us < TAB(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda)) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
               else fate = DW_FATE_SURFACE_ABSORBED;
             } else if (sf != 0xFF) {                                  // S7 explicit surface
               const size_t ss = (size_t)A.tab.n_surf * A.tab.nl_surf;
-              float c0 = table_at(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
-              float c1 = table_at(A.tab.surf + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
-              float c2 = table_at(A.tab.surf + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
-              float c3 = table_at(A.tab.surf + 3 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c0 = TAB(A.tab.surf, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c1 = TAB(A.tab.surf + ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c2 = TAB(A.tab.surf + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
+              float c3 = TAB(A.tab.surf + 3 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               if (us < c0) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
               else if (us < c1) { lambert(nh, k, e, draw4(A.seed, pid, step, 1u)); hist |= DW_H_REFLECT_DIFFUSE; }
               else if (us < c2) {                                     // specular: no plane of incidence needed
@@ -886,7 +894,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
               else if (us < c3) { hist |= DW_H_SURFACE_TRANSMIT; medium = m2; }
               else fate = DW_FATE_SURFACE_ABSORBED;
             } else {                                                  // S8 Fresnel
-              float n2 = table_at(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+              float n2 = TAB(A.tab.mat, m2, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
               bool crossed;
               hist |= fresnel(n1, n2, nh, k, e, uf, crossed);
               if (crossed) medium = m2;
@@ -907,9 +915,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           if ((!literal) && medium >= 0) {                            // medium known: S3/S4 draws before the query
             float4 r0 = draw4(A.seed, pid, step, 0u);
             us = r0.z; uf = r0.w;
-            n1 = table_at(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-            float La = table_at(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
-            float Ls = table_at(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            n1 = TAB(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float La = TAB(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
+            float Ls = TAB(A.tab.mat + 2 * (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
             float da = -La * logf(r0.x), ds = -Ls * logf(r0.y);
             absorb_first = da < ds;
             dbulk = fminf(da, ds);
@@ -1182,8 +1190,10 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)kWarpInts * (B / 32);
   int per_sm = 0;
   const bool films = c->tables.film != nullptr && c->tables.film_on != nullptr;
+  const bool flat = DW_FLAT_TABLES && c->tables.nl_mat == 1 && c->tables.nl_surf == 1;
   void (*kern)(PropArgs) = legacy ? (films ? propagate_kernel<true> : propagate_kernel<false>)
-                                  : (films ? propagate_pool_kernel<true> : propagate_pool_kernel<false>);
+                                  : (films ? (flat ? propagate_pool_kernel<true, true> : propagate_pool_kernel<true, false>)
+                                           : (flat ? propagate_pool_kernel<false, true> : propagate_pool_kernel<false, false>));
   DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, B, smem));
   if (params && params->blocks_per_sm > 0) per_sm = std::min(per_sm, params->blocks_per_sm);
   if (per_sm < 1) return dw_fail(c, DW_E_CUDA, "dw_propagate: kernel does not fit on an SM");
