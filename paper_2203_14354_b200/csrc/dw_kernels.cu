@@ -58,7 +58,14 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint32_t k0, uint32_t k1
   return c;
 }
 // ((x >> 9) + 0.5) * 2^-23: 24 significant bits, exact in fp32, strictly inside (0,1)
+#ifndef DW_U01_FMA
+#define DW_U01_FMA 1
+#endif
+#if DW_U01_FMA   // one FMA: (x >> 9) < 2^23, so f * 2^-23 + 2^-24 is exact and equals the expression above bit for bit
+__device__ __forceinline__ float u01(uint32_t x) { return fmaf((float)(x >> 9), 1.1920928955078125e-7f, 5.9604644775390625e-8f); }
+#else
 __device__ __forceinline__ float u01(uint32_t x) { return ((float)(x >> 9) + 0.5f) * 1.1920928955078125e-7f; }
+#endif
 __device__ DW_INL_PHILOX float4 draw4(uint64_t seed, uint64_t pid, uint32_t step, uint32_t block) {
   uint4 r = philox4x32_10(make_uint4((uint32_t)pid, (uint32_t)(pid >> 32), step, block), (uint32_t)seed, (uint32_t)(seed >> 32));
   return make_float4(u01(r.x), u01(r.y), u01(r.z), u01(r.w));
@@ -248,9 +255,10 @@ __device__ __forceinline__ void frame(V3 w, V3& a, V3& b) {
 
 // S6 Rayleigh scattering: the algorithm that reproduces the theoretical distribution:
 // isotropic k', accept with probability |e - (e.k')k'|^2; iteration j uses Philox block 1 + j.
-__device__ DW_INL_PHYS bool rayleigh(V3& k, V3& e, uint64_t seed, uint64_t pid, uint32_t step) {
+template <class Draw>   // draw(block) -> the four uniforms of Philox block `block` of this photon and step
+__device__ DW_INL_PHYS bool rayleigh(V3& k, V3& e, Draw draw) {
   for (uint32_t j = 0; j < 4096u; ++j) {
-    float4 r = draw4(seed, pid, step, 1u + j);
+    float4 r = draw(1u + j);
     float ct = 1.0f - 2.0f * r.x;
     float st = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
     float sp, cp;
@@ -384,6 +392,7 @@ __device__ __noinline__ int film_event(float n1, float nf, float kf, float d_nm,
 
 // ------------------------------------------------------------------------------------------------ propagation
 struct PropArgs {
+  uint32_t keys[20];                // Philox round keys of `seed` (k0 + r W0, k1 + r W1), filled by the host: constant-bank operands
   DwBvh bvh;
   DwTables tab;
   dw_photons in;
@@ -395,6 +404,21 @@ struct PropArgs {
   int32_t th_phys, th_leaf;         // phase-scheduling thresholds (lanes)
   unsigned long long* queue_head;   // device counter, zeroed before launch
 };
+
+// Philox4x32-10 with the round keys read from the kernel parameters (A.keys): same values as draw4(A.seed, ...).
+#ifndef DW_PHILOX_KEYS
+#define DW_PHILOX_KEYS 2
+#endif
+__device__ __forceinline__ float4 draw4_keys(const PropArgs& A, uint64_t pid, uint32_t step, uint32_t block) {
+  uint4 c = make_uint4((uint32_t)pid, (uint32_t)(pid >> 32), step, block);
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ A.keys[2 * r], lo1, hi0 ^ c.w ^ A.keys[2 * r + 1], lo0);
+  }
+  return make_float4(u01(c.x), u01(c.y), u01(c.z), u01(c.w));
+}
 
 constexpr int kChunk = 8;   // photons claimed per lane per queue transaction (x32 per warp)
 
@@ -542,7 +566,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
               if (absorb_first) {
                 fate = DW_FATE_BULK_ABSORBED;                         // S4 first branch
               } else {                                                // S4 second branch + S6
-                if (!rayleigh(k, e, A.seed, pid, step)) fate = DW_FATE_NAN_ABORT;
+                if (!rayleigh(k, e, [&](uint32_t b) { return draw4(A.seed, pid, step, b); })) fate = DW_FATE_NAN_ABORT;
                 hist |= DW_H_RAYLEIGH;
                 last_tri = -1;
               }
@@ -687,6 +711,15 @@ constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 #ifndef DW_POOL_MIN_BLOCKS
 #define DW_POOL_MIN_BLOCKS 6
 #endif
+#ifndef DW_NODE_REPS
+#define DW_NODE_REPS 2
+#endif
+#ifndef DW_TRI_REPS
+#define DW_TRI_REPS 1
+#endif
+#ifndef DW_NODE_REPS_MIN
+#define DW_NODE_REPS_MIN 16
+#endif
 // The film-enabled instantiation gets one block fewer per SM: at 80 registers it spills 106 bytes around the film call.
 // kFlat: all tables have one wavelength node (the BASELINE.json configs): a look-up is one load, no call.
 template <bool kFilm, bool kFlat>
@@ -695,6 +728,15 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   auto TAB = [](const float* __restrict__ tab, int row, int nl, float l0, float inv_dl, float lam) -> float {
     if constexpr (kFlat) return __ldg(tab + row);
     else return table_at(tab, row, nl, l0, inv_dl, lam);
+  };
+  // Philox at the two hot sites (block 0 of the next query, the Rayleigh loop) and at the cold ones (first step, Lambert)
+  auto DRAW_HOT = [&](uint64_t pid_, uint32_t step_, uint32_t block_) -> float4 {
+    if constexpr (DW_PHILOX_KEYS >= 1) return draw4_keys(A, pid_, step_, block_);
+    else return draw4(A.seed, pid_, step_, block_);
+  };
+  auto DRAW_COLD = [&](uint64_t pid_, uint32_t step_, uint32_t block_) -> float4 {
+    if constexpr (DW_PHILOX_KEYS >= 2) return draw4_keys(A, pid_, step_, block_);
+    else return draw4(A.seed, pid_, step_, block_);
   };
   __shared__ unsigned int s_fate[8];
   __shared__ unsigned long long s_steps;
@@ -827,7 +869,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           if (!have_hit) {
             fate = DW_FATE_ESCAPED;                                   // G3: ray leaves the world
           } else {
-            float4 r0 = draw4(A.seed, pid, step, 0u);                 // (u_a, u_s, u_surface, u_fresnel)
+            float4 r0 = DRAW_COLD(pid, step, 0u);                 // (u_a, u_s, u_surface, u_fresnel)
             us = r0.z; uf = r0.w;
             if (medium >= 0 && medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
             medium = m1;
@@ -850,7 +892,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
               if (absorb_first) {
                 fate = DW_FATE_BULK_ABSORBED;                         // S4 first branch
               } else {                                                // S4 second branch + S6
-                if (!rayleigh(k, e, A.seed, pid, step)) fate = DW_FATE_NAN_ABORT;
+                if (!rayleigh(k, e, [&](uint32_t b) { return DRAW_HOT(pid, step, b); })) fate = DW_FATE_NAN_ABORT;
                 hist |= DW_H_RAYLEIGH;
                 last_tri = -1;
               }
@@ -885,7 +927,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
               float c2 = TAB(A.tab.surf + 2 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               float c3 = TAB(A.tab.surf + 3 * ss, sf, A.tab.nl_surf, A.tab.surf_l0, A.tab.surf_inv_dl, lambda);
               if (us < c0) { fate = DW_FATE_DETECTED; channel = __float_as_int(tc.w); }
-              else if (us < c1) { lambert(nh, k, e, draw4(A.seed, pid, step, 1u)); hist |= DW_H_REFLECT_DIFFUSE; }
+              else if (us < c1) { lambert(nh, k, e, DRAW_COLD(pid, step, 1u)); hist |= DW_H_REFLECT_DIFFUSE; }
               else if (us < c2) {                                     // specular: no plane of incidence needed
                 k = unit(fma3(-2.0f * dot(k, nh), nh, k));
                 e = unit(fma3(-2.0f * dot(e, nh), nh, e));
@@ -913,7 +955,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           float tmax = INFINITY;
           bool skip = false;
           if ((!literal) && medium >= 0) {                            // medium known: S3/S4 draws before the query
-            float4 r0 = draw4(A.seed, pid, step, 0u);
+            float4 r0 = DRAW_HOT(pid, step, 0u);
             us = r0.z; uf = r0.w;
             n1 = TAB(A.tab.mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
             float La = TAB(A.tab.mat + (size_t)A.tab.n_mat * A.tab.nl_mat, medium, A.tab.nl_mat, A.tab.mat_l0, A.tab.mat_inv_dl, lambda);
@@ -1031,8 +1073,18 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       if (nAct == 0) break;
       if (32 - nAct >= th_fetch && (nQ_rem > 0 || nReady >= 32)) break;
       if (nI > 0 && nL < th_leaf) {
+#if DW_NODE_REPS > 1
+        // several node visits per vote while most lanes are in internal nodes: the votes are a quarter of the traversal's instructions
+        const int reps = nI >= DW_NODE_REPS_MIN ? DW_NODE_REPS : 1;
+#pragma unroll 1
+        for (int rep = 0; rep < reps; ++rep)
+#endif
         if (act && ts.node >= 0) step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
       } else {
+#if DW_TRI_REPS > 1
+#pragma unroll 1
+        for (int rep = 0; rep < DW_TRI_REPS; ++rep)
+#endif
         if (act && ts.node == kInLeaf) step_triangle(A.bvh, ray, ts, q_exclude, q_medium, my_stack, sstride, lstack);
       }
       if (act && ts.node == kDone) {                        // query finished: hand the slot to the physics phase
@@ -1181,6 +1233,10 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   A.bvh = c->bvh; A.tab = c->tables; A.in = *in;
   if (out) A.out = *out;
   if (hist) A.hist = *hist;
+  for (int r = 0; r < 10; ++r) {
+    A.keys[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+    A.keys[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
   A.seed = seed; A.max_steps = max_steps; A.flags = params ? params->flags : 0u;
   const bool legacy = (A.flags & DW_PROP_LEGACY_SCHEDULER) != 0;
   A.th_phys = (params && params->th_phys > 0) ? params->th_phys : (legacy ? 12 : 8);
