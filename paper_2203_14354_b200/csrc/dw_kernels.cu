@@ -715,7 +715,7 @@ constexpr int kWarpInts = kWarpStack + kStackShared * 32;
 #define DW_NODE_REPS 2
 #endif
 #ifndef DW_TRI_REPS
-#define DW_TRI_REPS 1
+#define DW_TRI_REPS 2
 #endif
 #ifndef DW_NODE_REPS_MIN
 #define DW_NODE_REPS_MIN 16
