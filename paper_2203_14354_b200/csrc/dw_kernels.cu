@@ -9,19 +9,21 @@
 
 namespace {
 
-// Inlining of helpers that are called from many places (profiles/r01_propagate_bvh4_c2.md, capture 6: instruction fetch
-// became the largest stall once the kernel grew to ~2900 instructions).  Level 0: everything inline; 1: Philox out of line;
-// 2: + table look-up; 3: + Rayleigh / Lambert / Fresnel.
-// Measured on C2 (alternating A/B, two rounds): level 0 173.8, 1 175.2, 2 188.6, 3 151.0 M photons/s.
 // Node planes read as four 256-bit loads instead of seven 128-bit ones.  Neutral while the kernel was bound by instruction issue (199.1 vs
 // 199.0); once Philox and the votes were cheaper the L1 data pipe (82 % busy, 97 % of its global wavefronts = lanes x node loads) was
-// the limit: C2 227.2 -> 232.8, C3 211.4 -> 220.7 M photons/s (profiles/r01_reps_c2.md).
+// the limit: C2 227.2 -> 232.8, C3 211.4 -> 220.7 M photons/s (profiles/r01_ldg256_c2.md).
 #ifndef DW_NODE_LDG256
 #define DW_NODE_LDG256 1
 #endif
 #ifndef DW_FLAT_TABLES
 #define DW_FLAT_TABLES 1
 #endif
+// Inlining of helpers that are called from many places (profiles/r01_propagate_bvh4_c2.md, capture 6: instruction fetch
+// became the largest stall once the kernel grew to ~2900 instructions).  Level 0: everything inline; 1: Philox out of line;
+// 2: + table look-up; 3: + Rayleigh / Lambert / Fresnel.
+// Measured on C2 (alternating A/B, two rounds): level 0 173.8, 1 175.2, 2 188.6, 3 151.0 M photons/s.
+// The pool kernel has since stopped calling either helper (flat tables, draw4_keys inlined: profiles/r01_ldg256_c2.md); the legacy
+// kernel and dw_emit still do.
 #ifndef DW_OUTLINE
 #define DW_OUTLINE 2
 #endif
