@@ -702,15 +702,18 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
 #endif
 constexpr int kSlots = DW_POOL_SLOTS;      // 33..64: lane l looks after slots l and l + 32 (the latter if it exists)
 static_assert(kSlots > 32 && kSlots <= 64, "pool size");
-enum : int { W_X = 0, W_Y, W_Z, W_KX, W_KY, W_KZ, W_EX, W_EY, W_EZ, W_LAMBDA, W_T, W_MEDIUM, W_LAST, W_STEP, W_HIST, W_PI,
-             W_DBULK, W_N1, W_US, W_UF, W_BEST_T, W_BEST_SLOT, kWords };
+// The last two words exist only in the full layout: with flat tables and no films the wavelength is never read again and n1 is one
+// table load from the medium, so the lean layout (20 words) leaves them out.  With 8 shared stack entries a lean block takes 26 kB, six of
+// them fit the 164 kB shared-memory configuration instead of 196 kB, and L1 grows from ~60 to ~92 kB (profiles/r01_ldg256_c2.md).
+enum : int { W_X = 0, W_Y, W_Z, W_KX, W_KY, W_KZ, W_EX, W_EY, W_EZ, W_T, W_MEDIUM, W_LAST, W_STEP, W_HIST, W_PI,
+             W_DBULK, W_US, W_UF, W_BEST_T, W_BEST_SLOT, kWordsLean, W_LAMBDA = kWordsLean, W_N1, kWordsFull };
 enum : int { S_EMPTY = 0, S_PHYS = 1, S_TRACE = 2, S_BUSY = 3 };
 constexpr uint32_t kAbsorbFirstBit = 0x80000000u;                 // kept in the W_HIST word
-constexpr int kWarpPool = kWords * kSlots;                        // ints
-constexpr int kWarpSt = kWarpPool;                                // status[kSlots]
-constexpr int kWarpQ = kWarpSt + kSlots;                          // queue[kSlots] (rank -> slot scratch)
-constexpr int kWarpStack = kWarpQ + kSlots;                       // stack[kStackShared][32]
-constexpr int kWarpInts = kWarpStack + kStackShared * 32;
+// per-warp layout in ints: pool[words][kSlots], status[kSlots], queue[kSlots] (rank -> slot scratch), stack[kStackShared][32]
+constexpr int warp_st(bool lean) { return (lean ? kWordsLean : kWordsFull) * kSlots; }
+constexpr int warp_q(bool lean) { return warp_st(lean) + kSlots; }
+constexpr int warp_stack(bool lean) { return warp_q(lean) + kSlots; }
+constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32; }
 
 // 6 resident blocks (24 warps) per SM: 80 registers, no spills; measured on C2 against 4 blocks (118 registers): 134 vs 117 M photons/s.
 #ifndef DW_POOL_MIN_BLOCKS
@@ -748,12 +751,13 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   if (threadIdx.x < 8) s_fate[threadIdx.x] = 0;
   if (threadIdx.x == 0) s_steps = 0ull;
   const int lane = threadIdx.x & 31;
-  int* const wbase = s_dyn + (threadIdx.x >> 5) * kWarpInts;
+  constexpr bool kLean = kFlat && !kFilm;
+  int* const wbase = s_dyn + (threadIdx.x >> 5) * warp_ints(kLean);
   int* const pool = wbase;
   float* const poolf = reinterpret_cast<float*>(wbase);
-  int* const st = wbase + kWarpSt;
-  int* const q = wbase + kWarpQ;
-  int* const my_stack = wbase + kWarpStack + lane;
+  int* const st = wbase + warp_st(kLean);
+  int* const q = wbase + warp_q(kLean);
+  int* const my_stack = wbase + warp_stack(kLean) + lane;
   constexpr int sstride = 32;
   const bool has2 = lane + 32 < kSlots;            // this lane also looks after slot lane + 32
   st[lane] = S_EMPTY;
@@ -833,7 +837,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         x = mk(poolf[W_X * kSlots + slot], poolf[W_Y * kSlots + slot], poolf[W_Z * kSlots + slot]);
         k = mk(poolf[W_KX * kSlots + slot], poolf[W_KY * kSlots + slot], poolf[W_KZ * kSlots + slot]);
         e = mk(poolf[W_EX * kSlots + slot], poolf[W_EY * kSlots + slot], poolf[W_EZ * kSlots + slot]);
-        lambda = poolf[W_LAMBDA * kSlots + slot];
+        if constexpr (!kLean) lambda = poolf[W_LAMBDA * kSlots + slot];
         t = poolf[W_T * kSlots + slot];
         medium = pool[W_MEDIUM * kSlots + slot];
         last_tri = pool[W_LAST * kSlots + slot];
@@ -843,11 +847,12 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         hist &= ~kAbsorbFirstBit;
         pi = (int64_t)(uint32_t)pool[W_PI * kSlots + slot];
         dbulk = poolf[W_DBULK * kSlots + slot];
-        n1 = poolf[W_N1 * kSlots + slot];
+        if constexpr (!kLean) n1 = poolf[W_N1 * kSlots + slot];
         us = poolf[W_US * kSlots + slot];
         uf = poolf[W_UF * kSlots + slot];
         best_t = poolf[W_BEST_T * kSlots + slot];
         best_slot = pool[W_BEST_SLOT * kSlots + slot];
+        if constexpr (kLean) { if (medium >= 0) n1 = __ldg(A.tab.mat + medium); }   // the value the query set-up computed
       }
       uint32_t fate = 0xFFu;           // 0xFF = still running
       int channel = -1;
@@ -994,7 +999,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
           poolf[W_KX * kSlots + slot] = k.x; poolf[W_KY * kSlots + slot] = k.y; poolf[W_KZ * kSlots + slot] = k.z;
           poolf[W_EX * kSlots + slot] = e.x; poolf[W_EY * kSlots + slot] = e.y; poolf[W_EZ * kSlots + slot] = e.z;
-          poolf[W_LAMBDA * kSlots + slot] = lambda;
+          if constexpr (!kLean) poolf[W_LAMBDA * kSlots + slot] = lambda;
           poolf[W_T * kSlots + slot] = t;
           pool[W_MEDIUM * kSlots + slot] = medium;
           pool[W_LAST * kSlots + slot] = last_tri;
@@ -1002,7 +1007,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           pool[W_HIST * kSlots + slot] = (int)(hist | (absorb_first ? kAbsorbFirstBit : 0u));
           pool[W_PI * kSlots + slot] = (int)(uint32_t)pi;
           poolf[W_DBULK * kSlots + slot] = dbulk;
-          poolf[W_N1 * kSlots + slot] = n1;
+          if constexpr (!kLean) poolf[W_N1 * kSlots + slot] = n1;
           poolf[W_US * kSlots + slot] = us;
           poolf[W_UF * kSlots + slot] = uf;
           poolf[W_BEST_T * kSlots + slot] = tmax;                     // the query starts from t_max
@@ -1248,10 +1253,10 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   A.th_leaf = (params && params->th_leaf > 0) ? params->th_leaf : 12;
   int B = (params && params->block_threads) ? params->block_threads : 128;
   if (B < 32 || B > 128 || (B & 31)) return dw_fail(c, DW_E_ARG, "dw_propagate: block_threads must be 32, 64, 96 or 128");
-  size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)kWarpInts * (B / 32);
   int per_sm = 0;
   const bool films = c->tables.film != nullptr && c->tables.film_on != nullptr;
   const bool flat = DW_FLAT_TABLES && c->tables.nl_mat == 1 && c->tables.nl_surf == 1;
+  size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)warp_ints(flat && !films) * (B / 32);
   void (*kern)(PropArgs) = legacy ? (films ? propagate_kernel<true> : propagate_kernel<false>)
                                   : (films ? (flat ? propagate_pool_kernel<true, true> : propagate_pool_kernel<true, false>)
                                            : (flat ? propagate_pool_kernel<false, true> : propagate_pool_kernel<false, false>));
