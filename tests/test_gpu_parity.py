@@ -548,6 +548,26 @@ def test_pool_scheduler_bit_identical_to_legacy(cfg, n, mode):
     assert int(a["fate_count"].sum()) == n
 
 
+@pytest.mark.parametrize("seed", [0xDEADBEEF12345678, 0xFFFFFFFFFFFFFFFF, 1 << 32])
+def test_round_keys_from_both_halves_of_a_64_bit_seed(seed):
+    """The pool kernel takes the Philox round keys of the seed from the kernel parameters (filled by the host, both 32-bit halves of
+    the key with their own Weyl constants); the legacy kernel computes them in draw4. A seed with a non-zero high word must give
+    the same photons in both, and other photons than its low word alone."""
+    c, ctx = ctx_for(1)
+    ph = c.make_photons(50_000 - 5)
+    a = gpu_run(ctx, ph, seed, c.max_steps, n_bins=200, dt=2.0)
+    b = gpu_run(ctx, ph, seed, c.max_steps, n_bins=200, dt=2.0, flags=dw.PROP_LEGACY_SCHEDULER)
+    for key in FULL + ("chan_count", "time_hist", "fate_count", "total_steps"):
+        assert np.array_equal(a[key], b[key]), f"seed {seed:#x}: '{key}' differs between schedulers"
+    low = gpu_run(ctx, ph, seed & 0xFFFFFFFF, c.max_steps, n_bins=200, dt=2.0)
+    assert not np.array_equal(a["steps"], low["steps"]), "the high word of the seed is ignored"
+    # and the oracle, which keys its own Philox with the same 64-bit seed, follows the same photons for the first steps
+    ref = oracle_for(1).propagate(ph, seed, 3)
+    r = gpu_run(ctx, ph, seed, 3)
+    same = (r["flags"] == ref["flags"]) & (r["steps"] == ref["steps"]) & (r["channel"] == ref["channel"]) & (r["last_tri"] == ref["last_tri"])
+    assert same.mean() >= 0.999, f"seed {seed:#x}: identical to the oracle on {same.mean():.5f}"
+
+
 @pytest.mark.parametrize("cfg,n", [(1, 400_000), (2, 400_000), (3, 400_000), (4, 200_000)])
 def test_empty_space_skip_is_invisible(cfg, n):
     """a bounded query whose segment lies in the triangle-free box of its origin cell is answered
