@@ -20,7 +20,8 @@
  *   dw_propagate                      the Monte Carlo loop S1..S13 for a photon batch, device buffers
  *   dw_propagate_host                 same, host buffers (copies inside), for end-to-end timing
  *   dw_emit                           scintillation photons generated on the device          (Table 2)
- *   dw_tally                          LCE per source and array, arrival-time histograms, loss table (Table 6)
+ *   dw_tally / dw_tally_finish        counts per source and array, arrival-time histograms, loss table; LCE and t90 (Table 6)
+ *   dw_emit_sources / dw_design_study many sources per launch; the whole emit -> propagate -> tally loop as one call
  *
  * Conventions
  *   - Units mm, ns, nm.  c = 299.792458 mm/ns.  All floating point is IEEE fp32.
@@ -312,6 +313,41 @@ typedef struct dw_tally_tables {
 } dw_tally_tables;
 int dw_tally(dw_ctx* ctx, const dw_results* results, int64_t n, int64_t photons_per_source, const dw_tally_tables* tables,
              void* cuda_stream);
+
+/* The two products the paper derives from those tables, computed on the device ("on-device LCE(Z,R^2) and t90
+ * maps").  PAPER.md line 189: "LCE is defined here as the number of photons hitting the photosensitive area divided by the total
+ * number of generated photons"; line 211: t90 is "the time to collect 90% of detected photons".
+ *   lce_out[s][g] = detected[s][g] / generated[s],  generated[s] = sum over the 8 columns of fate_by_source[s]   (NaN if 0 generated)
+ *   t90_out[s]    = the time by which the fraction `quantile` (0.9 for t90) of the photons counted in time_hist[s] has arrived.
+ *                   Reading T-t90 (the paper gives a definition, no estimator): with N = sum of the row and c(b) the count of bins
+ *                   0..b, take the first bin b with c(b) >= quantile N and place the crossing linearly inside it:
+ *                   t = t_min + dt (b + (quantile N - c(b-1)) / time_hist[s][b]).  NaN if the row is empty.  Underflow and overflow
+ *                   photons sit in the first and last bin (dw_tally clamps), so choose the range to hold the quantile.
+ * Sums and the division are done in double precision and rounded to fp32 once.  tables: the struct given to dw_tally (its detected,
+ * fate_by_source, time_hist, n_groups, n_bins, t_min, dt are read; nothing is modified).  lce_out [n_sources][n_groups] needs detected
+ * and fate_by_source, t90_out [n_sources] needs time_hist; either output may be NULL.  DEVICE pointers.  0 < quantile <= 1.
+ * Asynchronous on the stream. */
+int dw_tally_finish(dw_ctx* ctx, const dw_tally_tables* tables, int64_t n_sources, float quantile, float* lce_out, float* t90_out,
+                    void* cuda_stream);
+
+/* Many sources per launch ("close to 2500" point sources on a Z x R^2 grid, 1e6 photons
+ * each).  dw_emit for photon i of source i / photons_per_source, in ONE launch: out->n photons (at most n_sources *
+ * photons_per_source; the last source may be short), photon identity out->photon_id_base + i exactly as in dw_emit, so the photons are
+ * bit-identical to n_sources separate dw_emit calls with id bases out->photon_id_base + s * photons_per_source.
+ * sources: HOST pointer [n_sources] (copied to the device on the stream before the launch); out: DEVICE arrays.  Asynchronous,
+ * except that a pageable host array is read before the call returns. */
+int dw_emit_sources(dw_ctx* ctx, const dw_source* sources, int64_t n_sources, int64_t photons_per_source, uint64_t seed,
+                    const dw_photons* out, void* cuda_stream);
+
+/* The design-study loop of PAPER.md sections 4.1-4.2 (lines 189, 211, 249-253, 267-271) as one call: for sources_per_batch sources
+ * at a time dw_emit_sources -> dw_propagate -> dw_tally into `tables` (rows = sources, ACCUMULATED: the caller zeroes), then
+ * dw_tally_finish.  Photon ids are s * photons_per_source + i for photon i of source s, so no result depends on sources_per_batch.
+ * sources: HOST [n_sources]; tables and lce_out / t90_out (may be NULL): DEVICE.  sources_per_batch <= 0: as many as fit 2^25 photons.
+ * The call allocates and frees its photon and result buffers on the stream (60 B per photon of a batch).  Asynchronous like
+ * dw_emit_sources. */
+int dw_design_study(dw_ctx* ctx, const dw_source* sources, int64_t n_sources, int64_t photons_per_source, uint64_t seed,
+                    int32_t max_steps, const dw_tally_tables* tables, int64_t sources_per_batch, float quantile, float* lce_out,
+                    float* t90_out, void* cuda_stream);
 
 
 /* Measured denominators for the roofline (SURVEY.md 8(d) "Peaks": the driver's peaks file holds HBM and

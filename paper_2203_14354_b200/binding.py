@@ -26,7 +26,8 @@ PROP_NO_EMPTY_SKIP = 4
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
-           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh", "dw_render")
+           "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh", "dw_render",
+           "dw_tally_finish", "dw_emit_sources", "dw_design_study")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -93,6 +94,10 @@ def load(build_if_missing: bool = True) -> C.CDLL:
         if not build_if_missing:
             raise RuntimeError(f"{_LIB_PATH} is missing: run `python -m paper_2203_14354_b200.build`")
         _build.build()
+    elif _build.needs_build():                      # sources newer than the library: never run a stale build silently
+        if not build_if_missing or not _build.have_nvcc():
+            raise RuntimeError(f"{_LIB_PATH} is older than its sources: run `python -m paper_2203_14354_b200.build`")
+        _build.build()
     L = C.CDLL(str(_LIB_PATH))
     L.dw_create.argtypes = [C.c_int, C.POINTER(vp)]
     L.dw_destroy.argtypes = [vp]
@@ -113,6 +118,9 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     L.dw_emit.argtypes = [vp, C.POINTER(Source), u64, C.POINTER(Photons), vp]
     L.dw_probe_peaks.argtypes = [vp, vp]
     L.dw_tally.argtypes = [vp, C.POINTER(Results), i64, i64, C.POINTER(TallyTables), vp]
+    L.dw_tally_finish.argtypes = [vp, C.POINTER(TallyTables), i64, f32, vp, vp, vp]
+    L.dw_emit_sources.argtypes = [vp, C.POINTER(Source), i64, i64, u64, C.POINTER(Photons), vp]
+    L.dw_design_study.argtypes = [vp, C.POINTER(Source), i64, i64, u64, i32, C.POINTER(TallyTables), i64, f32, vp, vp, vp]
     L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
     for name in EXPORTS:
         if name not in ("dw_last_error",):
@@ -236,10 +244,16 @@ class Context:
     def emit(self, source: dict, seed: int, n: int, id_base: int = 0, device="cuda:0", stream=None) -> "EmittedPhotons":
         """n scintillation photons of `source` (see synth.source) generated on the device; the result goes to propagate()."""
         out = EmittedPhotons(n, id_base, device)
-        src = Source(shape=int(source["shape"]), centre=(f32 * 3)(*source["centre"]), radius=source["radius"], z0=source["z0"],
-                     z1=source["z1"], lambda_mean=source["lambda_mean"], lambda_sigma=source["lambda_sigma"],
-                     t_start=source["t_start"], tau1=source["tau1"], tau3=source["tau3"], f_singlet=source["f_singlet"])
-        self._check(self.L.dw_emit(self.h, C.byref(src), int(seed), C.byref(out.c), _stream_ptr(stream)))
+        self._check(self.L.dw_emit(self.h, C.byref(_source(source)), int(seed), C.byref(out.c), _stream_ptr(stream)))
+        return out
+
+    def emit_sources(self, sources, photons_per_source: int, seed: int, n: int | None = None, id_base: int = 0, device="cuda:0",
+                     stream=None) -> "EmittedPhotons":
+        """One launch for many sources (dw_emit_sources): photon i belongs to sources[i // photons_per_source]."""
+        n = len(sources) * int(photons_per_source) if n is None else int(n)
+        out = EmittedPhotons(n, id_base, device)
+        arr = (Source * len(sources))(*[_source(s) for s in sources])
+        self._check(self.L.dw_emit_sources(self.h, arr, len(sources), int(photons_per_source), int(seed), C.byref(out.c), _stream_ptr(stream)))
         return out
 
     # ---- design-study reductions (SURVEY.md 8(f) f3) ------------------------------------------------------
@@ -248,32 +262,26 @@ class Context:
         acc.check_sources(n, photons_per_source)
         self._check(self.L.dw_tally(self.h, C.byref(results.c), int(n), int(photons_per_source), C.byref(acc.c), _stream_ptr(stream)))
 
+    def tally_finish(self, acc: "Tally", quantile: float = 0.9, stream=None):
+        """LCE per source and group and t90 per source from the tables of `acc`, computed by the library (dw_tally_finish)."""
+        self._check(self.L.dw_tally_finish(self.h, C.byref(acc.c), acc.ns, float(quantile), _dp(acc.lce),
+                                           _dp(acc.t90) if acc.nb > 0 else None, _stream_ptr(stream)))
+
     def design_study(self, sources, photons_per_source, seed, max_steps, channel_group, n_groups, tri_component, n_components,
-                     n_bins=2000, t_min=0.0, dt=1.0, sources_per_batch=32, device="cuda:0"):
-        """The paper's design-study loop on the device: for every source emit
-        photons_per_source photons, propagate, and reduce to LCE per source and sensor array, arrival-time histograms (t90) and the
-        table of absorbed photons by component.  Photon ids are source_index * photons_per_source + i, so a result does not
-        depend on sources_per_batch.  Returns a dict of numpy arrays."""
+                     n_bins=2000, t_min=0.0, dt=1.0, sources_per_batch=32, device="cuda:0", quantile=0.9):
+        """The paper's design-study loop as ONE library call (dw_design_study): emission of
+        all sources of a batch in one launch, propagation, reduction to LCE per source and sensor array, arrival-time histograms,
+        t90 and the table of absorbed photons by component.  Photon ids are source_index * photons_per_source + i, so a result does
+        not depend on sources_per_batch.  Returns a dict of numpy arrays."""
         import torch
         ns = len(sources)
         acc = Tally(ns, channel_group, n_groups, tri_component, n_components, n_bins, t_min, dt, device)
-        pps = int(photons_per_source)
-        for b0 in range(0, ns, sources_per_batch):
-            b1 = min(ns, b0 + sources_per_batch)
-            nb = (b1 - b0) * pps
-            batch = EmittedPhotons(nb, b0 * pps, device)
-            for k, src in enumerate(sources[b0:b1]):            # one emission per source into its slice of the batch
-                part = _PhotonsBase()
-                part._fill({name: batch.t[name][k * pps:(k + 1) * pps] for name in _IN}, pps, (b0 + k) * pps)
-                s = Source(shape=int(src["shape"]), centre=(f32 * 3)(*src["centre"]), radius=src["radius"], z0=src["z0"], z1=src["z1"],
-                           lambda_mean=src["lambda_mean"], lambda_sigma=src["lambda_sigma"], t_start=src["t_start"], tau1=src["tau1"],
-                           tau3=src["tau3"], f_singlet=src["f_singlet"])
-                self._check(self.L.dw_emit(self.h, C.byref(s), int(seed), C.byref(part.c), _stream_ptr()))
-            out = DeviceResults(nb, ("flags", "channel", "t", "last_tri"), device)
-            self.propagate(batch, seed, max_steps, out, None)
-            self.tally(out, nb, pps, acc.view(b0, b1))
+        arr = (Source * ns)(*[_source(s) for s in sources])
+        self._check(self.L.dw_design_study(self.h, arr, ns, int(photons_per_source), int(seed), int(max_steps), C.byref(acc.c),
+                                           int(sources_per_batch), float(quantile), _dp(acc.lce), _dp(acc.t90) if acc.nb > 0 else None,
+                                           _stream_ptr()))
         torch.cuda.synchronize()
-        return acc.numpy(pps)
+        return acc.numpy()
 
     def probe_peaks(self) -> dict:
         """Measured issue rates and L2 read bandwidth of this device (include/darwinopt.h dw_probe_peaks)."""
@@ -333,6 +341,12 @@ class Context:
 _IN = ("px", "py", "pz", "kx", "ky", "kz", "ex", "ey", "ez", "wavelength", "t0")
 _OUT_DT = dict(flags="int32", channel="int32", t="float32", steps="int32", last_tri="int32", x="float32", y="float32",
                z="float32", kx="float32", ky="float32", kz="float32", ex="float32", ey="float32", ez="float32")
+
+
+def _source(src: dict) -> Source:
+    return Source(shape=int(src["shape"]), centre=(f32 * 3)(*src["centre"]), radius=src["radius"], z0=src["z0"], z1=src["z1"],
+                  lambda_mean=src["lambda_mean"], lambda_sigma=src["lambda_sigma"], t_start=src["t_start"], tau1=src["tau1"],
+                  tau3=src["tau3"], f_singlet=src["f_singlet"])
 
 
 class _PhotonsBase:
@@ -480,6 +494,8 @@ class Tally:
         self.time_hist = z((max(self.ns, 1), max(self.nb, 1)), torch.int32)
         self.fate_by_source = z((max(self.ns, 1), 8), torch.int64)
         self.absorbed = z((self.K,), torch.int64)
+        self.lce = torch.full((max(self.ns, 1), self.G), float("nan"), dtype=torch.float32, device=device)   # written by the library
+        self.t90 = torch.full((max(self.ns, 1),), float("nan"), dtype=torch.float32, device=device)
         self.c = self._tables(0)
         self._limit = self.ns
 
@@ -502,26 +518,10 @@ class Tally:
         if -(-int(n) // int(pps)) > self._limit:
             raise ValueError(f"{n} photons at {pps} per source need more than the {self._limit} sources of these tables")
 
-    def numpy(self, photons_per_source=None):
+    def numpy(self):
+        """The tables, and lce / t90 as dw_tally_finish / dw_design_study wrote them (NaN until one of them has run)."""
         det = self.detected[: self.ns].cpu().numpy().astype(np.uint64)
-        out = dict(detected=det, time_hist=self.time_hist[: self.ns, : self.nb].cpu().numpy().view(np.uint32).astype(np.uint64),
-                   fate_by_source=self.fate_by_source[: self.ns].cpu().numpy().astype(np.uint64),
-                   absorbed_by_component=self.absorbed.cpu().numpy().astype(np.uint64))
-        if photons_per_source:
-            gen = out["fate_by_source"].sum(1).astype(np.float64)
-            out["lce"] = det / np.maximum(gen, 1.0)[:, None]
-            out["t90"] = np.array([t90_from_hist(h, self.t_min, self.dt) for h in out["time_hist"]]) if self.nb > 0 else None
-        return out
-
-
-def t90_from_hist(hist, t_min, dt, q=0.9):
-    """Time by which the fraction q of the detected photons has arrived: linear interpolation inside the bin
-    where the cumulative count crosses q of the total; NaN if nothing was detected."""
-    h = np.asarray(hist, np.float64)
-    tot = h.sum()
-    if tot <= 0:
-        return float("nan")
-    cum = np.cumsum(h)
-    b = int(np.searchsorted(cum, q * tot, side="left"))
-    below = cum[b - 1] if b > 0 else 0.0
-    return float(t_min + dt * (b + (q * tot - below) / h[b]))
+        return dict(detected=det, time_hist=self.time_hist[: self.ns, : self.nb].cpu().numpy().view(np.uint32).astype(np.uint64),
+                    fate_by_source=self.fate_by_source[: self.ns].cpu().numpy().astype(np.uint64),
+                    absorbed_by_component=self.absorbed.cpu().numpy().astype(np.uint64),
+                    lce=self.lce[: self.ns].cpu().numpy(), t90=self.t90[: self.ns].cpu().numpy() if self.nb > 0 else None)

@@ -21,6 +21,13 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+def have_nvcc() -> bool:
+    try:
+        return subprocess.call([_nvcc(), "--version"], stdout=subprocess.DEVNULL, stderr=subprocess.DEVNULL) == 0
+    except Exception:
+        return False
+
+
 def needs_build() -> bool:
     if not LIB.exists():
         return True

@@ -375,21 +375,157 @@ extern "C" int dw_tally(dw_ctx* c, const dw_results* res, int64_t n, int64_t pps
   return DW_OK;
 }
 
+// LCE and t90 from the accumulated tables (dw_tally_finish).  One warp per source: the row of the arrival-time
+// histogram is summed, then scanned 32 bins at a time until the running count reaches quantile x total; the crossing is placed
+// linearly inside that bin.  Sums and divisions in double (the counts are integers), one rounding to fp32 at the end.
+__global__ void tally_finish_kernel(dw_tally_tables T, int64_t ns, double quantile, float* __restrict__ lce, float* __restrict__ t90) {
+  const int lane = threadIdx.x & 31;
+  const int64_t s = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  if (s >= ns) return;
+  if (lce) {
+    unsigned long long gen = lane < 8 ? (unsigned long long)T.fate_by_source[s * 8 + lane] : 0ull;
+    for (int o = 4; o > 0; o >>= 1) gen += __shfl_xor_sync(0xffffffffu, gen, o);
+    gen = __shfl_sync(0xffffffffu, gen, 0);
+    for (int g = lane; g < T.n_groups; g += 32)
+      lce[s * T.n_groups + g] = gen ? (float)((double)T.detected[s * T.n_groups + g] / (double)gen) : __int_as_float(0x7fc00000);
+  }
+  if (t90) {
+    const uint32_t* row = T.time_hist + s * T.n_bins;
+    unsigned long long tot = 0;
+    for (int64_t b = lane; b < T.n_bins; b += 32) tot += row[b];
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    float res = __int_as_float(0x7fc00000);                     // NaN: nothing was detected
+    if (tot > 0) {
+      const double target = quantile * (double)tot;
+      unsigned long long before = 0;                            // count of all bins below the current group of 32
+      for (int64_t b0 = 0; b0 < T.n_bins; b0 += 32) {
+        const int64_t b = b0 + lane;
+        const unsigned long long mine = b < T.n_bins ? row[b] : 0u;
+        unsigned long long incl = mine;                         // inclusive prefix sum over the group
+        for (int o = 1; o < 32; o <<= 1) {
+          const unsigned long long up = __shfl_up_sync(0xffffffffu, incl, o);
+          if (lane >= o) incl += up;
+        }
+        const unsigned hit = __ballot_sync(0xffffffffu, b < T.n_bins && (double)(before + incl) >= target && mine > 0);
+        if (hit) {
+          const int l = __ffs(hit) - 1;
+          const unsigned long long below = before + __shfl_sync(0xffffffffu, incl, l) - __shfl_sync(0xffffffffu, mine, l);
+          const double inside = (target - (double)below) / (double)__shfl_sync(0xffffffffu, mine, l);
+          res = (float)((double)T.t_min + (double)T.dt * ((double)(b0 + l) + inside));
+          break;
+        }
+        before += __shfl_sync(0xffffffffu, incl, 31);
+      }
+    }
+    if (lane == 0) t90[s] = res;
+  }
+}
+
+extern "C" int dw_tally_finish(dw_ctx* c, const dw_tally_tables* T, int64_t ns, float quantile, float* lce, float* t90, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!T || ns < 0 || !(quantile > 0.f && quantile <= 1.f)) return dw_fail(c, DW_E_ARG, "dw_tally_finish: null tables, n_sources < 0 or quantile outside (0, 1]");
+  if (lce && (!T->detected || !T->fate_by_source || T->n_groups < 1)) return dw_fail(c, DW_E_ARG, "dw_tally_finish: lce_out needs detected, fate_by_source and n_groups >= 1");
+  if (t90 && (!T->time_hist || T->n_bins < 1 || !(T->dt > 0.f))) return dw_fail(c, DW_E_ARG, "dw_tally_finish: t90_out needs time_hist, n_bins >= 1 and dt > 0");
+  if (ns == 0 || (!lce && !t90)) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  tally_finish_kernel<<<(unsigned)((ns * 32 + 255) / 256), 256, 0, (cudaStream_t)stream>>>(*T, ns, (double)quantile, lce, t90);
+  DW_CUDA(c, cudaGetLastError());
+  return DW_OK;
+}
+
+static int check_source(dw_ctx* c, const char* who, const dw_source* src) {
+  if (src->shape < DW_SOURCE_POINT || src->shape > DW_SOURCE_BALL) return dw_fail(c, DW_E_ARG, "%s: unknown shape %d", who, src->shape);
+  const float chk[] = {src->centre[0], src->centre[1], src->centre[2], src->radius, src->z0, src->z1, src->lambda_mean, src->lambda_sigma,
+                       src->t_start, src->tau1, src->tau3, src->f_singlet};
+  for (float v : chk) if (!std::isfinite(v)) return dw_fail(c, DW_E_ARG, "%s: non-finite source parameter", who);
+  if (src->radius < 0.f || src->lambda_sigma < 0.f || src->tau1 < 0.f || src->tau3 < 0.f || src->z1 < src->z0 ||
+      src->f_singlet < 0.f || src->f_singlet > 1.f)
+    return dw_fail(c, DW_E_ARG, "%s: radius, sigma, tau must be >= 0, z0 <= z1, 0 <= f_singlet <= 1", who);
+  return DW_OK;
+}
+static int check_emit_out(dw_ctx* c, const char* who, const dw_photons* out) {
+  if (out->n < 0) return dw_fail(c, DW_E_ARG, "%s: n < 0", who);
+  const float* const arr[11] = {out->px, out->py, out->pz, out->kx, out->ky, out->kz, out->ex, out->ey, out->ez, out->wavelength, out->t0};
+  if (out->n > 0) for (const float* a : arr) if (!a) return dw_fail(c, DW_E_ARG, "%s: null output array", who);
+  return DW_OK;
+}
+
 extern "C" int dw_emit(dw_ctx* c, const dw_source* src, uint64_t seed, const dw_photons* out, void* stream) {
   if (!c) return DW_E_ARG;
   if (!src || !out) return dw_fail(c, DW_E_ARG, "dw_emit: null source or output");
-  if (out->n < 0) return dw_fail(c, DW_E_ARG, "dw_emit: n < 0");
-  if (src->shape < DW_SOURCE_POINT || src->shape > DW_SOURCE_BALL) return dw_fail(c, DW_E_ARG, "dw_emit: unknown shape %d", src->shape);
-  const float chk[] = {src->centre[0], src->centre[1], src->centre[2], src->radius, src->z0, src->z1, src->lambda_mean, src->lambda_sigma,
-                       src->t_start, src->tau1, src->tau3, src->f_singlet};
-  for (float v : chk) if (!std::isfinite(v)) return dw_fail(c, DW_E_ARG, "dw_emit: non-finite source parameter");
-  if (src->radius < 0.f || src->lambda_sigma < 0.f || src->tau1 < 0.f || src->tau3 < 0.f || src->z1 < src->z0 ||
-      src->f_singlet < 0.f || src->f_singlet > 1.f)
-    return dw_fail(c, DW_E_ARG, "dw_emit: radius, sigma, tau must be >= 0, z0 <= z1, 0 <= f_singlet <= 1");
-  const float* const arr[11] = {out->px, out->py, out->pz, out->kx, out->ky, out->kz, out->ex, out->ey, out->ez, out->wavelength, out->t0};
-  if (out->n > 0) for (const float* a : arr) if (!a) return dw_fail(c, DW_E_ARG, "dw_emit: null output array");
+  int rc = check_emit_out(c, "dw_emit", out);
+  if (rc) return rc;
+  rc = check_source(c, "dw_emit", src);
+  if (rc) return rc;
   DW_CUDA(c, cudaSetDevice(c->device));
   return dw_emit_impl(c, src, seed, out, (cudaStream_t)stream);
+}
+
+// Stream-ordered scratch from the context's pool (memory is kept between calls).
+static cudaError_t scratch_alloc(dw_ctx* c, void** p, size_t bytes, cudaStream_t s) {
+  return c->pool ? cudaMallocFromPoolAsync(p, bytes, c->pool, s) : cudaMallocAsync(p, bytes, s);
+}
+
+static int upload_sources(dw_ctx* c, const char* who, const dw_source* sources, int64_t ns, dw_source** d_out, cudaStream_t s) {
+  for (int64_t i = 0; i < ns; ++i) { int rc = check_source(c, who, sources + i); if (rc) return rc; }
+  DW_CUDA(c, scratch_alloc(c, (void**)d_out, sizeof(dw_source) * (size_t)ns, s));
+  cudaError_t e = cudaMemcpyAsync(*d_out, sources, sizeof(dw_source) * (size_t)ns, cudaMemcpyHostToDevice, s);
+  if (e != cudaSuccess) { cudaFreeAsync(*d_out, s); *d_out = nullptr; return dw_fail(c, DW_E_CUDA, "%s: copy of the sources failed: %s", who, cudaGetErrorString(e)); }
+  return DW_OK;
+}
+
+extern "C" int dw_emit_sources(dw_ctx* c, const dw_source* sources, int64_t ns, int64_t pps, uint64_t seed, const dw_photons* out, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!sources || !out || ns < 1 || pps < 1) return dw_fail(c, DW_E_ARG, "dw_emit_sources: null argument, n_sources < 1 or photons_per_source < 1");
+  int rc = check_emit_out(c, "dw_emit_sources", out);
+  if (rc) return rc;
+  if (out->n > ns * pps) return dw_fail(c, DW_E_ARG, "dw_emit_sources: %lld photons need more than %lld sources of %lld", (long long)out->n, (long long)ns, (long long)pps);
+  if (out->n == 0) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)stream;
+  dw_source* d_src = nullptr;
+  rc = upload_sources(c, "dw_emit_sources", sources, ns, &d_src, s);
+  if (rc) return rc;
+  rc = dw_emit_sources_impl(c, d_src, pps, seed, out, s);
+  cudaFreeAsync(d_src, s);
+  return rc;
+}
+
+extern "C" int dw_design_study(dw_ctx* c, const dw_source* sources, int64_t ns, int64_t pps, uint64_t seed, int32_t max_steps,
+                               const dw_tally_tables* T, int64_t spb, float quantile, float* lce, float* t90, void* stream) {
+  if (!c) return DW_E_ARG;
+  if (!c->built) return dw_fail(c, DW_E_STATE, "dw_design_study: build the BVH first");
+  if (!sources || !T || ns < 1 || pps < 1 || max_steps < 0) return dw_fail(c, DW_E_ARG, "dw_design_study: null argument, n_sources < 1, photons_per_source < 1 or max_steps < 0");
+  if (pps > (int64_t(1) << 30)) return dw_fail(c, DW_E_ARG, "dw_design_study: photons_per_source above 2^30");
+  if (spb <= 0) spb = std::max<int64_t>(1, (int64_t(1) << 25) / pps);
+  spb = std::min(spb, ns);
+  DW_CUDA(c, cudaSetDevice(c->device));
+  cudaStream_t s = (cudaStream_t)stream;
+  dw_source* d_src = nullptr;
+  int rc = upload_sources(c, "dw_design_study", sources, ns, &d_src, s);
+  if (rc) return rc;
+  const int64_t cap = spb * pps;                       // photons of a full batch
+  float* buf = nullptr;                                // 11 input arrays + flags, channel, t, last_tri
+  cudaError_t e = scratch_alloc(c, (void**)&buf, sizeof(float) * 15 * (size_t)cap, s);
+  if (e != cudaSuccess) { cudaFreeAsync(d_src, s); return dw_fail(c, DW_E_CUDA, "dw_design_study: %zu bytes of batch buffers: %s", sizeof(float) * 15 * (size_t)cap, cudaGetErrorString(e)); }
+  auto arr = [&](int k) { return buf + (size_t)k * cap; };
+  for (int64_t s0 = 0; s0 < ns && rc == DW_OK; s0 += spb) {
+    const int64_t nsb = std::min(spb, ns - s0), nb = nsb * pps;
+    dw_photons ph{nb, (uint64_t)(s0 * pps), arr(0), arr(1), arr(2), arr(3), arr(4), arr(5), arr(6), arr(7), arr(8), arr(9), arr(10)};
+    dw_results res{};
+    res.flags = (uint32_t*)arr(11); res.channel = (int32_t*)arr(12); res.t = arr(13); res.last_tri = (int32_t*)arr(14);
+    dw_tally_tables tb = *T;                           // the same tables seen from source s0 on
+    if (tb.detected) tb.detected += s0 * tb.n_groups;
+    if (tb.time_hist) tb.time_hist += s0 * tb.n_bins;
+    if (tb.fate_by_source) tb.fate_by_source += s0 * 8;
+    rc = dw_emit_sources_impl(c, d_src + s0, pps, seed, &ph, s);
+    if (rc == DW_OK) rc = dw_propagate_impl(c, &ph, seed, max_steps, &res, nullptr, nullptr, s);
+    if (rc == DW_OK) rc = dw_tally(c, &res, nb, pps, &tb, s);
+  }
+  if (rc == DW_OK && (lce || t90)) rc = dw_tally_finish(c, T, ns, quantile, lce, t90, s);
+  cudaFreeAsync(buf, s);
+  cudaFreeAsync(d_src, s);
+  return rc;
 }
 
 extern "C" int dw_debug_philox(dw_ctx* c, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,

@@ -127,5 +127,7 @@ int dw_propagate_impl(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t 
                       const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream);
 int dw_render_impl(dw_ctx* ctx, const dw_camera* cam, int32_t* tri, float* depth, uint8_t* shade, cudaStream_t stream);
 int dw_emit_impl(dw_ctx* ctx, const dw_source* src, uint64_t seed, const dw_photons* out, cudaStream_t stream);
+int dw_emit_sources_impl(dw_ctx* ctx, const dw_source* d_sources, int64_t photons_per_source, uint64_t seed, const dw_photons* out,
+                         cudaStream_t stream);
 int dw_debug_philox_impl(dw_ctx* ctx, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
                          uint32_t* out_raw, float* out_u, cudaStream_t stream);

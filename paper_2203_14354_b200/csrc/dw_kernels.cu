@@ -1119,9 +1119,7 @@ __device__ __forceinline__ V3 isotropic(float u_cos, float u_phi) {
   sincospif(2.0f * u_phi, &sp, &cp);
   return mk(st * cp, st * sp, ct);
 }
-__global__ void emit_kernel(dw_source S, uint64_t seed, dw_photons P) {
-  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (i >= P.n) return;
+__device__ __forceinline__ void emit_one(const dw_source& S, uint64_t seed, const dw_photons& P, int64_t i) {
   const uint64_t pid = P.photon_id_base + (uint64_t)i;
   const float4 a = draw4(seed, pid, kEmitStep, 0u), b = draw4(seed, pid, kEmitStep, 1u), c = draw4(seed, pid, kEmitStep, 2u);
   V3 x = mk(S.centre[0], S.centre[1], S.centre[2]);
@@ -1143,6 +1141,21 @@ __global__ void emit_kernel(dw_source S, uint64_t seed, dw_photons P) {
   float* const* o = (float* const*)&P.px;          // the eleven arrays follow each other in dw_photons
   o[0][i] = x.x; o[1][i] = x.y; o[2][i] = x.z; o[3][i] = k.x; o[4][i] = k.y; o[5][i] = k.z;
   o[6][i] = e.x; o[7][i] = e.y; o[8][i] = e.z; o[9][i] = lambda; o[10][i] = t;
+}
+__global__ void emit_kernel(dw_source S, uint64_t seed, dw_photons P) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < P.n) emit_one(S, seed, P, i);
+}
+// dw_emit_sources: photon i belongs to source i / pps (many point sources per study); the source record is read through
+// the read-only path (neighbouring photons share it).
+__global__ void emit_sources_kernel(const dw_source* __restrict__ S, int64_t pps, uint64_t seed, dw_photons P) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= P.n) return;
+  const int4* q = reinterpret_cast<const int4*>(S + i / pps);
+  static_assert(sizeof(dw_source) == 64, "dw_source is read as four 128-bit words");
+  union { int4 w[4]; dw_source s; } u;
+  u.w[0] = __ldg(q); u.w[1] = __ldg(q + 1); u.w[2] = __ldg(q + 2); u.w[3] = __ldg(q + 3);
+  emit_one(u.s, seed, P, i);
 }
 
 __global__ void philox_debug_kernel(uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
@@ -1312,6 +1325,13 @@ int dw_emit_impl(dw_ctx* c, const dw_source* src, uint64_t seed, const dw_photon
   static_assert(offsetof(dw_photons, t0) - offsetof(dw_photons, px) == 10 * sizeof(float*), "dw_photons: eleven consecutive arrays");
   if (out->n == 0) return DW_OK;
   emit_kernel<<<(unsigned)((out->n + 255) / 256), 256, 0, stream>>>(*src, seed, *out);
+  DW_CUDA(c, cudaGetLastError());
+  return DW_OK;
+}
+
+int dw_emit_sources_impl(dw_ctx* c, const dw_source* d_sources, int64_t pps, uint64_t seed, const dw_photons* out, cudaStream_t stream) {
+  if (out->n == 0) return DW_OK;
+  emit_sources_kernel<<<(unsigned)((out->n + 255) / 256), 256, 0, stream>>>(d_sources, pps, seed, *out);
   DW_CUDA(c, cudaGetLastError());
   return DW_OK;
 }

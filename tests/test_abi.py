@@ -60,7 +60,6 @@ def test_null_context_is_an_argument_error():
 def test_product_path_does_not_import_the_oracle():
     for p in (ROOT / "paper_2203_14354_b200").rglob("*"):
         if p.suffix in (".py", ".cu", ".cuh", ".h"):
-            assert "oracle" not in p.read_text().replace("the oracle", "").replace("The oracle", "").replace("oracle's", "").replace("oracle/", "").replace("oracle ", "").replace("oracle,", "").replace("oracle)", "").replace("oracle.", "X") or True
             src = p.read_text()
             assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, p
 

@@ -53,10 +53,10 @@ def oracle_for(i):
     return _ORC[i]
 
 
-def gpu_run(ctx, ph, seed, max_steps, n_bins=0, dt=1.0, fields=FULL, flags=0, **kw):
+def gpu_run(ctx, ph, seed, max_steps, n_bins=0, dt=1.0, fields=FULL, flags=0, t_min=0.0, **kw):
     d = dw.DevicePhotons(ph)
     out = dw.DeviceResults(ph.n, fields)
-    hist = dw.DeviceHists(ctx.n_chan, n_bins, 0.0, dt)
+    hist = dw.DeviceHists(ctx.n_chan, n_bins, t_min, dt)
     ctx.propagate(d, seed, max_steps, out, hist, flags=flags, **kw)
     torch.cuda.synchronize()
     r = out.numpy()
@@ -304,11 +304,43 @@ def test_c4_s2_spot_sweep(rho):
         pu.assert_channels_agree(h["chan_count"], n_gpu, ref["chan_count"], n_orc, "C4 per-PMT")
         p = pu.ks_pvalue(np.concatenate(times).astype(np.float64), ref["t"][ref["fate"] == orc.FATE_DETECTED])
         assert p > 0.01, f"C4 KS p = {p}"
-        # the last time bin is the overflow bin
-        assert h["time_hist"][-1] >= 0
+        # the histogram of the sweep is the count of the batches' own arrival times (fp32 binning, DESIGN.md T-bin); the last bin holds the overflow
+        tt = np.concatenate(times)
+        assert np.array_equal(h["time_hist"], fp32_time_hist(tt, 0.0, 1.0, 2000))
+        assert int(h["time_hist"][-1]) == int((tt >= np.float32(1999.0)).sum())
+        pu.assert_channels_agree(h["time_hist"], n_gpu, ref["time_hist"], n_orc, "C4 arrival-time histogram, bin by bin")
     finally:
         c3 = synth.config(3)
         ctx.set_surfaces(c3.optics.detect, c3.optics.reflect_diffuse, c3.optics.reflect_specular, c3.optics.transmit)
+
+
+def fp32_time_hist(t, t_min, dt, n_bins):
+    """S13 recomputed from per-photon arrival times in the kernel's precision (reading T-bin): bin = floor((t - t_min) / dt)
+    in fp32, clamped to [0, n_bins - 1]."""
+    fb = np.floor((np.asarray(t, np.float32) - np.float32(t_min)) / np.float32(dt))
+    b = np.clip(fb, 0, n_bins - 1).astype(np.int64)
+    return np.bincount(b, minlength=n_bins).astype(np.uint64)
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 600_000), (4, 1_500_000)])
+def test_histograms_are_counts_of_the_launch_outputs(cfg, n):
+    """a10 / S13: time_hist and chan_count of dw_propagate, bit for bit, against a recount from the launch's own per-photon t and
+    channel (two ranges: one that clamps at both ends, the 1 ns x 2000 bins of BASELINE.json configs[4]); and bin by bin within
+    4 sigma of the oracle's histogram of its own run."""
+    c, ctx = ctx_for(3 if cfg == 4 else cfg)
+    conf = synth.config(cfg) if cfg == 4 else c                     # C4: the C3 geometry and tables (rho = 0.95), the S2 spot as the source
+    ph = conf.make_photons(n)
+    n_orc = 300_000
+    o = oracle_for(3 if cfg == 4 else cfg)
+    for t_min, dt, nb in ((5.0, 0.7, 50), (0.0, 1.0, 2000)):
+        r = gpu_run(ctx, ph, conf.seed, conf.max_steps, nb, dt, fields=("flags", "channel", "t"), t_min=t_min)
+        det = r["fate"] == dw.FATE_DETECTED
+        want = fp32_time_hist(r["t"][det], t_min, dt, nb)
+        assert np.array_equal(r["time_hist"], want), (cfg, t_min, dt, nb)
+        assert want[0] > 0 and want[-1] > 0 or nb == 2000
+        assert np.array_equal(r["chan_count"], np.bincount(r["channel"][det], minlength=ctx.n_chan).astype(np.uint64))
+        ref = o.propagate(ph.slice(0, n_orc), conf.seed + 7, conf.max_steps, n_bins=nb, t_min=t_min, dt=dt, full=False)
+        pu.assert_channels_agree(r["time_hist"], n, ref["time_hist"], n_orc, f"C{cfg} arrival-time histogram ({nb} bins of {dt} ns)")
 
 
 # ------------------------------------------------------------------------------------------- invariants

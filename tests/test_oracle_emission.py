@@ -103,6 +103,15 @@ def test_emission_is_a_function_of_seed_and_photon_id_only():
         assert np.array_equal(whole[key][..., 2000:3000], part[key])
     other = orc.emit(src, 22, 1000, 5000)
     assert not np.array_equal(whole["wavelength"], other["wavelength"])
+    # a two-source batch (dw_emit_sources: photon i belongs to source i // m, ids base + i) is the two single-source batches one
+    # after the other: nothing of a photon depends on its neighbours or on where its batch starts
+    a, b, m = synth.source_for(4), synth.source(synth.SHAPE_POINT, (1.0, 2.0, 3.0)), 700
+    ids = np.arange(9000, 9000 + 2 * m)
+    for s_, one in ((a, slice(0, m)), (b, slice(m, 2 * m))):
+        full = orc.emit(s_, 21, 9000, 2 * m)
+        alone = orc.emit(s_, 21, int(ids[one][0]), m)
+        for key in ("pos", "dir", "pol", "wavelength", "t0"):
+            assert np.array_equal(full[key][..., one], alone[key])
     # the draws are the documented Philox blocks of step 0xFFFFFFFF (guards the counter layout, not the laws)
     u = orc.uniforms(21, 1000, 0xFFFFFFFF, 0)
     assert abs(whole["pos"][2][0] - (2.0 + 2597.0 * u[2])) < 1e-9

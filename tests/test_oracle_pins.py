@@ -506,6 +506,32 @@ def test_integrating_sphere():
     assert int(out["chan_count"][0]) == fc["detected"]
 
 
+# ----------------------------------------------------------------------------- S13 reductions are plain counting
+def test_time_histogram_and_channel_counts_are_counts_of_the_per_photon_outputs():
+    """S13 (arrival times of the detected photons; line 189: photons per sensor): orc_propagate's time_hist must be
+    numpy's histogram of its own per-photon t over the detected photons, bins [t_min + k dt, t_min + (k + 1) dt), with earlier
+    arrivals in the first bin and later ones in the last; chan_count must be numpy's bincount of its own per-photon channel.  The
+    range (5 ns, 50 bins of 0.7 ns) is chosen so that both clamps are hit on C1."""
+    c = synth.config(1)
+    o = orc.Oracle(c.geometry, c.optics, bvh=True)
+    N, t_min, dt, nb = 40000, 5.0, 0.7, 50
+    out = o.propagate(c.make_photons(N), c.seed, c.max_steps, n_bins=nb, t_min=t_min, dt=dt, full=False)
+    det = out["fate"] == orc.FATE_DETECTED
+    t = out["t"][det]
+    edges = t_min + dt * np.arange(nb + 1)
+    want, _ = np.histogram(t, bins=edges)
+    want = want.astype(np.uint64)
+    below, above = int((t < edges[0]).sum()), int((t > edges[-1]).sum())
+    assert below > 100 and above > 100                      # both clamps are exercised
+    want[0] += below
+    want[-1] += above
+    assert np.array_equal(out["time_hist"], want)
+    assert np.array_equal(out["chan_count"], np.bincount(out["channel"][det], minlength=o.n_chan).astype(np.uint64))
+    # a one-bin histogram holds everything; no histogram asked for is no histogram
+    one = o.propagate(c.make_photons(2000), c.seed, c.max_steps, n_bins=1, t_min=1e9, dt=1.0, full=False)
+    assert one["time_hist"].tolist() == [int((one["fate"] == orc.FATE_DETECTED).sum())]
+
+
 # ----------------------------------------------------------------------------- P9 conservation, P11 determinism
 def test_conservation_and_invariants_on_small_tpc():
     c = synth.config(1)
