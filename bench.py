@@ -217,6 +217,7 @@ def main():
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
+    ap.add_argument("--counters", action="store_true", help="also run the instrumented instantiation once and print its counters to stderr")
     ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="cap on resident blocks per SM (0 = occupancy limit)")
     args = ap.parse_args()

@@ -358,6 +358,18 @@ int dw_design_study(dw_ctx* ctx, const dw_source* sources, int64_t n_sources, in
  * About 0.1 s.  Not part of the hot path. */
 int dw_probe_peaks(dw_ctx* ctx, double out[4]);
 
+/* Diagnostics for the roofline line ("n_node and n_tri are measured by an instrumented build of the kernel"): runs the
+ * counting instantiation of the default propagation kernel once over `in` (DEVICE arrays; no per-photon outputs, no histograms) on the
+ * legacy default stream, waits, and writes DW_N_COUNTERS values to the HOST array counters_out:
+ *   [0] box-node visits  [1] ray-triangle tests  [2] queries traversed  [3] queries answered by the empty-space grid
+ *   [4] physics phases  [5] finished queries evaluated in them  [6] lanes that ran an iteration of the Rayleigh loop
+ *   [7] queries set up  [8] photons loaded  [9,10] iterations and active lanes of the box-node phase of the traversal loop
+ *   [11,12] the same of its triangle phase  [13] fetches of queued queries  [14] unused  [15] physics phases that ran a Rayleigh iteration
+ * Several times slower than dw_propagate (shared-memory atomics per event); never part of a timed region. */
+enum { DW_N_COUNTERS = 24 };
+int dw_propagate_counters(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,
+                          uint64_t* counters_out);
+
 /* Diagnostics / tests: raw Philox4x32-10 blocks and the uniforms the kernel derives from them, computed on the
  * device.  out_raw [n][4] uint32, out_u [n][4] float (either may be NULL), DEVICE pointers; entry i uses
  * photon id photon_id_base + i, the given step and block. */

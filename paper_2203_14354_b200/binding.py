@@ -23,11 +23,13 @@ H_FILM = 0x1000
 PROP_UNBOUNDED_QUERY = 1
 PROP_LEGACY_SCHEDULER = 2
 PROP_NO_EMPTY_SKIP = 4
+COUNTER_NAMES = ("node_visits", "tri_tests", "queries_traced", "queries_skipped", "physics_phases", "lanes_physics", "lanes_rayleigh",
+                 "lanes_setup", "lanes_fresh", "iters_node", "lanes_node", "iters_leaf", "lanes_leaf", "fetches", "lanes_fetch", "rayleigh_iters")
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
            "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh", "dw_render",
-           "dw_tally_finish", "dw_emit_sources", "dw_design_study")
+           "dw_tally_finish", "dw_emit_sources", "dw_design_study", "dw_propagate_counters")
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -114,6 +116,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
                                C.POINTER(PropagateParams), vp]
     L.dw_propagate_host.argtypes = [vp, C.POINTER(Photons), u64, i32, C.POINTER(Results), C.POINTER(Hists),
                                     C.POINTER(PropagateParams)]
+    L.dw_propagate_counters.argtypes = [vp, C.POINTER(Photons), u64, i32, C.POINTER(PropagateParams), vp]
     L.dw_debug_philox.argtypes = [vp, u64, u64, u32, u32, i64, vp, vp, vp]
     L.dw_emit.argtypes = [vp, C.POINTER(Source), u64, C.POINTER(Photons), vp]
     L.dw_probe_peaks.argtypes = [vp, vp]
@@ -311,6 +314,13 @@ class Context:
         shade = torch.empty(shape, dtype=torch.uint8, device=device)
         self._check(self.L.dw_render(self.h, C.byref(cam), _dp(tri), _dp(depth), _dp(shade), _stream_ptr(stream)))
         return tri, depth, shade
+
+    def propagate_counters(self, ph: "DevicePhotons", seed: int, max_steps: int, flags: int = 0, **kw) -> dict:
+        """The instrumented instantiation of the propagation kernel, once over `ph` (dw_propagate_counters): raw event counts."""
+        pp = PropagateParams(flags=flags, **kw)
+        out = (u64 * 24)()
+        self._check(self.L.dw_propagate_counters(self.h, C.byref(ph.c), seed, max_steps, C.byref(pp), out))
+        return {k: int(out[i]) for i, k in enumerate(COUNTER_NAMES)}
 
     def propagate(self, ph: "DevicePhotons", seed: int, max_steps: int, out: "DeviceResults | None" = None,
                   hist: "DeviceHists | None" = None, flags: int = 0, block_threads: int = 0, blocks_per_sm: int = 0,

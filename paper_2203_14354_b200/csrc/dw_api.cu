@@ -322,6 +322,18 @@ extern "C" int dw_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   return dw_propagate_impl(c, in, seed, max_steps, out, hist, params, (cudaStream_t)stream);
 }
 
+extern "C" int dw_propagate_counters(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,
+                                     uint64_t* out) {
+  if (!c) return DW_E_ARG;
+  if (!out) return dw_fail(c, DW_E_ARG, "dw_propagate_counters: counters_out is NULL");
+  int rc = check_batch(c, "dw_propagate_counters", in, max_steps, nullptr);
+  if (rc) return rc;
+  for (int i = 0; i < DW_N_COUNTERS; ++i) out[i] = 0;
+  if (in->n == 0) return DW_OK;
+  DW_CUDA(c, cudaSetDevice(c->device));
+  return dw_propagate_counters_impl(c, in, seed, max_steps, params, out, DW_N_COUNTERS);
+}
+
 // Counting over the per-photon results (dw_tally).  Neighbouring photons share their source, so equal keys are merged inside the
 // warp first (__match_any_sync) and each distinct key costs one atomic.
 __device__ __forceinline__ void warp_count64(unsigned long long* base, long long key, bool on) {

@@ -125,6 +125,8 @@ int dw_first_hit_impl(dw_ctx* ctx, int64_t n, const float* ox, const float* oy, 
                       cudaStream_t stream);
 int dw_propagate_impl(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
                       const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream);
+int dw_propagate_counters_impl(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,
+                               uint64_t* host_out, int n_out);
 int dw_render_impl(dw_ctx* ctx, const dw_camera* cam, int32_t* tri, float* depth, uint8_t* shade, cudaStream_t stream);
 int dw_emit_impl(dw_ctx* ctx, const dw_source* src, uint64_t seed, const dw_photons* out, cudaStream_t stream);
 int dw_emit_sources_impl(dw_ctx* ctx, const dw_source* d_sources, int64_t photons_per_source, uint64_t seed, const dw_photons* out,

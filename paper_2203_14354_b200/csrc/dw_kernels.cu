@@ -165,20 +165,22 @@ __device__ __forceinline__ void ldg256(const float4* p, float4& a, float4& b) {
   asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(p));
 }
-__device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
-  const float4* p = bvh.nodes + 8 * (size_t)s.node;
-  float4 lx, ly, lz, hx, hy, hz, rf;
+struct NodeRegs { float4 lx, ly, lz, hx, hy, hz, rf; };
+__device__ __forceinline__ void node_load(const DwBvh& bvh, int node, NodeRegs& n) {
+  const float4* p = bvh.nodes + 8 * (size_t)node;
 #if DW_NODE_LDG256   // three 256-bit loads for the planes, 128 bits for the references (the pad is not fetched: C2 236.4 -> 239.3, C3 222.0 -> 227.7)
-  ldg256(p, lx, ly); ldg256(p + 2, lz, hx); ldg256(p + 4, hy, hz); rf = __ldg(p + 6);
+  ldg256(p, n.lx, n.ly); ldg256(p + 2, n.lz, n.hx); ldg256(p + 4, n.hy, n.hz); n.rf = __ldg(p + 6);
 #else
-  lx = __ldg(p); ly = __ldg(p + 1); lz = __ldg(p + 2); hx = __ldg(p + 3); hy = __ldg(p + 4); hz = __ldg(p + 5); rf = __ldg(p + 6);
+  n.lx = __ldg(p); n.ly = __ldg(p + 1); n.lz = __ldg(p + 2); n.hx = __ldg(p + 3); n.hy = __ldg(p + 4); n.hz = __ldg(p + 5); n.rf = __ldg(p + 6);
 #endif
-  const int r0 = __float_as_int(rf.x), r1 = __float_as_int(rf.y), r2 = __float_as_int(rf.z), r3 = __float_as_int(rf.w);
+}
+__device__ __forceinline__ void node_process(const DwBvh& bvh, const Ray& r, TraceState& s, const NodeRegs& n, int* sstack, int sstride, int* lstack) {
+  const int r0 = __float_as_int(n.rf.x), r1 = __float_as_int(n.rf.y), r2 = __float_as_int(n.rf.z), r3 = __float_as_int(n.rf.w);
   float n0, n1, n2, n3;
-  const bool h0 = slab(r, s.best_t, bvh.eps_len, lx.x, ly.x, lz.x, hx.x, hy.x, hz.x, n0) && (r0 != DW_REF_NONE);
-  const bool h1 = slab(r, s.best_t, bvh.eps_len, lx.y, ly.y, lz.y, hx.y, hy.y, hz.y, n1) && (r1 != DW_REF_NONE);
-  const bool h2 = slab(r, s.best_t, bvh.eps_len, lx.z, ly.z, lz.z, hx.z, hy.z, hz.z, n2) && (r2 != DW_REF_NONE);
-  const bool h3 = slab(r, s.best_t, bvh.eps_len, lx.w, ly.w, lz.w, hx.w, hy.w, hz.w, n3) && (r3 != DW_REF_NONE);
+  const bool h0 = slab(r, s.best_t, bvh.eps_len, n.lx.x, n.ly.x, n.lz.x, n.hx.x, n.hy.x, n.hz.x, n0) && (r0 != DW_REF_NONE);
+  const bool h1 = slab(r, s.best_t, bvh.eps_len, n.lx.y, n.ly.y, n.lz.y, n.hx.y, n.hy.y, n.hz.y, n1) && (r1 != DW_REF_NONE);
+  const bool h2 = slab(r, s.best_t, bvh.eps_len, n.lx.z, n.ly.z, n.lz.z, n.hx.z, n.hy.z, n.hz.z, n2) && (r2 != DW_REF_NONE);
+  const bool h3 = slab(r, s.best_t, bvh.eps_len, n.lx.w, n.ly.w, n.lz.w, n.hx.w, n.hy.w, n.hz.w, n3) && (r3 != DW_REF_NONE);
   // Nearest hit child by compare-and-select on the references themselves (children of a node are distinct).  Do NOT
   // index the children by a computed position: nvcc turns that into a jump table (BRX) inside the traversal loop, and
   // on sm_100a lanes that diverge at that indirect branch were observed not to reconverge before the warp votes of
@@ -195,14 +197,30 @@ __device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, Tr
   if (h3 && next != r3) ts_push(s, r3, sstack, sstride, lstack);
   ts_goto(s, next, sstack, sstride, lstack);
 }
+__device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
+  NodeRegs n;
+  node_load(bvh, s.node, n);
+  node_process(bvh, r, s, n, sstack, sstride, lstack);
+}
 
 // One triangle of the current leaf (Moeller-Trumbore on the pre-packed record).  exclude: caller id to ignore.
 // medium >= 0: only triangles whose near side (the side the ray comes from) is `medium` count (DESIGN.md
 // "medium culling"); medium < 0: every triangle counts (the definition S1).  Ties -> lowest caller id.
-__device__ __forceinline__ void step_triangle(const DwBvh& bvh, const Ray& r, TraceState& s, int exclude, int medium,
-                                              const int* sstack, int sstride, const int* lstack) {
-  const float4* p = bvh.tris + 3 * (size_t)s.tri_cur;
-  float4 a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+struct TriRegs { float4 a, b, c; };
+__device__ __forceinline__ void ldg128v(const float4* p, float4& a) {   // volatile: the load stays where it is written (issued early)
+  asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w) : "l"(p));
+}
+__device__ __forceinline__ void tri_load(const DwBvh& bvh, int slot, TriRegs& t) {
+  const float4* p = bvh.tris + 3 * (size_t)slot;
+  t.a = __ldg(p); t.b = __ldg(p + 1); t.c = __ldg(p + 2);
+}
+__device__ __forceinline__ void tri_load_early(const DwBvh& bvh, int slot, TriRegs& t) {
+  const float4* p = bvh.tris + 3 * (size_t)slot;
+  ldg128v(p, t.a); ldg128v(p + 1, t.b); ldg128v(p + 2, t.c);
+}
+__device__ __forceinline__ void tri_process(const Ray& r, TraceState& s, const TriRegs& T, int exclude, int medium,
+                                            const int* sstack, int sstride, const int* lstack) {
+  const float4 a = T.a, b = T.b, c = T.c;
   V3 e1 = mk(a.w, b.x, b.y), e2 = mk(b.z, b.w, c.x);
   V3 pv = cross(r.d, e2);
   float det = dot(e1, pv);
@@ -224,6 +242,12 @@ __device__ __forceinline__ void step_triangle(const DwBvh& bvh, const Ray& r, Tr
     if (ok) { s.best_t = t; s.best_slot = s.tri_cur; s.best_id = id; }
   }
   if (++s.tri_cur == s.tri_end) ts_goto(s, DW_REF_NONE, sstack, sstride, lstack);
+}
+__device__ __forceinline__ void step_triangle(const DwBvh& bvh, const Ray& r, TraceState& s, int exclude, int medium,
+                                              const int* sstack, int sstride, const int* lstack) {
+  TriRegs T;
+  tri_load(bvh, s.tri_cur, T);
+  tri_process(r, s, T, exclude, medium, sstack, sstride, lstack);
 }
 
 __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, const float* __restrict__ ox,
@@ -407,6 +431,7 @@ struct PropArgs {
   uint32_t flags;
   int32_t th_phys, th_leaf;         // phase-scheduling thresholds (lanes)
   unsigned long long* queue_head;   // device counter, zeroed before launch
+  unsigned long long* counters;     // kCount instantiation only: [kCounters] diagnostic counters, accumulated
 };
 
 // Philox4x32-10 with the round keys read from the kernel parameters (A.keys): same values as draw4(A.seed, ...).
@@ -727,11 +752,28 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 #ifndef DW_NODE_REPS_MIN
 #define DW_NODE_REPS_MIN 16
 #endif
+
 // The film-enabled instantiation gets one block fewer per SM: at 80 registers it spills 106 bytes around the film call.
 // kFlat: all tables have one wavelength node (the BASELINE.json configs): a look-up is one load, no call.
-template <bool kFilm, bool kFlat>
+// The Rayleigh loop S6 runs at most DW_RAYL_REQUEUE iterations inside a physics phase; a slot that is still rejected then goes back
+// to the list of the phase with its iteration number and continues in the next one, with a phase full of slots.  (The whole loop
+// inside the phase ran its later iterations for the few lanes still rejected: 9 of 32 lanes on average over the loop; one iteration
+// per phase costs more in slot traffic than it saves: profiles/r02_experiments.md.)  Draws are keyed by (photon, step, block 1 + j):
+// same results.  0: the loop of the first build.
+#ifndef DW_RAYL_REQUEUE
+#define DW_RAYL_REQUEUE 0
+#endif
+constexpr int kRaylPending = -2;           // W_BEST_SLOT <= kRaylPending: iteration kRaylPending - W_BEST_SLOT of S6 is due
+// diagnostic counters of the kCount instantiation (dw_propagate_counters)
+enum : int { C_NODE = 0, C_TRI, C_TRACED, C_SKIPPED, C_PHASES, C_LANES_PHYS, C_LANES_RAYL, C_LANES_SETUP, C_LANES_FRESH, C_ITER_NODE, C_LANES_NODE,
+             C_ITER_LEAF, C_LANES_LEAF, C_FETCH, C_LANES_FETCH, C_RAYL_ITER, kCounters = 24 };
+
+template <bool kFilm, bool kFlat, bool kCount>
 __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
+  __shared__ unsigned long long s_cnt[kCount ? kCounters : 1];
+  if constexpr (kCount) { if (threadIdx.x < kCounters) s_cnt[threadIdx.x] = 0ull; }
+#define CNT(i, v) do { if constexpr (kCount) { if ((threadIdx.x & 31) == 0) atomicAdd(&s_cnt[i], (unsigned long long)(v)); } } while (0)
   auto TAB = [](const float* __restrict__ tab, int row, int nl, float l0, float inv_dl, float lam) -> float {
     if constexpr (kFlat) return __ldg(tab + row);
     else return table_at(tab, row, nl, l0, inv_dl, lam);
@@ -820,6 +862,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       else if (lane < nPc + take) { slot = q[lane]; fresh = true; pi = w_next + (lane - nPc); }
       w_next += take;
       if (nPc + take == 0) continue;                        // nothing to do this round (queue just ran dry)
+      CNT(C_PHASES, 1); CNT(C_LANES_PHYS, nPc); CNT(C_LANES_FRESH, take);
 
       V3 x = mk(0, 0, 0), k = mk(0, 0, 1), e = mk(1, 0, 0);
       float lambda = 0.f, t = 0.f, dbulk = INFINITY, n1 = 1.f, us = 0.f, uf = 0.f, best_t = INFINITY;
@@ -856,7 +899,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       uint32_t fate = 0xFFu;           // 0xFF = still running
       int channel = -1;
       const uint64_t pid = A.in.photon_id_base + (uint64_t)pi;
-      if (slot >= 0 && !fresh) {
+      int rj = -1;                     // iteration of the Rayleigh loop S6 that this lane runs in this phase (-1: none)
+      if (DW_RAYL_REQUEUE && slot >= 0 && !fresh && best_slot <= kRaylPending) rj = kRaylPending - best_slot;
+      if (slot >= 0 && !fresh && rj < 0) {
         // ---------------------------------------------------------- evaluate the finished query: S2..S9
         const bool bounded = (!literal) && (medium >= 0);
         const bool have_hit = best_slot >= 0;
@@ -901,7 +946,12 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
               if (absorb_first) {
                 fate = DW_FATE_BULK_ABSORBED;                         // S4 first branch
               } else {                                                // S4 second branch + S6
+#if DW_RAYL_REQUEUE
+                rj = 0;                                               // the loop runs below, one iteration per phase
+                --step;                                               // S9 counts the step when the loop ends
+#else
                 if (!rayleigh(k, e, [&](uint32_t b) { return DRAW_HOT(pid, step, b); })) fate = DW_FATE_NAN_ABORT;
+#endif
                 hist |= DW_H_RAYLEIGH;
                 last_tri = -1;
               }
@@ -954,7 +1004,37 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         }
         ++step;                                                       // S9 (every executed iteration counts, also the last: S13)
       }
-      if (slot >= 0 && fate == 0xFFu) {
+#if DW_RAYL_REQUEUE
+#pragma unroll 1
+      for (int it = 0; it < DW_RAYL_REQUEUE; ++it) {
+        const unsigned rm = __ballot_sync(0xffffffffu, rj >= 0);
+        if (!rm) break;
+        CNT(C_RAYL_ITER, 1); CNT(C_LANES_RAYL, __popc(rm));
+        if (rj >= 0) {
+          // ------------------------------------------------------ S6, iteration rj: isotropic k', accept with probability |e - (e.k')k'|^2
+          const float4 r = DRAW_HOT(pid, step, 1u + (uint32_t)rj);
+          const float ct = 1.0f - 2.0f * r.x;
+          const float st_ = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+          float sp, cp;
+          sincospif(2.0f * r.y, &sp, &cp);
+          const V3 kn = mk(st_ * cp, st_ * sp, ct);
+          const V3 er = fma3(-dot(e, kn), kn, e);
+          const float w = dot(er, er);
+          if (r.z < w) { k = kn; e = rsqrtf(w) * er; ++step; rj = -1; }          // S9
+          else if (rj + 1 >= 4096) { fate = DW_FATE_NAN_ABORT; ++step; rj = -1; } // the loop gives up (never observed)
+          else ++rj;
+        }
+      }
+      if (slot >= 0 && rj >= 0) {
+        // rejected: the slot waits for the next phase with the iteration number (position and time are those of the scatter point)
+        poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
+        poolf[W_T * kSlots + slot] = t;
+        pool[W_LAST * kSlots + slot] = last_tri;
+        pool[W_HIST * kSlots + slot] = (int)hist;
+        pool[W_BEST_SLOT * kSlots + slot] = kRaylPending - rj;
+      }
+#endif
+      if (slot >= 0 && fate == 0xFFu && rj < 0) {
         // ---------------------------------------------------------- set up the query of the next iteration: S1 (+S3/S4 draws)
         if ((int32_t)step >= A.max_steps) {
           fate = DW_FATE_TRUNCATED;                                   // S10
@@ -1012,6 +1092,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           poolf[W_BEST_T * kSlots + slot] = tmax;                     // the query starts from t_max
           pool[W_BEST_SLOT * kSlots + slot] = -1;
           st[slot] = skip ? S_PHYS : S_TRACE;                         // a skipped query is already finished: no hit
+          if constexpr (kCount) { atomicAdd(&s_cnt[C_LANES_SETUP], 1ull); if (skip) atomicAdd(&s_cnt[C_SKIPPED], 1ull); }
         }
       }
 
@@ -1066,7 +1147,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         q_exclude = pool[W_LAST * kSlots + my];
         q_medium = literal ? -1 : pool[W_MEDIUM * kSlots + my];
         st[my] = S_BUSY;
+        if constexpr (kCount) atomicAdd(&s_cnt[C_TRACED], 1ull);
       }
+      CNT(C_FETCH, 1);
       __syncwarp();
     }
     int nQ_rem = max(0, nQ - __popc(idle));
@@ -1085,16 +1168,24 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
 #if DW_NODE_REPS > 1
         // several node visits per vote while most lanes are in internal nodes: the votes are a quarter of the traversal's instructions
         const int reps = nI >= DW_NODE_REPS_MIN ? DW_NODE_REPS : 1;
+        CNT(C_ITER_NODE, reps); CNT(C_LANES_NODE, nI * reps);
 #pragma unroll 1
         for (int rep = 0; rep < reps; ++rep)
 #endif
-        if (act && ts.node >= 0) step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
+        if (act && ts.node >= 0) {
+          step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
+          if constexpr (kCount) atomicAdd(&s_cnt[C_NODE], 1ull);
+        }
       } else {
+        CNT(C_ITER_LEAF, DW_TRI_REPS); CNT(C_LANES_LEAF, nL * DW_TRI_REPS);
 #if DW_TRI_REPS > 1
 #pragma unroll 1
         for (int rep = 0; rep < DW_TRI_REPS; ++rep)
 #endif
-        if (act && ts.node == kInLeaf) step_triangle(A.bvh, ray, ts, q_exclude, q_medium, my_stack, sstride, lstack);
+        if (act && ts.node == kInLeaf) {
+          step_triangle(A.bvh, ray, ts, q_exclude, q_medium, my_stack, sstride, lstack);
+          if constexpr (kCount) atomicAdd(&s_cnt[C_TRI], 1ull);
+        }
       }
       if (act && ts.node == kDone) {                        // query finished: hand the slot to the physics phase
         poolf[W_BEST_T * kSlots + my] = ts.best_t;
@@ -1109,6 +1200,8 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   __syncthreads();
   if (threadIdx.x < 8 && A.hist.fate_count && s_fate[threadIdx.x]) atomicAdd((unsigned long long*)&A.hist.fate_count[threadIdx.x], (unsigned long long)s_fate[threadIdx.x]);
   if (threadIdx.x == 0 && A.hist.total_steps && s_steps) atomicAdd((unsigned long long*)A.hist.total_steps, s_steps);
+  if constexpr (kCount) { if (threadIdx.x < kCounters && A.counters && s_cnt[threadIdx.x]) atomicAdd(&A.counters[threadIdx.x], s_cnt[threadIdx.x]); }
+#undef CNT
 }
 
 // ------------------------------------------------------------------------------------------------ emission (f1)
@@ -1249,7 +1342,8 @@ int dw_render_impl(dw_ctx* c, const dw_camera* cam, int32_t* tri, float* depth, 
 
 // One launch over photons [0, in->n) of `in`; n <= kMaxLaunch for the pool kernel (slot word W_PI is 32 bits).
 static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
-                            const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream) {
+                            const dw_hists* hist, const dw_propagate_params* params, cudaStream_t stream,
+                            unsigned long long* counters = nullptr) {
   static_assert(sizeof(PropArgs) <= 4000, "kernel parameter block too large");
   PropArgs A{};
   A.bvh = c->bvh; A.tab = c->tables; A.in = *in;
@@ -1263,15 +1357,20 @@ static int launch_propagate(dw_ctx* c, const dw_photons* in, uint64_t seed, int3
   const bool legacy = (A.flags & DW_PROP_LEGACY_SCHEDULER) != 0;
   A.th_phys = (params && params->th_phys > 0) ? params->th_phys : (legacy ? 12 : 8);
   A.th_leaf = (params && params->th_leaf > 0) ? params->th_leaf : 12;
+  A.counters = counters;
   int B = (params && params->block_threads) ? params->block_threads : 128;
   if (B < 32 || B > 128 || (B & 31)) return dw_fail(c, DW_E_ARG, "dw_propagate: block_threads must be 32, 64, 96 or 128");
   int per_sm = 0;
   const bool films = c->tables.film != nullptr && c->tables.film_on != nullptr;
   const bool flat = DW_FLAT_TABLES && c->tables.nl_mat == 1 && c->tables.nl_surf == 1;
+  if (counters && legacy) return dw_fail(c, DW_E_ARG, "dw_propagate_counters: the counters exist in the default scheduler only");
   size_t smem = legacy ? sizeof(int) * kStackShared * B : sizeof(int) * (size_t)warp_ints(flat && !films) * (B / 32);
-  void (*kern)(PropArgs) = legacy ? (films ? propagate_kernel<true> : propagate_kernel<false>)
-                                  : (films ? (flat ? propagate_pool_kernel<true, true> : propagate_pool_kernel<true, false>)
-                                           : (flat ? propagate_pool_kernel<false, true> : propagate_pool_kernel<false, false>));
+  void (*kern)(PropArgs) = nullptr;
+  if (legacy) kern = films ? propagate_kernel<true> : propagate_kernel<false>;
+  else if (counters) kern = films ? (flat ? propagate_pool_kernel<true, true, true> : propagate_pool_kernel<true, false, true>)
+                                  : (flat ? propagate_pool_kernel<false, true, true> : propagate_pool_kernel<false, false, true>);
+  else kern = films ? (flat ? propagate_pool_kernel<true, true, false> : propagate_pool_kernel<true, false, false>)
+                    : (flat ? propagate_pool_kernel<false, true, false> : propagate_pool_kernel<false, false, false>);
   DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, B, smem));
   if (params && params->blocks_per_sm > 0) per_sm = std::min(per_sm, params->blocks_per_sm);
   if (per_sm < 1) return dw_fail(c, DW_E_CUDA, "dw_propagate: kernel does not fit on an SM");
@@ -1318,6 +1417,22 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
     int rc = launch_propagate(c, &pi, seed, max_steps, out ? &po : nullptr, hist, params, stream);
     if (rc != DW_OK) return rc;
   }
+  return DW_OK;
+}
+
+int dw_propagate_counters_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,
+                               uint64_t* host_out, int n_out) {
+  if (in->n > (int64_t(1) << 30)) return dw_fail(c, DW_E_ARG, "dw_propagate_counters: at most 2^30 photons");
+  unsigned long long* d = nullptr;
+  DW_CUDA(c, cudaMalloc(&d, sizeof(unsigned long long) * kCounters));
+  cudaMemset(d, 0, sizeof(unsigned long long) * kCounters);
+  int rc = launch_propagate(c, in, seed, max_steps, nullptr, nullptr, params, nullptr, d);
+  unsigned long long h[kCounters] = {0};
+  cudaError_t e = cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (rc != DW_OK) return rc;
+  if (e != cudaSuccess) return dw_fail(c, DW_E_CUDA, "dw_propagate_counters: %s", cudaGetErrorString(e));
+  for (int i = 0; i < n_out; ++i) host_out[i] = i < kCounters ? h[i] : 0;
   return DW_OK;
 }
 

@@ -308,7 +308,7 @@ def test_c4_s2_spot_sweep(rho):
         tt = np.concatenate(times)
         assert np.array_equal(h["time_hist"], fp32_time_hist(tt, 0.0, 1.0, 2000))
         assert int(h["time_hist"][-1]) == int((tt >= np.float32(1999.0)).sum())
-        pu.assert_channels_agree(h["time_hist"], n_gpu, ref["time_hist"], n_orc, "C4 arrival-time histogram, bin by bin")
+        pu.assert_time_hist_agrees(h["time_hist"], n_gpu, ref["time_hist"], n_orc, "C4 arrival-time histogram, bin by bin")
     finally:
         c3 = synth.config(3)
         ctx.set_surfaces(c3.optics.detect, c3.optics.reflect_diffuse, c3.optics.reflect_specular, c3.optics.transmit)
@@ -340,7 +340,7 @@ def test_histograms_are_counts_of_the_launch_outputs(cfg, n):
         assert want[0] > 0 and want[-1] > 0 or nb == 2000
         assert np.array_equal(r["chan_count"], np.bincount(r["channel"][det], minlength=ctx.n_chan).astype(np.uint64))
         ref = o.propagate(ph.slice(0, n_orc), conf.seed + 7, conf.max_steps, n_bins=nb, t_min=t_min, dt=dt, full=False)
-        pu.assert_channels_agree(r["time_hist"], n, ref["time_hist"], n_orc, f"C{cfg} arrival-time histogram ({nb} bins of {dt} ns)")
+        pu.assert_time_hist_agrees(r["time_hist"], n, ref["time_hist"], n_orc, f"C{cfg} arrival-time histogram ({nb} bins of {dt} ns)")
 
 
 # ------------------------------------------------------------------------------------------- invariants
