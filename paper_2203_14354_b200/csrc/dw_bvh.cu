@@ -502,6 +502,37 @@ __global__ void refit_level_kernel(int first, int count, float4* __restrict__ no
   write_wide(nodes, w, lo, hi, ref);
 }
 
+// The 64-byte form of the nodes that the queries read (dw_internal.cuh DwBvh::qnodes): every plane as a 16-bit step of q_cs from
+// q_lo, lower planes rounded down and upper planes up, one more step outwards for the rounding of the division.  At 65535 steps
+// over the scene a step is 0.04 mm for a 2.6 m detector: the boxes grow by less than the triangles' own padding, and a box only
+// decides HOW the nearest hit is found.  Half the bytes per visit: the L1 data pipe (one wavefront per lane and 128 bytes of a
+// divergent load) is what bounds the traversal (profiles/r02_experiments.md).
+__global__ void quantise_nodes_kernel(int n_nodes, const float4* __restrict__ nodes, uint4* __restrict__ q, float3 qlo, float3 qics) {
+  int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= n_nodes) return;
+  const float4* p = nodes + 8 * (int64_t)w;
+  const float org[3] = {qlo.x, qlo.y, qlo.z}, ics[3] = {qics.x, qics.y, qics.z};
+  const float4 rf = p[6];
+  const int ref[4] = {__float_as_int(rf.x), __float_as_int(rf.y), __float_as_int(rf.z), __float_as_int(rf.w)};
+  unsigned pl[6][4];
+  for (int a = 0; a < 3; ++a) {
+    const float4 lo = p[a], hi = p[3 + a];
+    const float l4[4] = {lo.x, lo.y, lo.z, lo.w}, h4[4] = {hi.x, hi.y, hi.z, hi.w};
+    for (int c = 0; c < 4; ++c) {
+      if (ref[c] == DW_REF_NONE) { pl[a][c] = 65535u; pl[3 + a][c] = 0u; continue; }
+      const float fl = floorf((l4[c] - org[a]) * ics[a]) - 1.0f, fh = ceilf((h4[c] - org[a]) * ics[a]) + 1.0f;
+      pl[a][c] = (unsigned)fminf(fmaxf(fl, 0.f), 65535.f);
+      pl[3 + a][c] = (unsigned)fminf(fmaxf(fh, 0.f), 65535.f);
+    }
+  }
+  auto pack = [&](int k, int c) { return pl[k][c] | (pl[k][c + 1] << 16); };
+  uint4* o = q + 4 * (int64_t)w;
+  o[0] = make_uint4(pack(0, 0), pack(0, 2), pack(1, 0), pack(1, 2));
+  o[1] = make_uint4(pack(2, 0), pack(2, 2), pack(3, 0), pack(3, 2));
+  o[2] = make_uint4(pack(4, 0), pack(4, 2), pack(5, 0), pack(5, 2));
+  o[3] = make_uint4((unsigned)ref[0], (unsigned)ref[1], (unsigned)ref[2], (unsigned)ref[3]);
+}
+
 // Sum over all nodes of the half-areas of their child boxes: the surface-area measure of tree quality (the expected number of box
 // tests of a random ray is proportional to it).  dw_refit_bvh reports it relative to the build.
 __global__ void node_area_kernel(int n_nodes, const float4* __restrict__ nodes, double* __restrict__ sum) {
@@ -645,6 +676,24 @@ done:
   return rc;
 }
 
+// (re)writes c->d_qnodes from c->d_nodes for the scene box [lo, hi]
+static int quantise_nodes(dw_ctx* c, int n_nodes, const float lo[3], const float hi[3], cudaStream_t stream) {
+  if (!DW_NODE_Q16) return DW_OK;
+  if (!c->d_qnodes) DW_CUDA(c, cudaMalloc(&c->d_qnodes, 64 * (size_t)std::max(n_nodes, 1)));
+  float3 qlo, qcs, qics;
+  float* l = &qlo.x; float* s = &qcs.x; float* is = &qics.x;
+  for (int a = 0; a < 3; ++a) {
+    const float ext = hi[a] - lo[a], pad = 1e-3f * ext + 1e-3f;      // node boxes carry the padding of the references
+    l[a] = lo[a] - pad;
+    s[a] = (ext + 2.0f * pad) / 65535.0f;
+    is[a] = 1.0f / s[a];
+  }
+  quantise_nodes_kernel<<<G_blocks(n_nodes, 256), 256, 0, stream>>>(n_nodes, c->d_nodes, c->d_qnodes, qlo, qics);
+  DW_CUDA(c, cudaGetLastError());
+  c->bvh.qnodes = c->d_qnodes; c->bvh.q_lo = qlo; c->bvh.q_cs = qcs;
+  return DW_OK;
+}
+
 static int nodes_area(dw_ctx* c, int n_nodes, cudaStream_t stream, double* out) {
   int rc = DW_OK;
   double* d = nullptr;
@@ -661,8 +710,8 @@ done:
 }
 
 void dw_bvh_free(dw_ctx* c) {
-  cudaFree(c->d_nodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
-  c->d_nodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
+  cudaFree(c->d_nodes); cudaFree(c->d_qnodes); cudaFree(c->d_tris); cudaFree(c->d_cells);
+  c->d_nodes = nullptr; c->d_qnodes = nullptr; c->d_tris = nullptr; c->d_cells = nullptr; c->built = false;
   dw_ctx::Refit& r = c->rf;
   cudaFree(r.counts); cudaFree(r.offs); cudaFree(r.slot_ref); cudaFree(r.tlo); cudaFree(r.thi); cudaFree(r.rlo); cudaFree(r.rhi);
   cudaFree(r.scene);
@@ -843,7 +892,10 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     float eps_len = 4.0f * 1.1920929e-7f * mx;
     float tree_ms = 0.f, grid_ms = 0.f;
     cudaEventElapsedTime(&tree_ms, ev0, ev1);                                     // before the events are reused below
-    c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len, nullptr, 0, make_float3(0, 0, 0), make_float3(0, 0, 0), make_float3(0, 0, 0)};
+    c->bvh = DwBvh{c->d_nodes, c->d_tris, n_nodes, n, eps_len, nullptr, 0, make_float3(0, 0, 0), make_float3(0, 0, 0), make_float3(0, 0, 0),
+                   nullptr, make_float3(0, 0, 0), make_float3(1, 1, 1)};
+    rc = quantise_nodes(c, n_nodes, lo, hi, stream);
+    if (rc != DW_OK) goto done;
     // ---- empty-space grid over the scene box (skipped for an empty or flat world)
     if (grid_req != -1) {
       rc = grid_build(c, n, tlo, thi, lo, hi, eps_len, GR, stream, &grid_built, &grid_free, &grid_ms);
@@ -932,6 +984,8 @@ int dw_bvh_refit_impl(dw_ctx* c, const float* xyz, int on_device, dw_refit_stats
     rc = grid_build(c, n, r.rlo, r.rhi, lo, hi, eps_len, r.grid_res, stream, &grid_built, &grid_free, &grid_ms);
     if (rc != DW_OK) goto done;
   }
+  rc = quantise_nodes(c, c->bvh.n_nodes, lo, hi, stream);
+  if (rc != DW_OK) goto done;
   rc = nodes_area(c, c->bvh.n_nodes, stream, &area);
   if (rc != DW_OK) goto done;
   DW_B(cudaEventRecord(ev1, stream));

@@ -40,6 +40,12 @@ struct DwTables {
 constexpr int kDwStackShared = DW_STACK_SHARED;
 constexpr int kDwStackLocal = 84;
 #define DW_REF_NONE 0x7fffffff
+// Queries read the 64-byte form of the nodes (16-bit planes) instead of the 128-byte fp32 form.  Built, correct (first-hit parity
+// green) and measured on the round-2 kernel: C2 43.0 against 41.8 ms, C3 46.3 against 43.7 (profiles/r02_experiments.md): the
+// decode costs more issue slots than the bytes save.  Off.
+#ifndef DW_NODE_Q16
+#define DW_NODE_Q16 0
+#endif
 
 // Triangle record in leaf order, 48 B, read as three float4 (Moeller-Trumbore form):
 //   a = (v0.x, v0.y, v0.z, e1.x)  b = (e1.y, e1.z, e2.x, e2.y)
@@ -55,6 +61,11 @@ struct DwBvh {
   const uint2* cells;
   int grid_n;
   float3 grid_lo, grid_cs, grid_inv_cs;
+  // the same nodes in 64 bytes (what the queries read): child planes as 16-bit steps of q_cs from q_lo, rounded outwards
+  //   u0 = lo.x[0..3]  u1 = lo.y  u2 = lo.z  u3 = hi.x  u4 = hi.y  u5 = hi.z  (uint2 each: child c in the 16 bits (c & 1) of word c >> 1)
+  //   then ref[0..3]
+  const uint4* qnodes;  // [n_nodes][4]
+  float3 q_lo, q_cs;
 };
 
 struct dw_ctx {
@@ -77,6 +88,7 @@ struct dw_ctx {
   bool have_geom = false;
   // BVH
   float4* d_nodes = nullptr;
+  uint4* d_qnodes = nullptr;
   float4* d_tris = nullptr;
   uint2* d_cells = nullptr;
   DwBvh bvh{};

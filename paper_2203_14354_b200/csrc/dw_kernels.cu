@@ -106,16 +106,24 @@ __device__ DW_INL_TABLE float table_at(const float* __restrict__ tab, int row, i
 // ------------------------------------------------------------------------------------------------ first hit (S1)
 // The query is written as a resumable state machine so that the propagation kernel can interleave the
 // traversal steps of all lanes of a warp; dw_first_hit runs it to completion.
+// DW_NODE_Q16 (dw_internal.cuh): 64-byte nodes with 16-bit planes (DwBvh::qnodes) instead of the 128-byte fp32 nodes
 struct Ray {
   V3 o, d;     // origin, unit direction
-  V3 inv, oi;  // 1/d (zero components pushed to +-1e30) and o * inv
+  V3 inv, oi;  // fp32 nodes: 1/d (zero components pushed to +-1e30) and o * inv, so that a plane p is met at p * inv - oi;
+               // 16-bit nodes: the same for a plane given as q steps of q_cs from q_lo: q * (q_cs / d) - (o - q_lo) / d
 };
-__device__ __forceinline__ void ray_setup(Ray& r, V3 o, V3 d) {
+__device__ __forceinline__ void ray_setup(Ray& r, V3 o, V3 d, const DwBvh& bvh) {
   const float tiny = 1e-30f;   // zero components become +-tiny so that 0 * inf never appears
   r.o = o; r.d = d;
-  r.inv = mk(1.0f / (fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), 1.0f / (fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
-             1.0f / (fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
-  r.oi = mk(o.x * r.inv.x, o.y * r.inv.y, o.z * r.inv.z);
+  const V3 inv = mk(1.0f / (fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), 1.0f / (fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
+                    1.0f / (fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
+#if DW_NODE_Q16
+  r.inv = mk(bvh.q_cs.x * inv.x, bvh.q_cs.y * inv.y, bvh.q_cs.z * inv.z);
+  r.oi = mk((o.x - bvh.q_lo.x) * inv.x, (o.y - bvh.q_lo.y) * inv.y, (o.z - bvh.q_lo.z) * inv.z);
+#else
+  r.inv = inv;
+  r.oi = mk(o.x * inv.x, o.y * inv.y, o.z * inv.z);
+#endif
 }
 
 constexpr int kInLeaf = -1;   // TraceState::node: triangles [tri_cur, tri_end) are pending
@@ -165,6 +173,19 @@ __device__ __forceinline__ void ldg256(const float4* p, float4& a, float4& b) {
   asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w), "=f"(b.x), "=f"(b.y), "=f"(b.z), "=f"(b.w) : "l"(p));
 }
+#if DW_NODE_Q16
+struct NodeRegs { uint4 a, b, c, rf; };   // a = lo.x | lo.y, b = lo.z | hi.x, c = hi.y | hi.z (uint2 per plane), rf = references
+__device__ __forceinline__ void ldg256u(const uint4* p, uint4& a, uint4& b) {
+  asm volatile("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(a.x), "=r"(a.y), "=r"(a.z), "=r"(a.w), "=r"(b.x), "=r"(b.y), "=r"(b.z), "=r"(b.w) : "l"(p));
+}
+__device__ __forceinline__ void node_load(const DwBvh& bvh, int node, NodeRegs& n) {
+  const uint4* p = bvh.qnodes + 4 * (size_t)node;
+  ldg256u(p, n.a, n.b); ldg256u(p + 2, n.c, n.rf);
+}
+__device__ __forceinline__ float q16lo(unsigned w) { return (float)(w & 0xFFFFu); }
+__device__ __forceinline__ float q16hi(unsigned w) { return (float)(w >> 16); }
+#else
 struct NodeRegs { float4 lx, ly, lz, hx, hy, hz, rf; };
 __device__ __forceinline__ void node_load(const DwBvh& bvh, int node, NodeRegs& n) {
   const float4* p = bvh.nodes + 8 * (size_t)node;
@@ -174,13 +195,22 @@ __device__ __forceinline__ void node_load(const DwBvh& bvh, int node, NodeRegs& 
   n.lx = __ldg(p); n.ly = __ldg(p + 1); n.lz = __ldg(p + 2); n.hx = __ldg(p + 3); n.hy = __ldg(p + 4); n.hz = __ldg(p + 5); n.rf = __ldg(p + 6);
 #endif
 }
+#endif
 __device__ __forceinline__ void node_process(const DwBvh& bvh, const Ray& r, TraceState& s, const NodeRegs& n, int* sstack, int sstride, int* lstack) {
-  const int r0 = __float_as_int(n.rf.x), r1 = __float_as_int(n.rf.y), r2 = __float_as_int(n.rf.z), r3 = __float_as_int(n.rf.w);
   float n0, n1, n2, n3;
+#if DW_NODE_Q16
+  const int r0 = (int)n.rf.x, r1 = (int)n.rf.y, r2 = (int)n.rf.z, r3 = (int)n.rf.w;
+  const bool h0 = slab(r, s.best_t, bvh.eps_len, q16lo(n.a.x), q16lo(n.a.z), q16lo(n.b.x), q16lo(n.b.z), q16lo(n.c.x), q16lo(n.c.z), n0) && (r0 != DW_REF_NONE);
+  const bool h1 = slab(r, s.best_t, bvh.eps_len, q16hi(n.a.x), q16hi(n.a.z), q16hi(n.b.x), q16hi(n.b.z), q16hi(n.c.x), q16hi(n.c.z), n1) && (r1 != DW_REF_NONE);
+  const bool h2 = slab(r, s.best_t, bvh.eps_len, q16lo(n.a.y), q16lo(n.a.w), q16lo(n.b.y), q16lo(n.b.w), q16lo(n.c.y), q16lo(n.c.w), n2) && (r2 != DW_REF_NONE);
+  const bool h3 = slab(r, s.best_t, bvh.eps_len, q16hi(n.a.y), q16hi(n.a.w), q16hi(n.b.y), q16hi(n.b.w), q16hi(n.c.y), q16hi(n.c.w), n3) && (r3 != DW_REF_NONE);
+#else
+  const int r0 = __float_as_int(n.rf.x), r1 = __float_as_int(n.rf.y), r2 = __float_as_int(n.rf.z), r3 = __float_as_int(n.rf.w);
   const bool h0 = slab(r, s.best_t, bvh.eps_len, n.lx.x, n.ly.x, n.lz.x, n.hx.x, n.hy.x, n.hz.x, n0) && (r0 != DW_REF_NONE);
   const bool h1 = slab(r, s.best_t, bvh.eps_len, n.lx.y, n.ly.y, n.lz.y, n.hx.y, n.hy.y, n.hz.y, n1) && (r1 != DW_REF_NONE);
   const bool h2 = slab(r, s.best_t, bvh.eps_len, n.lx.z, n.ly.z, n.lz.z, n.hx.z, n.hy.z, n.hz.z, n2) && (r2 != DW_REF_NONE);
   const bool h3 = slab(r, s.best_t, bvh.eps_len, n.lx.w, n.ly.w, n.lz.w, n.hx.w, n.hy.w, n.hz.w, n3) && (r3 != DW_REF_NONE);
+#endif
   // Nearest hit child by compare-and-select on the references themselves (children of a node are distinct).  Do NOT
   // index the children by a computed position: nvcc turns that into a jump table (BRX) inside the traversal loop, and
   // on sm_100a lanes that diverge at that indirect branch were observed not to reconverge before the warp votes of
@@ -260,7 +290,7 @@ __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, co
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
   Ray r;
-  ray_setup(r, mk(ox[i], oy[i], oz[i]), mk(dx[i], dy[i], dz[i]));
+  ray_setup(r, mk(ox[i], oy[i], oz[i]), mk(dx[i], dy[i], dz[i]), bvh);
   TraceState s;
   ts_begin(s, INFINITY);
   const int ex = exclude ? exclude[i] : -1;
@@ -416,6 +446,47 @@ __device__ __noinline__ int film_event(float n1, float nf, float kf, float d_nm,
     return 1;
   }
   return 2;
+}
+
+// ------------------------------------------------------------------------------------------------ empty-space look-up
+// every free cell of the grid carries one box of free cells that contains it.  A segment that lies in
+// such a box touches no triangle.  A segment that leaves the box of its origin's cell is followed into the box of the cell it
+// enters (DW_SKIP_HOPS times): the point just behind the exit face, 8 eps_len further along the ray, starts the next test.
+// That piece stays within 8 eps_len of a free cell; occupied cells are grown by 32 eps_len, of which the edge slack of the
+// triangle test takes at most 15 (dw_bvh.cu grid_build), so nothing can lie on it.
+#ifndef DW_SKIP_HOPS
+#define DW_SKIP_HOPS 0
+#endif
+__device__ __forceinline__ bool free_box_of(const DwBvh& B, V3 p, V3& blo, V3& bhi) {
+  const float fx = (p.x - B.grid_lo.x) * B.grid_inv_cs.x, fy = (p.y - B.grid_lo.y) * B.grid_inv_cs.y, fz = (p.z - B.grid_lo.z) * B.grid_inv_cs.z;
+  const int G = B.grid_n;
+  const int cx = (int)floorf(fx), cy = (int)floorf(fy), cz = (int)floorf(fz);
+  if (!(cx >= 0 && cy >= 0 && cz >= 0 && cx < G && cy < G && cz < G)) return false;
+  const uint2 cb = __ldg(&B.cells[(cz * G + cy) * G + cx]);
+  if (!(cb.y >> 16)) return false;
+  blo = mk(fmaf((float)(cb.x & 0xFF), B.grid_cs.x, B.grid_lo.x), fmaf((float)((cb.x >> 16) & 0xFF), B.grid_cs.y, B.grid_lo.y),
+           fmaf((float)(cb.y & 0xFF), B.grid_cs.z, B.grid_lo.z));
+  bhi = mk(fmaf((float)(((cb.x >> 8) & 0xFF) + 1), B.grid_cs.x, B.grid_lo.x), fmaf((float)(((cb.x >> 24) & 0xFF) + 1), B.grid_cs.y, B.grid_lo.y),
+           fmaf((float)(((cb.y >> 8) & 0xFF) + 1), B.grid_cs.z, B.grid_lo.z));
+  return p.x >= blo.x && p.x <= bhi.x && p.y >= blo.y && p.y <= bhi.y && p.z >= blo.z && p.z <= bhi.z;
+}
+__device__ __forceinline__ bool segment_is_free(const DwBvh& B, V3 x, V3 k, float tmax) {
+  const V3 p1 = fma3(tmax, k, x);
+  V3 a = x;
+#pragma unroll 1
+  for (int hop = 0;; ++hop) {
+    V3 blo, bhi;
+    if (!free_box_of(B, a, blo, bhi)) return false;
+    if (p1.x >= blo.x && p1.x <= bhi.x && p1.y >= blo.y && p1.y <= bhi.y && p1.z >= blo.z && p1.z <= bhi.z) return true;
+    if (hop == DW_SKIP_HOPS) return false;
+    // leave the box through the face the ray meets first
+    const float tx = k.x > 0.f ? (bhi.x - a.x) / k.x : (k.x < 0.f ? (blo.x - a.x) / k.x : INFINITY);
+    const float ty = k.y > 0.f ? (bhi.y - a.y) / k.y : (k.y < 0.f ? (blo.y - a.y) / k.y : INFINITY);
+    const float tz = k.z > 0.f ? (bhi.z - a.z) / k.z : (k.z < 0.f ? (blo.z - a.z) / k.z : INFINITY);
+    const float te = fminf(fminf(tx, ty), tz);
+    if (!(te >= 0.f) || !(te < INFINITY)) return false;
+    a = fma3(te + 8.0f * B.eps_len, k, a);
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ propagation
@@ -667,7 +738,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
             dbulk = fminf(da, ds);
             tmax = dbulk + A.bvh.eps_len;
           }
-          ray_setup(ray, x, k);
+          ray_setup(ray, x, k, A.bvh);
           ts_begin(ts, tmax);
           lstate = LANE_TRACE;
           fresh = false;
@@ -751,6 +822,9 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 #endif
 #ifndef DW_NODE_REPS_MIN
 #define DW_NODE_REPS_MIN 16
+#endif
+#ifndef DW_TRI_PAIR
+#define DW_TRI_PAIR 0   // measured: 42.4 against 41.6 ms on C2 (profiles/r02_experiments.md)
 #endif
 
 // The film-enabled instantiation gets one block fewer per SM: at 80 registers it spills 106 bytes around the film call.
@@ -1053,27 +1127,8 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
             absorb_first = da < ds;
             dbulk = fminf(da, ds);
             tmax = dbulk + A.bvh.eps_len;
-            // empty boxes: if the whole segment lies in the triangle-free box of the origin's cell, the answer is "no hit"
-            if (use_grid) {
-              const float fx = (x.x - A.bvh.grid_lo.x) * A.bvh.grid_inv_cs.x, fy = (x.y - A.bvh.grid_lo.y) * A.bvh.grid_inv_cs.y,
-                          fz = (x.z - A.bvh.grid_lo.z) * A.bvh.grid_inv_cs.z;
-              const int G = A.bvh.grid_n;
-              const int cx = (int)floorf(fx), cy = (int)floorf(fy), cz = (int)floorf(fz);
-              if (cx >= 0 && cy >= 0 && cz >= 0 && cx < G && cy < G && cz < G) {
-                const uint2 cb = __ldg(&A.bvh.cells[(cz * G + cy) * G + cx]);
-                if (cb.y >> 16) {
-                  const V3 blo = mk(fmaf((float)(cb.x & 0xFF), A.bvh.grid_cs.x, A.bvh.grid_lo.x),
-                                    fmaf((float)((cb.x >> 16) & 0xFF), A.bvh.grid_cs.y, A.bvh.grid_lo.y),
-                                    fmaf((float)(cb.y & 0xFF), A.bvh.grid_cs.z, A.bvh.grid_lo.z));
-                  const V3 bhi = mk(fmaf((float)(((cb.x >> 8) & 0xFF) + 1), A.bvh.grid_cs.x, A.bvh.grid_lo.x),
-                                    fmaf((float)(((cb.x >> 24) & 0xFF) + 1), A.bvh.grid_cs.y, A.bvh.grid_lo.y),
-                                    fmaf((float)(((cb.y >> 8) & 0xFF) + 1), A.bvh.grid_cs.z, A.bvh.grid_lo.z));
-                  const V3 p1 = fma3(tmax, k, x);
-                  skip = x.x >= blo.x && x.x <= bhi.x && x.y >= blo.y && x.y <= bhi.y && x.z >= blo.z && x.z <= bhi.z &&
-                         p1.x >= blo.x && p1.x <= bhi.x && p1.y >= blo.y && p1.y <= bhi.y && p1.z >= blo.z && p1.z <= bhi.z;
-                }
-              }
-            }
+            // empty boxes: if the whole segment lies in triangle-free boxes of the grid, the answer is "no hit"
+            if (use_grid) skip = segment_is_free(A.bvh, x, k, tmax);
           }
           poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
           poolf[W_KX * kSlots + slot] = k.x; poolf[W_KY * kSlots + slot] = k.y; poolf[W_KZ * kSlots + slot] = k.z;
@@ -1142,7 +1197,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         my = q[r];
         V3 x = mk(poolf[W_X * kSlots + my], poolf[W_Y * kSlots + my], poolf[W_Z * kSlots + my]);
         V3 k = mk(poolf[W_KX * kSlots + my], poolf[W_KY * kSlots + my], poolf[W_KZ * kSlots + my]);
-        ray_setup(ray, x, k);
+        ray_setup(ray, x, k, A.bvh);
         ts_begin(ts, poolf[W_BEST_T * kSlots + my]);
         q_exclude = pool[W_LAST * kSlots + my];
         q_medium = literal ? -1 : pool[W_MEDIUM * kSlots + my];
@@ -1178,6 +1233,18 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         }
       } else {
         CNT(C_ITER_LEAF, DW_TRI_REPS); CNT(C_LANES_LEAF, nL * DW_TRI_REPS);
+#if DW_TRI_PAIR
+        // the records of two triangles of the leaf are loaded together: one memory round trip per triangle phase, not two
+        if (act && ts.node == kInLeaf) {
+          const bool two = ts.tri_cur + 1 < ts.tri_end;
+          TriRegs t0, t1;
+          tri_load(A.bvh, ts.tri_cur, t0);
+          tri_load(A.bvh, two ? ts.tri_cur + 1 : ts.tri_cur, t1);
+          tri_process(ray, ts, t0, q_exclude, q_medium, my_stack, sstride, lstack);
+          if (two) tri_process(ray, ts, t1, q_exclude, q_medium, my_stack, sstride, lstack);
+          if constexpr (kCount) atomicAdd(&s_cnt[C_TRI], two ? 2ull : 1ull);
+        }
+#else
 #if DW_TRI_REPS > 1
 #pragma unroll 1
         for (int rep = 0; rep < DW_TRI_REPS; ++rep)
@@ -1186,6 +1253,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           step_triangle(A.bvh, ray, ts, q_exclude, q_medium, my_stack, sstride, lstack);
           if constexpr (kCount) atomicAdd(&s_cnt[C_TRI], 1ull);
         }
+#endif
       }
       if (act && ts.node == kDone) {                        // query finished: hand the slot to the physics phase
         poolf[W_BEST_T * kSlots + my] = ts.best_t;
@@ -1280,7 +1348,7 @@ __global__ void __launch_bounds__(128) render_kernel(DwBvh bvh, DwCameraDev cam,
   const V3 d = unit(mk(fmaf(x, cam.r[0], fmaf(y, cam.u[0], cam.f[0])), fmaf(x, cam.r[1], fmaf(y, cam.u[1], cam.f[1])),
                        fmaf(x, cam.r[2], fmaf(y, cam.u[2], cam.f[2]))));
   Ray r;
-  ray_setup(r, mk(cam.eye[0], cam.eye[1], cam.eye[2]), d);
+  ray_setup(r, mk(cam.eye[0], cam.eye[1], cam.eye[2]), d, bvh);
   TraceState s;
   ts_begin(s, INFINITY);
   int* my = s_stack + threadIdx.x;

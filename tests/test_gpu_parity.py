@@ -81,6 +81,9 @@ def test_philox_bit_exact_against_oracle():
 
 
 # ------------------------------------------------------------------------------------------- first hit
+FIRST_HIT_PLAIN = {}
+
+
 def check_first_hit(i, n, use_brute):
     c, ctx = ctx_for(i)
     o = oracle_for(i)
@@ -107,6 +110,13 @@ def check_first_hit(i, n, use_brute):
         # and on all but the grazing 1% the plain criterion holds
         assert np.quantile(err / (1e-5 * do[hit] + eps), 0.99) <= 1.0
         assert np.all(np.isinf(dg[same & (to < 0)]))
+        # the number BASELINE.json states, literally: |dd| / d <= 1e-5 with nothing added.  Recorded (BASELINE.md quotes it per
+        # config) and held to a floor: what misses it is the fp32 resolution of the coordinates (eps), which R-dist allows for
+        plain = float((err <= 1e-5 * do[hit]).mean())
+        FIRST_HIT_PLAIN[label] = plain
+        print(f"first-hit {label}: ids identical {same.mean():.6f}, plain |dd|/d <= 1e-5 on {plain:.6f} of {int(hit.sum())} matched rays, "
+              f"median |dd|/d {np.median(err / do[hit]):.2e}")
+        assert plain >= 0.995, f"{label}: plain 1e-5 relative distance criterion on only {plain:.5f}"
         return to, do
 
     # set A: the config's photons as rays
@@ -274,7 +284,7 @@ def test_c3_statistical_parity_full_size():
     check_statistical_parity(3, 10_000_000, 1_000_000)
 
 
-@pytest.mark.parametrize("rho", [0.90, 0.99])
+@pytest.mark.parametrize("rho", [0.90, 0.95, 0.99])
 def test_c4_s2_spot_sweep(rho):
     """C4: S2-like spot in the gas gap, batches with photon_id_base, PTFE reflectivity swapped without a
     BVH rebuild; per-PMT hit map and arrival-time histogram against the oracle."""
@@ -341,6 +351,56 @@ def test_histograms_are_counts_of_the_launch_outputs(cfg, n):
         assert np.array_equal(r["chan_count"], np.bincount(r["channel"][det], minlength=ctx.n_chan).astype(np.uint64))
         ref = o.propagate(ph.slice(0, n_orc), conf.seed + 7, conf.max_steps, n_bins=nb, t_min=t_min, dt=dt, full=False)
         pu.assert_time_hist_agrees(r["time_hist"], n, ref["time_hist"], n_orc, f"C{cfg} arrival-time histogram ({nb} bins of {dt} ns)")
+
+
+def test_c4_full_size_as_baseline_json_states_it():
+    """BASELINE.json configs[4] as written: 1e8 photons in batches of 1e7 (photon_id_base = b * 1e7) from the S2 spot, repeated for
+    PTFE reflectivity 0.90 / 0.95 / 0.99 with only dw_set_surfaces between them (no BVH rebuild), per-PMT hit map and arrival-time
+    histogram; against an oracle run of 1e6 photons per reflectivity: per-PMT 4 sigma, LCE 0.2 % absolute, arrival times KS
+    p > 0.01, escapes <= 1e-6 N (G3).  Prints the wall time of the sweep."""
+    import time
+    _, ctx = ctx_for(3)
+    n_batch, n_b, n_orc = 10_000_000, 10, 1_000_000
+    n_gpu = n_batch * n_b
+    t_sweep = 0.0
+    try:
+        for rho in (0.90, 0.95, 0.99):
+            c4 = synth.config(4, ptfe_reflectivity=rho)
+            t0 = time.perf_counter()
+            ctx.set_surfaces(c4.optics.detect, c4.optics.reflect_diffuse, c4.optics.reflect_specular, c4.optics.transmit)
+            t_sweep += time.perf_counter() - t0
+            hist = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0)
+            out = dw.DeviceResults(n_batch, ("flags", "t"))
+            times = []
+            for b in range(n_b):
+                d_ph = dw.DevicePhotons(c4.make_photons(n_batch, b * n_batch))       # input generation is not part of the sweep time
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                ctx.propagate(d_ph, c4.seed, c4.max_steps, out, hist)
+                torch.cuda.synchronize()
+                t_sweep += time.perf_counter() - t0
+                rr = out.numpy()
+                times.append(rr["t"][rr["fate"] == dw.FATE_DETECTED][::10])                 # every tenth arrival time: 2e6 per reflectivity
+                del d_ph
+            h = hist.numpy()
+            ref = orc.Oracle(c4.geometry, c4.optics, bvh=True).propagate(c4.make_photons(n_orc, 10 ** 10), c4.seed, c4.max_steps,
+                                                                         n_bins=2000, dt=1.0, full=False)
+            fg, fo = pu.fates(h["fate_count"], dw.FATE_NAMES), pu.fates(ref["fate_count"], orc.FATE_NAMES)
+            assert sum(fg.values()) == n_gpu and int(h["chan_count"].sum()) == fg["detected"] == int(h["time_hist"].sum())
+            assert fg["nan_abort"] == 0 and fg["truncated"] == 0
+            assert fg["escaped"] <= int(1e-6 * n_gpu), f"rho {rho}: {fg['escaped']} escapes in {n_gpu}"       # G3
+            d_lce = pu.assert_fraction_agrees(fg["detected"], n_gpu, fo["detected"], n_orc, 0.002, f"C4 rho {rho} LCE")
+            worst, chi2, ndf = pu.assert_channels_agree(h["chan_count"], n_gpu, ref["chan_count"], n_orc, f"C4 rho {rho} per-PMT")
+            pu.assert_time_hist_agrees(h["time_hist"], n_gpu, ref["time_hist"], n_orc, f"C4 rho {rho} arrival-time histogram")
+            p = pu.ks_pvalue(np.concatenate(times).astype(np.float64), ref["t"][ref["fate"] == orc.FATE_DETECTED])
+            assert p > 0.01, f"C4 rho {rho} KS p = {p}"
+            print(f"C4 full size rho {rho}: LCE {fg['detected'] / n_gpu:.5f} (oracle {fo['detected'] / n_orc:.5f}, diff {d_lce:.5f}), escapes "
+                  f"{fg['escaped']} of {n_gpu}, per-PMT max |z| {worst:.2f} chi2/ndf {chi2:.0f}/{ndf}, KS p {p:.3f}, "
+                  f"steps/photon {int(h['total_steps'][0]) / n_gpu:.2f}")
+        print(f"C4 sweep: 3 reflectivities x 10 batches x 1e7 photons propagated in {t_sweep:.2f} s including the table swaps")
+    finally:
+        c3 = synth.config(3)
+        ctx.set_surfaces(c3.optics.detect, c3.optics.reflect_diffuse, c3.optics.reflect_specular, c3.optics.transmit)
 
 
 # ------------------------------------------------------------------------------------------- invariants
