@@ -37,7 +37,7 @@ def algorithmic_work(n_tri):
 
 
 ALG_LANE_INSTR_PER_STEP, ALG_BYTES_PER_STEP = algorithmic_work(113_280)     # C2: 5 levels -> 1055 lane-instr, 592 B
-ALG_STATE_BYTES_PER_PHOTON = 52 + 32
+ALG_STATE_BYTES_PER_PHOTON = 44 + 32          # eleven fp32 words in, eight 4-byte result words out (what dw_propagate is handed)
 SM_COUNT, LANES_PER_SM = 148, 128
 
 
@@ -217,7 +217,11 @@ def main():
     ap.add_argument("--legacy", action="store_true", help="DW_PROP_LEGACY_SCHEDULER (first-generation kernel, diagnostic)")
     ap.add_argument("--th-phys", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
     ap.add_argument("--th-leaf", type=int, default=0, help="phase-scheduling threshold (0 = library default)")
-    ap.add_argument("--counters", action="store_true", help="also run the instrumented instantiation once and print its counters to stderr")
+    ap.add_argument("--sweep", action="store_true", help="with --config 4: also run BASELINE.json configs[4] as written (PTFE reflectivity 0.90 / 0.95 / "
+                    "0.99, 10 batches of 1e7 photons each with photon_id_base = b * 1e7, only dw_set_surfaces between them) and report the wall "
+                    "time of the sweep, the hit map totals and the arrival-time histogram per reflectivity in config.sweep")
+    ap.add_argument("--no-counters", action="store_true", help="skip the run of the counting instantiation (roofline.implementation_counters)")
+    ap.add_argument("--counter-sample", type=int, default=2_000_000, help="photons of the batch that the counting instantiation runs over")
     ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="cap on resident blocks per SM (0 = occupancy limit)")
     args = ap.parse_args()
@@ -349,6 +353,38 @@ def main():
                          achieved_gbs=44.0 * n / (ems * 1e-3) / 1e9, hbm_peak_gbs=peaks0["hbm_gbs"],
                          frac_of_hbm=44.0 * n / (ems * 1e-3) / 1e9 / peaks0["hbm_gbs"])
 
+    sweep_info = None
+    if args.sweep and args.config == 4 and world == 1 and not args.emit:
+        nb = 10
+        batches = [dw.DevicePhotons(c.make_photons(n, b * n), dev) for b in range(nb)]       # 10 x 440 MB resident; generation is not timed
+        sweep_info, t_all = {}, 0.0
+        for rho in (0.90, 0.95, 0.99):
+            o4 = _synth.config(4, ptfe_reflectivity=rho).optics
+            hs = dw.DeviceHists(ctx.n_chan, 2000, 0.0, 1.0, dev)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ctx.set_surfaces(o4.detect, o4.reflect_diffuse, o4.reflect_specular, o4.transmit)    # the only thing that changes: no BVH rebuild
+            for b in range(nb):
+                ctx.propagate(batches[b], c.seed, c.max_steps, out, hs, flags=flags, stream=stream)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            t_all += dt
+            hh = hs.numpy()
+            det = int(hh["fate_count"][0])
+            th = hh["time_hist"].astype(np.int64)
+            cum = np.cumsum(th)
+            nch = ctx.n_chan // 2
+            sweep_info[f"rho_{rho:.2f}"] = dict(seconds=dt, photons=n * nb, photons_per_s=n * nb / dt, detected=det, lce=det / (n * nb),
+                                                hits_bottom_array=int(hh["chan_count"][:nch].sum()), hits_top_array=int(hh["chan_count"][nch:].sum()),
+                                                max_hits_one_pmt=int(hh["chan_count"].max()), escaped=int(hh["fate_count"][3]),
+                                                arrival_hist_peak_bin_ns=int(th.argmax()), arrival_hist_overflow=int(th[-1]),
+                                                bin_holding_90_percent_ns=int(np.searchsorted(cum, 0.9 * cum[-1])),
+                                                steps_per_photon=int(hh["total_steps"][0]) / (n * nb))
+        sweep_info["wall_seconds_3_reflectivities"] = t_all
+        o4 = c.optics
+        ctx.set_surfaces(o4.detect, o4.reflect_diffuse, o4.reflect_specular, o4.transmit)
+        del batches
+
     # ---- end to end through the host-buffer entry (pinned host memory, H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e and not args.emit:
@@ -367,7 +403,8 @@ def main():
         torch.cuda.synchronize()
         dt = dwdist.max_over_ranks(time.perf_counter() - t0)
         e2e = dict(value=n_all * reps / dt, unit=UNIT, h2d_bytes_per_step=int(hp.nbytes), d2h_bytes_per_step=int(hout.nbytes + hh.nbytes),
-                   ms_per_step=1e3 * dt / reps, ms_each=each, api="dw_propagate_host (pinned host buffers, chunked copies overlapped with propagation)")
+                   ms_per_step=1e3 * dt / reps, ms_each=each, api="dw_propagate_host (pinned host buffers, chunked copies overlapped with propagation)",
+                   h2d="11 fp32 arrays (44 B / photon)", d2h="flags, channel, t (12 B / photon) + the four reductions")
 
     if rank != 0:
         dwdist.finalize()
@@ -376,25 +413,72 @@ def main():
     peaks = measured_peaks()
     alg_instr, alg_step_bytes = algorithmic_work(c.geometry.n_tri)
     kernel_ms = float(np.mean(per_step_ms))
+    kernel_s = kernel_ms * 1e-3
     steps_per_launch = local_steps / args.steps
     peak_lane = SM_COUNT * LANES_PER_SM * peaks["sm_max_mhz"] * 1e6          # lane-instructions / s
-    achieved_lane = steps_per_launch * alg_instr / (kernel_ms * 1e-3)
-    alg_bytes = steps_per_launch * alg_step_bytes + n * ALG_STATE_BYTES_PER_PHOTON
-    roofline = dict(bound="alu", achieved=achieved_lane / 1e12, peak=peak_lane / 1e12, unit="Tlane-instr/s",
-                    frac=achieved_lane / peak_lane, traffic=None, kernel="propagate_kernel" if args.legacy else "propagate_pool_kernel", kernel_ms=kernel_ms,
-                    algorithmic_lane_instr_per_photon_step=alg_instr,
-                    algorithmic_bytes_per_launch=alg_bytes,
-                    memory_side=dict(achieved_gbs=alg_bytes / (kernel_ms * 1e-3) / 1e9, hbm_peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
-                    peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)")
-    # the derived ALU peak against what this device issues in register-only streams (dw_probe_peaks: ~0.1 s, outside the timed region)
+    achieved_lane = steps_per_launch * alg_instr / kernel_s
+    tree_bytes = steps_per_launch * alg_step_bytes                              # BVH bytes of the ideal path: L2-resident tree (C0-C2) or L2 + HBM
+    state_bytes = n * ALG_STATE_BYTES_PER_PHOTON                                # photon state in and results out: HBM
+    # the derived ALU peak against what this device issues in register-only streams, and the L2 read bandwidth (dw_probe_peaks:
+    # ~0.1 s, outside the timed region)
+    probe = None
     try:
         pk = ctx.probe_peaks()
-        roofline["issue_probe"] = dict(fma_tlane_instr_s=pk["fma_lane_instr_per_s"] / 1e12, alu_tlane_instr_s=pk["alu_lane_instr_per_s"] / 1e12,
-                                       mix_tlane_instr_s=pk["mix_lane_instr_per_s"] / 1e12, l2_read_gbs=pk["l2_read_bytes_per_s"] / 1e9,
-                                       note="pure FP32 FMA / pure integer ALU / even mix, lane-instructions per second; peak above is the derived "
-                                            "148 x 128 x clock, which the FMA stream reaches to within a few per cent")
+        probe = dict(fma_tlane_instr_s=pk["fma_lane_instr_per_s"] / 1e12, alu_tlane_instr_s=pk["alu_lane_instr_per_s"] / 1e12,
+                     mix_tlane_instr_s=pk["mix_lane_instr_per_s"] / 1e12, l2_read_gbs=pk["l2_read_bytes_per_s"] / 1e9,
+                     note="dw_probe_peaks in this run: pure FP32 FMA / pure integer ALU / even mix in lane-instructions per second, and the read "
+                          "bandwidth of a 32 MiB buffer resident in L2 (the denominator of frac_l2)")
     except Exception as ex:                      # the probe is context, never a reason to lose the line
-        roofline["issue_probe"] = dict(error=str(ex))
+        probe = dict(error=str(ex))
+    l2_gbs = probe.get("l2_read_gbs") if probe else None
+    # T_roof = max(B_L2 / BW_L2, B_HBM / BW_HBM, F / P_FP32); each term as a fraction of the measured time
+    frac_alu = achieved_lane / peak_lane
+    frac_l2 = (tree_bytes / kernel_s / 1e9) / l2_gbs if l2_gbs else None
+    tree_in_l2 = (stats["node_bytes"] + stats["tri_bytes"]) < 100e6
+    hbm_bytes = state_bytes + (0 if tree_in_l2 else tree_bytes)
+    frac_hbm = (hbm_bytes / kernel_s / 1e9) / peaks["hbm_gbs"]
+    terms = dict(alu=frac_alu, l2=frac_l2 or 0.0, hbm=frac_hbm)
+    binding = max(terms, key=terms.get)
+    roofline = dict(bound="alu", achieved=achieved_lane / 1e12, peak=peak_lane / 1e12, unit="Tlane-instr/s",
+                    frac=frac_alu, traffic=None,
+                    frac_alu=frac_alu, frac_l2=frac_l2, frac_hbm=frac_hbm, binding_term=binding, frac_of_t_roof=terms[binding],
+                    frac_note="frac = frac_alu, the conservative (smaller) of the two terms that matter; T_roof of SURVEY.md 8(d) is the max of the "
+                              "three terms, i.e. binding_term / frac_of_t_roof",
+                    kernel="propagate_kernel" if args.legacy else "propagate_pool_kernel", kernel_ms=kernel_ms,
+                    photon_steps_per_launch=steps_per_launch,
+                    algorithmic_lane_instr_per_photon_step=alg_instr, algorithmic_tree_bytes_per_photon_step=alg_step_bytes,
+                    algorithmic_state_bytes_per_photon=ALG_STATE_BYTES_PER_PHOTON,
+                    algorithmic_bytes_per_launch=tree_bytes + state_bytes,
+                    l2_side=dict(achieved_gbs=tree_bytes / kernel_s / 1e9, peak_gbs=l2_gbs, peak_source="dw_probe_peaks, this run",
+                                 tree_bytes=int(stats["node_bytes"] + stats["tri_bytes"]), tree_resident_in_l2=bool(tree_in_l2)),
+                    hbm_side=dict(achieved_gbs=hbm_bytes / kernel_s / 1e9, peak_gbs=peaks["hbm_gbs"], peak_source=peaks["source"]),
+                    peak_derivation=f"{SM_COUNT} SMs x {LANES_PER_SM} FP32 lanes x {peaks['sm_max_mhz']:.0f} MHz ({peaks['source']} max SM clock)",
+                    issue_probe=probe)
+    # what the kernel actually does per photon-step: the counting instantiation, once over a sample, outside the timed region
+    if not args.legacy and not args.literal and not args.no_counters:
+        try:
+            ns = min(n, args.counter_sample)
+            hs = dw.DeviceHists(ctx.n_chan, 0, 0.0, 1.0, dev)
+            ps = dw.DevicePhotons(ph.slice(0, ns), dev)
+            ctx.propagate(ps, c.seed, c.max_steps, None, hs, flags=flags, stream=stream)
+            torch.cuda.synchronize()
+            S = float(hs.numpy()["total_steps"][0])
+            k = ctx.propagate_counters(ps, c.seed, c.max_steps, flags=flags)
+            q = max(k["queries_traced"], 1)
+            roofline["implementation_counters"] = dict(
+                sample_photons=ns, photon_steps=S,
+                node_visits_per_step=k["node_visits"] / S, tri_tests_per_step=k["tri_tests"] / S,
+                node_visits_per_traced_query=k["node_visits"] / q, tri_tests_per_traced_query=k["tri_tests"] / q,
+                queries_traced_per_step=k["queries_traced"] / S, queries_skipped_share=k["queries_skipped"] / max(k["queries_skipped"] + k["queries_traced"], 1),
+                tree_bytes_per_step=(k["node_visits"] * 112 + k["tri_tests"] * 48) / S,
+                lanes_per_node_iteration=k["lanes_node"] / max(k["iters_node"], 1), lanes_per_triangle_iteration=k["lanes_leaf"] / max(k["iters_leaf"], 1),
+                node_iterations_per_step=k["iters_node"] / S, triangle_iterations_per_step=k["iters_leaf"] / S,
+                slots_per_physics_phase=(k["lanes_physics"] + k["lanes_fresh"]) / max(k["physics_phases"], 1),
+                physics_phases_per_step=k["physics_phases"] / S,
+                note="dw_propagate_counters (counting instantiation of the same kernel) over the first sample_photons of the batch; 112 B are "
+                     "read per node visit and 48 B per triangle test; lanes per executed instruction and pipe utilisation need ncu: profiles/")
+        except Exception as ex:
+            roofline["implementation_counters"] = dict(error=str(ex))
     # measured DRAM traffic per launch of the dominant kernel, from the ncu capture named in the file (null if none for this workload)
     traffic_file = ROOT / "profiles" / "traffic.csv"
     if traffic_file.exists() and n == c.n_photons and not args.legacy:
@@ -403,7 +487,7 @@ def main():
             for row in csv.DictReader(traffic_file.open()):
                 if row["config"] == f"C{args.config}":
                     roofline["traffic"] = int(row["dram_bytes_per_launch"])
-                    roofline["traffic_source"] = row["source"]
+                    roofline["traffic_source"] = "NOT measured in this run: " + row["source"]
         except Exception:
             pass
 
@@ -415,7 +499,7 @@ def main():
                 ms_per_step=total_ms / args.steps, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                 data="synthetic",
                 config=dict(workload=c.name, photons_per_step_per_gpu=n, triangles=c.geometry.n_tri, max_steps=c.max_steps,
-                            seed=c.seed, l2="inputs larger than L2 (520 MB photon state in, 320 MB results out per step)",
+                            seed=c.seed, l2="inputs larger than L2 (440 MB photon state in, 320 MB results out per step)",
                             mode="literal" if args.literal else "bounded rays",
                             inputs="dw_emit on the device, a new batch of photon ids every step" if args.emit else "resident batch, same photons every step",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
@@ -423,7 +507,8 @@ def main():
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch(),
                             **({"moved": args.move, "refit": refit_info} if args.move else {}),
                             **({"render": render_info} if render_info else {}),
-                            **({"pipelined": pipelined} if pipelined else {})),
+                            **({"pipelined": pipelined} if pipelined else {}),
+                            **({"sweep": sweep_info} if sweep_info else {})),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
