@@ -33,7 +33,7 @@ struct DwTables {
 // ref >= 0: wide node index; ref < 0: leaf, ~ref = (first_slot << 3) | (count - 1); DW_REF_NONE = empty child.
 // Traversal stack: kDwStackShared entries per thread in shared memory, kDwStackLocal more in local memory; a step
 // pushes at most 3, so trees up to (kDwStackShared + kDwStackLocal) / 3 levels fit (dw_build_bvh checks).
-// 8 and 12 measure the same (profiles/r01_final_c2.md, r01_ldg256_c2.md); 8 lets six lean blocks fit the 164 kB shared-memory configuration.
+// 8 and 12 measure the same (profiles/r01_final_c2.md, r01_captures_9_to_12_c2.md); 8 lets six lean blocks fit the 164 kB shared-memory configuration.
 #ifndef DW_STACK_SHARED
 #define DW_STACK_SHARED 8
 #endif

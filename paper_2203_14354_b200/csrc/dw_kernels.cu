@@ -11,7 +11,7 @@ namespace {
 
 // Node planes read as four 256-bit loads instead of seven 128-bit ones.  Neutral while the kernel was bound by instruction issue (199.1 vs
 // 199.0); once Philox and the votes were cheaper the L1 data pipe (82 % busy, 97 % of its global wavefronts = lanes x node loads) was
-// the limit: C2 227.2 -> 232.8, C3 211.4 -> 220.7 M photons/s (profiles/r01_ldg256_c2.md).
+// the limit: C2 227.2 -> 232.8, C3 211.4 -> 220.7 M photons/s (profiles/r01_captures_9_to_12_c2.md).
 #ifndef DW_NODE_LDG256
 #define DW_NODE_LDG256 1
 #endif
@@ -22,7 +22,7 @@ namespace {
 // became the largest stall once the kernel grew to ~2900 instructions).  Level 0: everything inline; 1: Philox out of line;
 // 2: + table look-up; 3: + Rayleigh / Lambert / Fresnel.
 // Measured on C2 (alternating A/B, two rounds): level 0 173.8, 1 175.2, 2 188.6, 3 151.0 M photons/s.
-// The pool kernel has since stopped calling either helper (flat tables, draw4_keys inlined: profiles/r01_ldg256_c2.md); the legacy
+// The pool kernel has since stopped calling either helper (flat tables, draw4_keys inlined: profiles/r01_captures_9_to_12_c2.md); the legacy
 // kernel and dw_emit still do.
 #ifndef DW_OUTLINE
 #define DW_OUTLINE 2
@@ -799,7 +799,7 @@ constexpr int kSlots = DW_POOL_SLOTS;      // 33..64: lane l looks after slots l
 static_assert(kSlots > 32 && kSlots <= 64, "pool size");
 // The last two words exist only in the full layout: with flat tables and no films the wavelength is never read again and n1 is one
 // table load from the medium, so the lean layout (20 words) leaves them out.  With 8 shared stack entries a lean block takes 26 kB, six of
-// them fit the 164 kB shared-memory configuration instead of 196 kB, and L1 grows from ~60 to ~92 kB (profiles/r01_ldg256_c2.md).
+// them fit the 164 kB shared-memory configuration instead of 196 kB, and L1 grows from ~60 to ~92 kB (profiles/r01_captures_9_to_12_c2.md).
 enum : int { W_X = 0, W_Y, W_Z, W_KX, W_KY, W_KZ, W_EX, W_EY, W_EZ, W_T, W_MEDIUM, W_LAST, W_STEP, W_HIST, W_PI,
              W_DBULK, W_US, W_UF, W_BEST_T, W_BEST_SLOT, kWordsLean, W_LAMBDA = kWordsLean, W_N1, kWordsFull };
 enum : int { S_EMPTY = 0, S_PHYS = 1, S_TRACE = 2, S_BUSY = 3 };
