@@ -236,9 +236,13 @@ typedef struct dw_propagate_params {
   int32_t reserved[3];
 } dw_propagate_params;
 enum {
-  /* Follow the oracle literally: every query is unbounded and the medium comes from the hit triangle (S2).
-   * Default (flag clear): the medium is carried in the photon state after the first query and the sampled
-   * bulk distance bounds the ray; equal in distribution in a closed world. */
+  /* Follow the oracle's loop literally (S1..S4 in its order): every query is unbounded, the medium is read from the side of the hit
+   * triangle (S2), and the bulk lengths compete with the hit distance afterwards.  One concession to fp32: right after a surface
+   * event a triangle whose near side is not the medium the photon was just sent into is not a candidate (the hit point can lie
+   * 1e-4 mm behind a neighbouring facet; in fp64 that hit does not exist).  A hit from the bulk on a side that contradicts the
+   * carried medium is accepted and reported with DW_H_MEDIUM_MISMATCH: the test for an ill-formed mesh.
+   * Default (flag clear): the medium is carried in the photon state after the first query and the sampled bulk distance bounds
+   * the ray; equal in distribution in a closed world. */
   DW_PROP_UNBOUNDED_QUERY = 1u,
   /* Diagnostic: run the first-generation kernel (photon state in registers, one photon per lane, physics and
    * traversal phases chosen per warp) instead of the pool scheduler.  Same results photon by photon. */
@@ -365,6 +369,8 @@ int dw_probe_peaks(dw_ctx* ctx, double out[4]);
  *   [4] physics phases  [5] finished queries evaluated in them  [6] lanes that ran an iteration of the Rayleigh loop
  *   [7] queries set up  [8] photons loaded  [9,10] iterations and active lanes of the box-node phase of the traversal loop
  *   [11,12] the same of its triangle phase  [13] fetches of queued queries  [14] unused  [15] physics phases that ran a Rayleigh iteration
+ *   [16,17] first (unbounded) queries of photons and their node visits  [18,19,20] queries that start on a surface, their node
+ *   visits, those that hit something  [21,22,23] the same for queries that start in the bulk
  * Several times slower than dw_propagate (shared-memory atomics per event); never part of a timed region. */
 enum { DW_N_COUNTERS = 24 };
 int dw_propagate_counters(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,

@@ -24,7 +24,9 @@ PROP_UNBOUNDED_QUERY = 1
 PROP_LEGACY_SCHEDULER = 2
 PROP_NO_EMPTY_SKIP = 4
 COUNTER_NAMES = ("node_visits", "tri_tests", "queries_traced", "queries_skipped", "physics_phases", "lanes_physics", "lanes_rayleigh",
-                 "lanes_setup", "lanes_fresh", "iters_node", "lanes_node", "iters_leaf", "lanes_leaf", "fetches", "lanes_fetch", "rayleigh_iters")
+                 "lanes_setup", "lanes_fresh", "iters_node", "lanes_node", "iters_leaf", "lanes_leaf", "fetches", "lanes_fetch", "rayleigh_iters",
+                 "first_queries", "first_query_visits", "surface_queries", "surface_query_visits", "surface_query_hits",
+                 "bulk_queries", "bulk_query_visits", "bulk_query_hits")
 
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",

@@ -99,6 +99,8 @@ extern "C" int dw_set_materials(dw_ctx* c, int n_mat, int nl, float l0, float dl
   if (!c) return DW_E_ARG;
   if (n_mat < 1 || n_mat > 255 || nl < 1 || !n || !la || !ls || !(dl > 0.f) || !isfinite(l0))
     return dw_fail(c, DW_E_ARG, "dw_set_materials: bad argument (n_mat=%d n_lambda=%d dlambda=%g)", n_mat, nl, dl);
+  if (c->have_geom && n_mat < c->tables.n_mat)        // the packed triangle codes index the table on the device
+    return dw_fail(c, DW_E_RANGE, "dw_set_materials: geometry was validated against %d materials, got %d", c->tables.n_mat, n_mat);
   size_t m = (size_t)n_mat * nl;
   std::vector<float> h(3 * m);
   for (size_t i = 0; i < m; ++i) {

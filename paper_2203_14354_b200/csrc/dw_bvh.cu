@@ -791,6 +791,10 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
       div /= 2;
     }
     split_used = div;
+    if (n < 0 || n >= (1 << 28)) {                              // a leaf reference is (slot << 3) | (count - 1) in 31 bits
+      rc = dw_fail(c, DW_E_RANGE, "dw_build_bvh: %d box references (limit 2^28)", n);
+      goto done;
+    }
     DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * (size_t)n)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * (size_t)n));
     DW_B(cudaMalloc(&ref_tri, 4 * (size_t)n));
     split_emit_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene, div, pad, offs, counts, tlo, thi, ref_tri);

@@ -46,6 +46,13 @@ namespace {
 constexpr float kInvC = 1.0f / 299.792458f;   // ns per mm in vacuum
 constexpr int kStackShared = kDwStackShared;  // per-thread traversal stack entries kept in shared memory
 constexpr int kStackLocal = kDwStackLocal;    // overflow entries (local memory; only unusually deep trees reach it)
+#ifndef DW_SEAM_BACK
+#define DW_SEAM_BACK 1
+#endif
+#ifndef DW_EDGE_REFINE
+#define DW_EDGE_REFINE 1
+#endif
+constexpr int kThruSlack = 0x40000000;
 constexpr float kEdgeSlack = 2e-6f;           // barycentric slack that closes fp32 cracks between triangles
 constexpr float kBoxSlack = 1.0000005f;       // conservative slab test (robust traversal)
 
@@ -133,7 +140,8 @@ struct TraceState {
   int sp;                     // stack depth
   int tri_cur, tri_end;       // pending triangle slots of the current leaf
   float best_t;               // nearest accepted distance so far (starts at t_max)
-  int best_slot, best_id;     // leaf-order slot and caller id of the nearest triangle (-1 / INT_MAX: none)
+  int best_slot, best_id;     // leaf-order slot and caller id of the nearest triangle (-1 / INT_MAX: none); bit 30 of best_id
+                              // (kThruSlack): that triangle was accepted through the edge slack only (ids are < 2^28)
 };
 __device__ __forceinline__ void ts_begin(TraceState& s, float tmax) {
   s.node = 0; s.sp = 0; s.tri_cur = 0; s.tri_end = 0; s.best_t = tmax; s.best_slot = -1; s.best_id = 0x7fffffff;
@@ -237,6 +245,10 @@ __device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, Tr
 // medium >= 0: only triangles whose near side (the side the ray comes from) is `medium` count (DESIGN.md
 // "medium culling"); medium < 0: every triangle counts (the definition S1).  Ties -> lowest caller id.
 struct TriRegs { float4 a, b, c; };
+// out of line: one triangle test in ten thousand asks for it
+__device__ __noinline__ float edge_slack(V3 tv, V3 pv, V3 qv, float idet) {
+  return fminf(1e-5f, 4.0f * 1.1920929e-7f * (sqrtf(dot(tv, tv) * dot(pv, pv)) + sqrtf(dot(qv, qv))) * fabsf(idet));
+}
 __device__ __forceinline__ void ldg128v(const float4* p, float4& a) {   // volatile: the load stays where it is written (issued early)
   asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(a.x), "=f"(a.y), "=f"(a.z), "=f"(a.w) : "l"(p));
 }
@@ -248,7 +260,11 @@ __device__ __forceinline__ void tri_load_early(const DwBvh& bvh, int slot, TriRe
   const float4* p = bvh.tris + 3 * (size_t)slot;
   ldg128v(p, t.a); ldg128v(p + 1, t.b); ldg128v(p + 2, t.c);
 }
-__device__ __forceinline__ void tri_process(const Ray& r, TraceState& s, const TriRegs& T, int exclude, int medium,
+// tback (<= 0): smallest accepted distance.  0 in a plain query.  A photon that has just left a surface (exclude >= 0) and whose
+// medium is known passes -8 eps_len: its fp32 position can lie 1e-4 mm BEHIND a neighbouring facet that it would, exactly, meet
+// at once (the corner between two facets of a closed shell, seen from inside, heading outwards); the medium test below keeps
+// everything else out, the coplanar neighbours included, because it is made with the side the ray comes from (DESIGN.md R-seam).
+__device__ __forceinline__ void tri_process(const Ray& r, TraceState& s, const TriRegs& T, int exclude, int medium, float tback,
                                             const int* sstack, int sstride, const int* lstack) {
   const float4 a = T.a, b = T.b, c = T.c;
   V3 e1 = mk(a.w, b.x, b.y), e2 = mk(b.z, b.w, c.x);
@@ -262,14 +278,30 @@ __device__ __forceinline__ void tri_process(const Ray& r, TraceState& s, const T
     float v = dot(r.d, qv) * idet;
     float t = dot(e2, qv) * idet;
     int id = __float_as_int(c.y);
-    bool ok = (u >= -kEdgeSlack) && (v >= -kEdgeSlack) && (u + v <= 1.0f + kEdgeSlack) && (t > 0.f) &&
-              (t < s.best_t || (t == s.best_t && id < s.best_id)) && (id != exclude);
-    if (ok && medium >= 0) {
-      uint32_t cw = __float_as_uint(c.z);
-      int near_side = (det > 0.f) ? (int)((cw >> 8) & 0xFF) : (int)(cw & 0xFF);   // det > 0: the ray comes from the outer side
-      ok = (near_side == medium);
+    // inside, both edges inclusive (G5), with a slack that closes the fp32 cracks between neighbours: 2e-6 for the usual ray; for a
+    // ray that comes from far away onto a small triangle the rounding of u and v themselves is larger (a 1.1 m ray on a 15 mm facet
+    // missed BOTH neighbours by 3e-6 and 7e-6: profiles/r02_leaks.md), so a near miss is judged again against 4 units of the
+    // rounding error of the two dot products, eps (|tv| |pv| + |qv|) / |det|, at most 1e-5 (a wider band makes the owner of a point
+    // between coplanar slivers a matter of rounding: first-hit ids).
+    const float inside = fminf(fminf(u, v), 1.0f - (u + v));
+    bool in = inside >= -kEdgeSlack;
+    if (DW_EDGE_REFINE && !in && inside > -1e-5f) in = inside >= -edge_slack(tv, pv, qv, idet);
+    if (in && t > tback && id != exclude && t <= fmaf(1e-6f, fabsf(t), s.best_t)) {   // a candidate: the rare part of the test
+      bool ok = t > 0.f;
+      if (medium >= 0) {
+        const uint32_t cw = __float_as_uint(c.z);
+        const int near_side = (det > 0.f) ? (int)((cw >> 8) & 0xFF) : (int)(cw & 0xFF);   // det > 0: the ray comes from the outer side
+        ok = near_side == medium;
+      }
+      if (ok) {
+        const bool thru = inside < 0.f;                      // the point lies outside this triangle by rounding, or by the slack
+        bool closer = t < s.best_t || (t == s.best_t && id < (s.best_id & ~kThruSlack));
+        // two neighbours met at the same distance up to rounding: the one that holds the point wins over the one that nearly
+        // does (with exact arithmetic only the former is hit at all; S1)
+        if (DW_EDGE_REFINE && s.best_slot >= 0 && thru != ((s.best_id & kThruSlack) != 0) && fabsf(t - s.best_t) <= 1e-6f * fabsf(t)) closer = !thru;
+        if (closer) { s.best_t = t; s.best_slot = s.tri_cur; s.best_id = thru ? (id | kThruSlack) : id; }
+      }
     }
-    if (ok) { s.best_t = t; s.best_slot = s.tri_cur; s.best_id = id; }
   }
   if (++s.tri_cur == s.tri_end) ts_goto(s, DW_REF_NONE, sstack, sstride, lstack);
 }
@@ -277,7 +309,7 @@ __device__ __forceinline__ void step_triangle(const DwBvh& bvh, const Ray& r, Tr
                                               const int* sstack, int sstride, const int* lstack) {
   TriRegs T;
   tri_load(bvh, s.tri_cur, T);
-  tri_process(r, s, T, exclude, medium, sstack, sstride, lstack);
+  tri_process(r, s, T, exclude, medium, (DW_SEAM_BACK && exclude >= 0 && medium >= 0) ? -8.0f * bvh.eps_len : 0.f, sstack, sstride, lstack);
 }
 
 __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, const float* __restrict__ ox,
@@ -299,7 +331,7 @@ __global__ void __launch_bounds__(128) first_hit_kernel(DwBvh bvh, int64_t n, co
     if (s.node >= 0) step_internal(bvh, r, s, my, blockDim.x, lstack);
     else step_triangle(bvh, r, s, ex, -1, my, blockDim.x, lstack);
   }
-  tri[i] = s.best_slot >= 0 ? s.best_id : -1;
+  tri[i] = s.best_slot >= 0 ? (s.best_id & ~kThruSlack) : -1;
   dist[i] = s.best_slot >= 0 ? s.best_t : INFINITY;
 }
 
@@ -580,7 +612,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
         if (tracing && ts.node >= 0) step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
       } else {
         if (tracing && ts.node == kInLeaf)
-          step_triangle(A.bvh, ray, ts, last_tri, (!literal) ? medium : -1, my_stack, sstride, lstack);
+          step_triangle(A.bvh, ray, ts, last_tri, (literal && last_tri < 0) ? -1 : medium, my_stack, sstride, lstack);
       }
       if (tracing && ts.node == kDone) { lstate = LANE_PHYS; fresh = false; }
       continue;
@@ -674,7 +706,7 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
           } else {                                                    // S4 third branch, S5
             x = fma3(ts.best_t, k, x);
             t = fmaf(ts.best_t * n1, kInvC, t);
-            last_tri = ts.best_id;
+            last_tri = ts.best_id & ~kThruSlack;
             if (medium != m1) hist |= DW_H_MEDIUM_MISMATCH;
             V3 nh = toward_outer ? mk(-ng.x, -ng.y, -ng.z) : ng;
             uint32_t cw = __float_as_uint(tc.z);
@@ -840,7 +872,8 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 constexpr int kRaylPending = -2;           // W_BEST_SLOT <= kRaylPending: iteration kRaylPending - W_BEST_SLOT of S6 is due
 // diagnostic counters of the kCount instantiation (dw_propagate_counters)
 enum : int { C_NODE = 0, C_TRI, C_TRACED, C_SKIPPED, C_PHASES, C_LANES_PHYS, C_LANES_RAYL, C_LANES_SETUP, C_LANES_FRESH, C_ITER_NODE, C_LANES_NODE,
-             C_ITER_LEAF, C_LANES_LEAF, C_FETCH, C_LANES_FETCH, C_RAYL_ITER, kCounters = 24 };
+             C_ITER_LEAF, C_LANES_LEAF, C_FETCH, C_LANES_FETCH, C_RAYL_ITER,
+             C_Q_FRESH, C_N_FRESH, C_Q_SURF, C_N_SURF, C_H_SURF, C_Q_BULK, C_N_BULK, C_H_BULK, kCounters = 24 };
 
 template <bool kFilm, bool kFlat, bool kCount>
 __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
@@ -895,6 +928,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   TraceState ts;
   ts_begin(ts, 0.f);
   ts.node = kDone;
+  [[maybe_unused]] int my_visits = 0;   // kCount: box-node visits of the running query
 
   for (;;) {
     // ---------------------------------------------------------------- census of the warp's slots
@@ -1200,7 +1234,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         ray_setup(ray, x, k, A.bvh);
         ts_begin(ts, poolf[W_BEST_T * kSlots + my]);
         q_exclude = pool[W_LAST * kSlots + my];
-        q_medium = literal ? -1 : pool[W_MEDIUM * kSlots + my];
+        // literal mode: every triangle counts, except right after a surface event, where a hit whose near side is not the medium the
+        // photon was just sent into is an artefact of the fp32 position (G3)
+        q_medium = (literal && q_exclude < 0) ? -1 : pool[W_MEDIUM * kSlots + my];
         st[my] = S_BUSY;
         if constexpr (kCount) atomicAdd(&s_cnt[C_TRACED], 1ull);
       }
@@ -1229,7 +1265,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
 #endif
         if (act && ts.node >= 0) {
           step_internal(A.bvh, ray, ts, my_stack, sstride, lstack);
-          if constexpr (kCount) atomicAdd(&s_cnt[C_NODE], 1ull);
+          if constexpr (kCount) { atomicAdd(&s_cnt[C_NODE], 1ull); ++my_visits; }
         }
       } else {
         CNT(C_ITER_LEAF, DW_TRI_REPS); CNT(C_LANES_LEAF, nL * DW_TRI_REPS);
@@ -1240,8 +1276,9 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           TriRegs t0, t1;
           tri_load(A.bvh, ts.tri_cur, t0);
           tri_load(A.bvh, two ? ts.tri_cur + 1 : ts.tri_cur, t1);
-          tri_process(ray, ts, t0, q_exclude, q_medium, my_stack, sstride, lstack);
-          if (two) tri_process(ray, ts, t1, q_exclude, q_medium, my_stack, sstride, lstack);
+          const float tback = (q_exclude >= 0 && q_medium >= 0) ? -8.0f * A.bvh.eps_len : 0.f;
+          tri_process(ray, ts, t0, q_exclude, q_medium, tback, my_stack, sstride, lstack);
+          if (two) tri_process(ray, ts, t1, q_exclude, q_medium, tback, my_stack, sstride, lstack);
           if constexpr (kCount) atomicAdd(&s_cnt[C_TRI], two ? 2ull : 1ull);
         }
 #else
@@ -1256,6 +1293,13 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
 #endif
       }
       if (act && ts.node == kDone) {                        // query finished: hand the slot to the physics phase
+        if constexpr (kCount) {                             // by kind of query: first (unbounded), from a surface, from the bulk
+          const int cls = q_medium < 0 ? C_Q_FRESH : (q_exclude >= 0 ? C_Q_SURF : C_Q_BULK);
+          atomicAdd(&s_cnt[cls], 1ull);
+          atomicAdd(&s_cnt[cls + 1], (unsigned long long)my_visits);
+          if (cls != C_Q_FRESH && ts.best_slot >= 0) atomicAdd(&s_cnt[cls + 2], 1ull);
+          my_visits = 0;
+        }
         poolf[W_BEST_T * kSlots + my] = ts.best_t;
         pool[W_BEST_SLOT * kSlots + my] = ts.best_slot;
         st[my] = S_PHYS;
@@ -1358,7 +1402,7 @@ __global__ void __launch_bounds__(128) render_kernel(DwBvh bvh, DwCameraDev cam,
   }
   const int64_t px = (int64_t)j * cam.w + i;
   const bool hit = s.best_slot >= 0;
-  if (tri) tri[px] = hit ? s.best_id : -1;
+  if (tri) tri[px] = hit ? (s.best_id & ~kThruSlack) : -1;
   if (depth) depth[px] = hit ? s.best_t : INFINITY;
   if (shade) {
     float v = 0.f;

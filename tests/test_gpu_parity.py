@@ -609,13 +609,10 @@ def test_integrating_sphere_on_device():
     assert abs(r["steps"].mean() - ref["steps"].mean()) < 4 * math.sqrt(r["steps"].var() / N + ref["steps"].var() / 4e5)
 
 
-@pytest.mark.xfail(strict=True, reason="KNOWN DEFECT (profiles/r01_leaks.md): DW_PROP_UNBOUNDED_QUERY leaks 45 of 2e6 photons "
-                                       "(2.25e-5 N) out of a closed Lambertian sphere, 22x the G3 budget of 1e-6 N: without "
-                                       "medium culling a reflected photon whose fp32 position fell behind the neighbouring "
-                                       "facet hits that facet from outside (H_MEDIUM_MISMATCH) and is reflected outwards")
 def test_literal_mode_leak_budget_on_closed_sphere():
-    """G3 held to the same number in the diagnostic literal mode.  Strict xfail: it fails the suite the day it passes,
-    so that the defect note is removed together with the defect."""
+    """G3 held to the same number in the literal mode.  (Round 1: 45 of 2e6 escaped, because a reflected photon whose fp32 position
+    fell behind the neighbouring facet hit that facet from outside; since round 2 a triangle whose near side contradicts the medium
+    the photon was just sent into is no candidate right after a surface event, include/darwinopt.h DW_PROP_UNBOUNDED_QUERY.)"""
     g, op, f = _random_detector_sphere(0.1, 0.95, subdiv=5)
     ctx = dw.make_context(g, op)
     N = 2_000_000
@@ -623,6 +620,22 @@ def test_literal_mode_leak_budget_on_closed_sphere():
     fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
     assert sum(fc.values()) == N
     assert fc["escaped"] <= max(1, int(1e-6 * N)), f"{fc['escaped']} photons leaked"
+    print(f"literal mode, closed sphere: {fc['escaped']} escapes of {N}")
+
+
+@pytest.mark.parametrize("subdiv,seed", [(5, 77), (6, 31)])
+def test_leak_budget_second_seed_and_finer_sphere(subdiv, seed):
+    """G3 on the closed Lambertian sphere again, on another seed and on 81 920 facets (four times the seams): 1e-6 N in both modes,
+    over 4e6 photons (about 2.8e7 reflections)."""
+    g, op, f = _random_detector_sphere(0.1, 0.95, subdiv=subdiv)
+    ctx = dw.make_context(g, op)
+    N = 4_000_000
+    for flags in (0, dw.PROP_UNBOUNDED_QUERY):
+        r = gpu_run(ctx, synth.photons_point(seed, N), seed, 5000, fields=("flags",), flags=flags)
+        fc = pu.fates(r["fate_count"], dw.FATE_NAMES)
+        assert sum(fc.values()) == N and fc["nan_abort"] == 0 and fc["truncated"] == 0
+        print(f"closed sphere subdiv {subdiv} seed {seed} mode {flags}: {fc['escaped']} escapes of {N}")
+        assert fc["escaped"] <= int(1e-6 * N), f"subdivision {subdiv}, seed {seed}, mode {flags}: {fc['escaped']} photons leaked"
 
 
 @pytest.mark.parametrize("cfg,n,mode", [(1, 300_000, 0), (1, 100_000, dw.PROP_UNBOUNDED_QUERY), (2, 300_000, 0), (0, 100_000, 0)])
