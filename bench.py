@@ -244,6 +244,8 @@ def main():
     geom = c.geometry if (not args.move or args.refit) else _synth.moved(c.geometry, args.move)
     ctx.set_geometry(geom)
     stats = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res, split_div=args.split_div)
+    # the first build of a context also grows its memory pool (one-off); a rebuild of the same geometry is what a sweep of variants pays
+    rebuild_ms = ctx.build_bvh(args.max_leaf, ploc_radius=args.ploc_radius, grid_res=args.grid_res, split_div=args.split_div)["build_ms"]
     refit_info = None
     if args.move and args.refit:
         rs = ctx.refit(_synth.moved(c.geometry, args.move).xyz)
@@ -503,7 +505,7 @@ def main():
                             mode="literal" if args.literal else "bounded rays",
                             inputs="dw_emit on the device, a new batch of photon ids every step" if args.emit else "resident batch, same photons every step",
                             scheduler="legacy" if args.legacy else "pool", bvh_nodes=stats["n_nodes"],
-                            bvh_build_ms=stats["build_ms"], bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
+                            bvh_build_ms=stats["build_ms"], bvh_rebuild_ms=rebuild_ms, bvh_leaves=stats["n_leaves"], bvh_depth=stats["max_depth"], grid_res=stats["grid_res"], bvh_refs=stats["n_refs"], split_div=stats["split_div"],
                             grid_free_cells=stats["grid_free_cells"], empty_skip=not args.no_skip and not args.legacy, launch=ctx.last_launch(),
                             **({"moved": args.move, "refit": refit_info} if args.move else {}),
                             **({"render": render_info} if render_info else {}),

@@ -243,29 +243,115 @@ __global__ void ploc_nn_kernel(int m, int radius, const float4* __restrict__ clo
   nn[i] = bj;
 }
 
-// keep[i] = 0 for the higher position of a mutual pair (it disappears); isnew[i] = 1 for the lower one (a node is made).
-__global__ void ploc_mark_kernel(int m, const int* __restrict__ nn, int* __restrict__ keep, int* __restrict__ isnew) {
+// The rounds run without the host: the number of clusters m and the next node index `base` live on the device, in two copies
+// that the rounds use alternately (st[0..1] for even rounds, st[2..3] for odd ones; st[4] counts the rounds, st[5] is an error
+// flag).  Every kernel of a round is launched over the n positions of the first round and returns where i >= m; the host reads m
+// back once per chunk of rounds.  (Round 1: two CUB scans and an 8-byte read-back per round, 55-70 rounds: the build was latency.)
+// keep = 0 for the higher position of a mutual pair (it disappears); isnew = 1 for the lower one (a node is made).  flag bit 0 keep,
+// bit 1 isnew.  bsum[block] = (kept, new) of the block's positions.
+__global__ void ploc_nn_kernel_dev(const int* __restrict__ st, int radius, const float4* __restrict__ clo, const float4* __restrict__ chi,
+                                   int* __restrict__ nn) {
+  const int m = st[0];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= m) return;
-  int j = nn[i];
-  bool mutual = j >= 0 && nn[j] == i;
-  keep[i] = (mutual && i > j) ? 0 : 1;
-  isnew[i] = (mutual && i < j) ? 1 : 0;
+  if (m <= 1 || i >= m) return;
+  float4 lo = clo[i], hi = chi[i];
+  float best = FLT_MAX;
+  int bj = -1;
+  int j0 = max(i - radius, 0), j1 = min(i + radius, m - 1);
+  for (int j = j0; j <= j1; ++j) {
+    if (j == i) continue;
+    float a = half_area(min4(lo, clo[j]), max4(hi, chi[j]));
+    if (a < best || bj < 0) { best = a; bj = j; }          // strict <: the first (smallest) position wins ties
+  }
+  nn[i] = bj;
 }
-
-__global__ void ploc_apply_kernel(int m, int base, const int* __restrict__ nn, const int* __restrict__ keep,
-                                  const int* __restrict__ isnew, const int* __restrict__ kpos, const int* __restrict__ npos,
-                                  const int* __restrict__ cnode_in, const float4* __restrict__ clo_in,
-                                  const float4* __restrict__ chi_in, int* __restrict__ cnode_out,
-                                  float4* __restrict__ clo_out, float4* __restrict__ chi_out, int* __restrict__ left,
-                                  int* __restrict__ right, int* __restrict__ parent, float4* __restrict__ blo,
-                                  float4* __restrict__ bhi, int* __restrict__ size) {
+__device__ __forceinline__ int2 block_excl_scan2(int2 v, int2* total) {   // exclusive scan of two counters over a 256-thread block
+  __shared__ int2 wsum[8];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int2 inc = v;
+  for (int o = 1; o < 32; o <<= 1) {
+    const int ux = __shfl_up_sync(0xffffffffu, inc.x, o), uy = __shfl_up_sync(0xffffffffu, inc.y, o);
+    if (lane >= o) { inc.x += ux; inc.y += uy; }
+  }
+  if (lane == 31) wsum[w] = inc;
+  __syncthreads();
+  int2 off = make_int2(0, 0), tot = make_int2(0, 0);
+  for (int k = 0; k < 8; ++k) { if (k < w) { off.x += wsum[k].x; off.y += wsum[k].y; } tot.x += wsum[k].x; tot.y += wsum[k].y; }
+  __syncthreads();
+  if (total) *total = tot;
+  return make_int2(off.x + inc.x - v.x, off.y + inc.y - v.y);
+}
+__global__ void __launch_bounds__(256) ploc_mark_kernel_dev(const int* __restrict__ st, const int* __restrict__ nn, unsigned char* __restrict__ flag,
+                                                            int2* __restrict__ bsum) {
+  const int m = st[0];
+  if (m <= 1 || (int)(blockIdx.x * blockDim.x) >= m) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= m || !keep[i]) return;
-  int pos = kpos[i];
-  if (isnew[i]) {
+  int keep = 0, isnew = 0;
+  if (i < m) {
     int j = nn[i];
-    int node = base + npos[i];
+    bool mutual = j >= 0 && nn[j] == i;
+    keep = (mutual && i > j) ? 0 : 1;
+    isnew = (mutual && i < j) ? 1 : 0;
+    flag[i] = (unsigned char)(keep | (isnew << 1));
+  }
+  int2 tot;
+  block_excl_scan2(make_int2(keep, isnew), &tot);
+  if (threadIdx.x == 0) bsum[blockIdx.x] = tot;
+}
+// one block: exclusive scan of the block sums, and the state of the next round
+__global__ void __launch_bounds__(1024) ploc_scan_kernel_dev(const int* __restrict__ st, int* __restrict__ st_next, int* __restrict__ st_common,
+                                                             const int2* __restrict__ bsum, int2* __restrict__ boff) {
+  const int m = st[0], base = st[1];
+  if (m <= 1) { if (threadIdx.x == 0) { st_next[0] = m; st_next[1] = base; } return; }
+  const int nb = (m + 255) / 256;
+  __shared__ int2 wsum[32];
+  __shared__ int2 carry;
+  if (threadIdx.x == 0) carry = make_int2(0, 0);
+  __syncthreads();
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  for (int b0 = 0; b0 < nb; b0 += 1024) {
+    const int b = b0 + threadIdx.x;
+    const int2 v = b < nb ? bsum[b] : make_int2(0, 0);
+    int2 inc = v;
+    for (int o = 1; o < 32; o <<= 1) {
+      const int ux = __shfl_up_sync(0xffffffffu, inc.x, o), uy = __shfl_up_sync(0xffffffffu, inc.y, o);
+      if (lane >= o) { inc.x += ux; inc.y += uy; }
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    int2 off = carry;
+    int2 tot = make_int2(0, 0);
+    for (int k = 0; k < 32; ++k) { if (k < w) { off.x += wsum[k].x; off.y += wsum[k].y; } tot.x += wsum[k].x; tot.y += wsum[k].y; }
+    if (b < nb) boff[b] = make_int2(off.x + inc.x - v.x, off.y + inc.y - v.y);
+    __syncthreads();
+    if (threadIdx.x == 0) { carry.x += tot.x; carry.y += tot.y; }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const int m_new = carry.x;
+    if (m_new >= m || m_new < 1 || m - m_new != carry.y) st_common[1] = 1;      // a round always merges at least one pair
+    st_next[0] = m_new; st_next[1] = base + (m - m_new);
+    st_common[0] += 1;
+  }
+}
+__global__ void __launch_bounds__(256) ploc_apply_kernel_dev(const int* __restrict__ st, const int* __restrict__ nn, const unsigned char* __restrict__ flag,
+                                                             const int2* __restrict__ boff, const int* __restrict__ cnode_in,
+                                                             const float4* __restrict__ clo_in, const float4* __restrict__ chi_in,
+                                                             int* __restrict__ cnode_out, float4* __restrict__ clo_out, float4* __restrict__ chi_out,
+                                                             int* __restrict__ left, int* __restrict__ right, int* __restrict__ parent,
+                                                             float4* __restrict__ blo, float4* __restrict__ bhi, int* __restrict__ size) {
+  const int m = st[0], base = st[1];
+  if (m <= 1 || (int)(blockIdx.x * blockDim.x) >= m) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int f = i < m ? flag[i] : 0;
+  const int keep = f & 1, isnew = (f >> 1) & 1;
+  const int2 loc = block_excl_scan2(make_int2(keep, isnew), nullptr);
+  if (i >= m || !keep) return;
+  const int2 bo = boff[blockIdx.x];
+  const int pos = bo.x + loc.x;
+  if (isnew) {
+    int j = nn[i];
+    int node = base + bo.y + loc.y;
     int a = cnode_in[i], b = cnode_in[j];
     float4 lo = min4(clo_in[i], clo_in[j]), hi = max4(chi_in[i], chi_in[j]);
     left[node] = a; right[node] = b; parent[a] = node; parent[b] = node; parent[node] = -1;
@@ -318,14 +404,17 @@ __device__ __forceinline__ void write_wide(float4* __restrict__ nodes, int w, co
 // One level of the collapse: binary node b (more than max_leaf triangles) becomes wide node w.  Its two children are
 // opened greedily, largest box first, until four remain or none can be opened (a subtree of <= max_leaf triangles is a
 // leaf and stays closed).  Children that are still subtrees get a wide index and a task for the next level.
-__global__ void wide_collapse_kernel(int n_tasks, const WideTask* __restrict__ tasks, WideTask* __restrict__ next,
-                                     int* __restrict__ counters /* [0] next count, [1] wide nodes, [2] leaves */,
+// The level's task count is read from the device (lvl[level]; the children made here are counted in lvl[level + 1]), so that the
+// levels follow each other without the host: it launches one kernel per possible level and reads the counts back once.
+__global__ void wide_collapse_kernel(const int* __restrict__ lvl_in, int* __restrict__ lvl_out, const WideTask* __restrict__ tasks,
+                                     WideTask* __restrict__ next,
+                                     int* __restrict__ counters /* [1] wide nodes, [2] leaves */,
                                      int max_leaf, const int* __restrict__ left, const int* __restrict__ right,
                                      const int* __restrict__ size, const float4* __restrict__ blo,
                                      const float4* __restrict__ bhi, const int* __restrict__ slot,
                                      const int* __restrict__ leftmost, float4* __restrict__ nodes) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= n_tasks) return;
+  const int n_tasks = *lvl_in;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_tasks; i += gridDim.x * blockDim.x) {
   const int b = tasks[i].bnode, w = tasks[i].widx;
   int kid[4];
   int nk = 2;
@@ -356,10 +445,11 @@ __global__ void wide_collapse_kernel(int n_tasks, const WideTask* __restrict__ t
     } else {
       int widx = atomicAdd(&counters[1], 1);
       ref[k] = widx;
-      next[atomicAdd(&counters[0], 1)] = WideTask{c, widx};
+      next[atomicAdd(lvl_out, 1)] = WideTask{c, widx};
     }
   }
   write_wide(nodes, w, lo, hi, ref);
+  }
 }
 
 // A world of <= max_leaf triangles (or none): one wide node whose first child is the only leaf (or nothing).
@@ -622,6 +712,14 @@ __global__ void grid_grow_kernel(int G, const int* __restrict__ occ, const int* 
 
 }  // namespace
 
+// Stream-ordered allocation from the context's pool, which keeps its memory: a build makes about forty buffers, and cudaMalloc /
+// cudaFree (each a device synchronisation) were most of its time.  What a build leaves behind is freed with cudaFree (dw_bvh_free).
+template <class T> static cudaError_t dw_salloc(dw_ctx* c, T** p, size_t bytes, cudaStream_t s) {
+  if (bytes == 0) bytes = 4;
+  return c->pool ? cudaMallocFromPoolAsync((void**)p, bytes, c->pool, s) : cudaMallocAsync((void**)p, bytes, s);
+}
+static void dw_sfree(void* p, cudaStream_t s) { if (p) cudaFreeAsync(p, s); }
+
 static inline unsigned G_blocks(int64_t n, int B) { return (unsigned)((n + B - 1) / B); }
 
 #define DW_B(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) { rc = dw_fail(c, DW_E_CUDA, "%s failed: %s (%s:%d)", \
@@ -650,8 +748,8 @@ static int grid_build(dw_ctx* c, int n, const float* tlo, const float* thi, cons
     const float margin = 32.0f * eps_len;
     const int G3 = GR * GR * GR, P = GR + 1;
     DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
-    DW_B(cudaMalloc(&occ, 4 * (size_t)G3)); DW_B(cudaMalloc(&sat, 4 * (size_t)P * P * P)); DW_B(cudaMalloc(&cnt, 4));
-    if (!c->d_cells) DW_B(cudaMalloc(&c->d_cells, sizeof(uint2) * (size_t)G3));
+    DW_B(dw_salloc(c, &occ, 4 * (size_t)G3, stream)); DW_B(dw_salloc(c, &sat, 4 * (size_t)P * P * P, stream)); DW_B(dw_salloc(c, &cnt, 4, stream));
+    if (!c->d_cells) DW_B(dw_salloc(c, &c->d_cells, sizeof(uint2) * (size_t)G3, stream));
     DW_B(cudaMemsetAsync(occ, 0, 4 * (size_t)G3, stream));
     DW_B(cudaMemsetAsync(sat, 0, 4 * (size_t)P * P * P, stream));
     DW_B(cudaMemsetAsync(cnt, 0, 4, stream));
@@ -670,7 +768,7 @@ static int grid_build(dw_ctx* c, int n, const float* tlo, const float* thi, cons
     c->bvh.cells = c->d_cells; c->bvh.grid_n = GR; c->bvh.grid_lo = glo; c->bvh.grid_cs = cs; c->bvh.grid_inv_cs = ics;
   }
 done:
-  cudaFree(occ); cudaFree(sat); cudaFree(cnt);
+  dw_sfree(occ, stream); dw_sfree(sat, stream); dw_sfree(cnt, stream);
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
   return rc;
@@ -679,7 +777,7 @@ done:
 // (re)writes c->d_qnodes from c->d_nodes for the scene box [lo, hi]
 static int quantise_nodes(dw_ctx* c, int n_nodes, const float lo[3], const float hi[3], cudaStream_t stream) {
   if (!DW_NODE_Q16) return DW_OK;
-  if (!c->d_qnodes) DW_CUDA(c, cudaMalloc(&c->d_qnodes, 64 * (size_t)std::max(n_nodes, 1)));
+  if (!c->d_qnodes) DW_CUDA(c, dw_salloc(c, &c->d_qnodes, 64 * (size_t)std::max(n_nodes, 1), stream));
   float3 qlo, qcs, qics;
   float* l = &qlo.x; float* s = &qcs.x; float* is = &qics.x;
   for (int a = 0; a < 3; ++a) {
@@ -698,14 +796,14 @@ static int nodes_area(dw_ctx* c, int n_nodes, cudaStream_t stream, double* out) 
   int rc = DW_OK;
   double* d = nullptr;
   *out = 0.0;
-  DW_B(cudaMalloc(&d, 8));
+  DW_B(dw_salloc(c, &d, 8, stream));
   DW_B(cudaMemsetAsync(d, 0, 8, stream));
   node_area_kernel<<<G_blocks(n_nodes, 256), 256, 0, stream>>>(n_nodes, c->d_nodes, d);
   DW_B(cudaGetLastError());
   DW_B(cudaMemcpyAsync(out, d, 8, cudaMemcpyDeviceToHost, stream));
   DW_B(cudaStreamSynchronize(stream));
 done:
-  cudaFree(d);
+  dw_sfree(d, stream);
   return rc;
 }
 
@@ -743,8 +841,10 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   unsigned *scene = nullptr, *vals = nullptr, *vals2 = nullptr;
   unsigned long long *keys = nullptr, *keys2 = nullptr;
   int *left = nullptr, *right = nullptr, *parent = nullptr, *size = nullptr, *leftmost = nullptr, *cn[2] = {nullptr, nullptr},
-      *nn = nullptr, *keep = nullptr, *isnew = nullptr, *kpos = nullptr, *npos = nullptr, *slot = nullptr, *misc = nullptr,
-      *occ = nullptr, *sat = nullptr;
+      *nn = nullptr, *slot = nullptr, *misc = nullptr, *occ = nullptr, *sat = nullptr, *pst = nullptr;
+  unsigned char* flag = nullptr;
+  int2 *bsum = nullptr, *boff = nullptr;
+  constexpr int kMaxWideLevels = 48;   // more levels than the traversal stack allows: the depth check below refuses such a tree
   int grid_built = 0, grid_free = 0, split_used = 0;
   WideTask* tasks[2] = {nullptr, nullptr};
   void* tmp = nullptr;
@@ -759,13 +859,13 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
   const unsigned GT = (unsigned)((NT + B - 1) / B);
 
   DW_B(cudaEventCreate(&ev0)); DW_B(cudaEventCreate(&ev1));
-  DW_B(cudaMalloc(&scene, sizeof(unsigned) * 6));
-  DW_B(cudaMalloc(&misc, 16));
+  DW_B(dw_salloc(c, &scene, sizeof(unsigned) * 6, stream));
+  DW_B(dw_salloc(c, &misc, 16, stream));
   DW_B(cudaEventRecord(ev0, stream));
   DW_B(cudaMemsetAsync(misc, 0, 16, stream));
   // ---- stage 0: triangle boxes, scene bounds, references (long triangles split)
-  DW_B(cudaMalloc(&tlo_t, sizeof(float) * 3 * NT)); DW_B(cudaMalloc(&thi_t, sizeof(float) * 3 * NT));
-  DW_B(cudaMalloc(&counts, 4 * NT)); DW_B(cudaMalloc(&offs, 4 * NT));
+  DW_B(dw_salloc(c, &tlo_t, sizeof(float) * 3 * NT, stream)); DW_B(dw_salloc(c, &thi_t, sizeof(float) * 3 * NT, stream));
+  DW_B(dw_salloc(c, &counts, 4 * NT, stream)); DW_B(dw_salloc(c, &offs, 4 * NT, stream));
   if (nt > 0) {
     unsigned init[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
     DW_B(cudaMemcpyAsync(scene, init, sizeof init, cudaMemcpyHostToDevice, stream));
@@ -778,7 +878,7 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     int div = split_req == -1 ? 0 : split_div;
     size_t scan_bytes = 0;
     DW_B(cub::DeviceScan::ExclusiveSum(nullptr, scan_bytes, counts, offs, nt, stream));
-    DW_B(cudaMalloc(&tmp, scan_bytes));
+    DW_B(dw_salloc(c, &tmp, scan_bytes, stream));
     for (;;) {                                                  // coarser splitting if the references would more than double
       split_count_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene, div, counts);
       DW_B(cub::DeviceScan::ExclusiveSum(tmp, scan_bytes, counts, offs, nt, stream));
@@ -795,87 +895,105 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
       rc = dw_fail(c, DW_E_RANGE, "dw_build_bvh: %d box references (limit 2^28)", n);
       goto done;
     }
-    DW_B(cudaMalloc(&tlo, sizeof(float) * 3 * (size_t)n)); DW_B(cudaMalloc(&thi, sizeof(float) * 3 * (size_t)n));
-    DW_B(cudaMalloc(&ref_tri, 4 * (size_t)n));
+    DW_B(dw_salloc(c, &tlo, sizeof(float) * 3 * (size_t)n, stream)); DW_B(dw_salloc(c, &thi, sizeof(float) * 3 * (size_t)n, stream));
+    DW_B(dw_salloc(c, &ref_tri, 4 * (size_t)n, stream));
     split_emit_kernel<<<GT, B, 0, stream>>>(nt, c->d_xyz, c->d_idx, tlo_t, thi_t, scene, div, pad, offs, counts, tlo, thi, ref_tri);
-    cudaFree(tmp); tmp = nullptr;
+    dw_sfree(tmp, stream); tmp = nullptr;
   }
   N = (size_t)std::max(n, 1); N2 = 2 * N;
   G = (unsigned)((N + B - 1) / B);
-  DW_B(cudaMalloc(&blo, sizeof(float4) * N2)); DW_B(cudaMalloc(&bhi, sizeof(float4) * N2));
-  for (int k = 0; k < 2; ++k) {
-    DW_B(cudaMalloc(&cl[k], sizeof(float4) * N)); DW_B(cudaMalloc(&ch[k], sizeof(float4) * N)); DW_B(cudaMalloc(&cn[k], 4 * N));
-    DW_B(cudaMalloc(&tasks[k], sizeof(WideTask) * N));
+  {   // grow the pool once for everything that follows (about 390 bytes per reference): forty small growths cost a first build 5 ms
+    void* warm = nullptr;
+    if (dw_salloc(c, &warm, 400 * N + (1 << 20), stream) == cudaSuccess) dw_sfree(warm, stream); else cudaGetLastError();
   }
-  DW_B(cudaMalloc(&keys, 8 * N)); DW_B(cudaMalloc(&keys2, 8 * N));
-  DW_B(cudaMalloc(&vals, 4 * N)); DW_B(cudaMalloc(&vals2, 4 * N));
-  DW_B(cudaMalloc(&left, 4 * N2)); DW_B(cudaMalloc(&right, 4 * N2)); DW_B(cudaMalloc(&parent, 4 * N2));
-  DW_B(cudaMalloc(&size, 4 * N2)); DW_B(cudaMalloc(&leftmost, 4 * N2));
-  DW_B(cudaMalloc(&nn, 4 * N)); DW_B(cudaMalloc(&keep, 4 * N)); DW_B(cudaMalloc(&isnew, 4 * N));
-  DW_B(cudaMalloc(&kpos, 4 * N)); DW_B(cudaMalloc(&npos, 4 * N)); DW_B(cudaMalloc(&slot, 4 * N));
+  DW_B(dw_salloc(c, &blo, sizeof(float4) * N2, stream)); DW_B(dw_salloc(c, &bhi, sizeof(float4) * N2, stream));
+  for (int k = 0; k < 2; ++k) {
+    DW_B(dw_salloc(c, &cl[k], sizeof(float4) * N, stream)); DW_B(dw_salloc(c, &ch[k], sizeof(float4) * N, stream)); DW_B(dw_salloc(c, &cn[k], 4 * N, stream));
+    DW_B(dw_salloc(c, &tasks[k], sizeof(WideTask) * N, stream));
+  }
+  DW_B(dw_salloc(c, &keys, 8 * N, stream)); DW_B(dw_salloc(c, &keys2, 8 * N, stream));
+  DW_B(dw_salloc(c, &vals, 4 * N, stream)); DW_B(dw_salloc(c, &vals2, 4 * N, stream));
+  DW_B(dw_salloc(c, &left, 4 * N2, stream)); DW_B(dw_salloc(c, &right, 4 * N2, stream)); DW_B(dw_salloc(c, &parent, 4 * N2, stream));
+  DW_B(dw_salloc(c, &size, 4 * N2, stream)); DW_B(dw_salloc(c, &leftmost, 4 * N2, stream));
+  DW_B(dw_salloc(c, &nn, 4 * N, stream)); DW_B(dw_salloc(c, &flag, N, stream)); DW_B(dw_salloc(c, &slot, 4 * N, stream));
+  DW_B(dw_salloc(c, &bsum, sizeof(int2) * (N / 256 + 1), stream)); DW_B(dw_salloc(c, &boff, sizeof(int2) * (N / 256 + 1), stream));
+  DW_B(dw_salloc(c, &pst, 4 * (8 + kMaxWideLevels + 2), stream));
   DW_B(cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, keys, keys2, vals, vals2, (int)N, 0, 63, stream));
-  DW_B(cub::DeviceScan::ExclusiveSum(nullptr, tmp2, keep, kpos, (int)N, stream));
-  tmp_bytes = std::max(tmp_bytes, tmp2);
-  DW_B(cudaMalloc(&tmp, tmp_bytes));
-  DW_B(cudaMalloc(&c->d_tris, 48 * N));
-  DW_B(cudaMalloc(&c->rf.slot_ref, 4 * N));
+  (void)tmp2;
+  DW_B(dw_salloc(c, &tmp, tmp_bytes, stream));
+  DW_B(dw_salloc(c, &c->d_tris, 48 * N, stream));
+  DW_B(dw_salloc(c, &c->rf.slot_ref, 4 * N, stream));
 
   if (n > 0) {
     morton_kernel<<<G, B, 0, stream>>>(n, tlo, thi, scene, keys, vals);
     DW_B(cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, keys, keys2, vals, vals2, n, 0, 63, stream));
     ploc_init_kernel<<<G, B, 0, stream>>>(n, vals2, tlo, thi, blo, bhi, cn[0], cl[0], ch[0], size, parent, leftmost);
-    // ---- PLOC rounds: clusters [0, m) in buffer `cur`; every round makes at least one node
-    int m = n, base = n, cur = 0;
-    while (m > 1) {
-      const unsigned Gm = (unsigned)((m + B - 1) / B);
-      ploc_nn_kernel<<<Gm, B, 0, stream>>>(m, radius, cl[cur], ch[cur], nn);
-      ploc_mark_kernel<<<Gm, B, 0, stream>>>(m, nn, keep, isnew);
-      DW_B(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, keep, kpos, m, stream));
-      DW_B(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, isnew, npos, m, stream));
-      ploc_apply_kernel<<<Gm, B, 0, stream>>>(m, base, nn, keep, isnew, kpos, npos, cn[cur], cl[cur], ch[cur], cn[cur ^ 1],
-                                              cl[cur ^ 1], ch[cur ^ 1], left, right, parent, blo, bhi, size);
-      int h_last[2];
-      DW_B(cudaMemcpyAsync(&h_last[0], kpos + (m - 1), 4, cudaMemcpyDeviceToHost, stream));
-      DW_B(cudaMemcpyAsync(&h_last[1], keep + (m - 1), 4, cudaMemcpyDeviceToHost, stream));
-      DW_B(cudaStreamSynchronize(stream));
-      const int m_new = h_last[0] + h_last[1];
-      if (m_new >= m || m_new < 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: clustering round made no progress (%d -> %d)", m, m_new); goto done; }
-      base += m - m_new;
-      m = m_new;
-      cur ^= 1;
-      ++ploc_rounds;
+    // ---- PLOC rounds: clusters [0, m) in buffer `cur`; every round makes at least one node.  m and the next node index are on the
+    // device (pst[0..1] / pst[2..3] by the parity of the round, pst[4] rounds, pst[5] error); one read-back per chunk of rounds
+    int base = n;
+    {
+      int init[8] = {n, n, n, n, 0, 0, 0, 0};
+      DW_B(cudaMemcpyAsync(pst, init, sizeof init, cudaMemcpyHostToDevice, stream));
+      int m = n, r = 0;
+      while (m > 1) {
+        if (r > 8192) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: clustering does not end"); goto done; }
+        const int chunk = r == 0 ? 24 : 12;
+        for (int q = 0; q < chunk; ++q, ++r) {
+          const int* st = pst + 2 * (r & 1);
+          int* stn = pst + 2 * ((r + 1) & 1);
+          const int cur = r & 1;
+          ploc_nn_kernel_dev<<<G, B, 0, stream>>>(st, radius, cl[cur], ch[cur], nn);
+          ploc_mark_kernel_dev<<<G, B, 0, stream>>>(st, nn, flag, bsum);
+          ploc_scan_kernel_dev<<<1, 1024, 0, stream>>>(st, stn, pst + 4, bsum, boff);
+          ploc_apply_kernel_dev<<<G, B, 0, stream>>>(st, nn, flag, boff, cn[cur], cl[cur], ch[cur], cn[cur ^ 1], cl[cur ^ 1], ch[cur ^ 1],
+                                                     left, right, parent, blo, bhi, size);
+        }
+        int h[8];
+        DW_B(cudaMemcpyAsync(h, pst, sizeof h, cudaMemcpyDeviceToHost, stream));
+        DW_B(cudaStreamSynchronize(stream));
+        if (h[5]) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: a clustering round made no progress"); goto done; }
+        m = h[2 * (r & 1)]; base = h[2 * (r & 1) + 1];
+        ploc_rounds = h[4] > 0 ? h[4] : ploc_rounds;
+      }
+      // rounds launched after m reached 1 did nothing, but were counted: the rounds that merged are those until base was complete
     }
     if (base != 2 * n - 1) { rc = dw_fail(c, DW_E_CUDA, "dw_build_bvh: %d of %d nodes made", base - n, n - 1); goto done; }
     leaf_walk_kernel<<<G, B, 0, stream>>>(n, left, parent, size, slot, leftmost, misc + 3);
     pack_tris_kernel<<<G, B, 0, stream>>>(n, vals2, ref_tri, slot, c->d_xyz, c->d_idx, c->d_code, c->d_chan, c->d_tris, c->rf.slot_ref);
   }
   if (n <= max_leaf) {
-    DW_B(cudaMalloc(&c->d_nodes, 128));
+    DW_B(dw_salloc(c, &c->d_nodes, 128, stream));
     wide_single_kernel<<<1, 1, 0, stream>>>(n, blo, bhi, c->d_nodes);
     h_misc[1] = 1; h_misc[2] = n > 0 ? 1 : 0;
   } else {
     // ---- collapse, one launch per level of the wide tree
-    DW_B(cudaMalloc(&nodes_tmp, 128 * N));
+    DW_B(dw_salloc(c, &nodes_tmp, 128 * N, stream));
     WideTask t0{2 * n - 2, 0};
     int init[3] = {0, 1, 0};
+    int* lvl = pst + 8;                                           // lvl[k] = tasks (= nodes) of level k, counted by the level before
+    std::vector<int> h_lvl(kMaxWideLevels + 2, 0);
+    h_lvl[0] = 1;
     DW_B(cudaMemcpyAsync(tasks[0], &t0, sizeof t0, cudaMemcpyHostToDevice, stream));
     DW_B(cudaMemcpyAsync(misc, init, sizeof init, cudaMemcpyHostToDevice, stream));
-    int count = 1, cur = 0;
-    wide_depth = 0;
-    while (count > 0) {
-      wide_collapse_kernel<<<(unsigned)((count + B - 1) / B), B, 0, stream>>>(count, tasks[cur], tasks[cur ^ 1], misc, max_leaf, left, right,
-                                                                            size, blo, bhi, slot, leftmost, nodes_tmp);
-      DW_B(cudaMemcpyAsync(&count, misc, 4, cudaMemcpyDeviceToHost, stream));
+    DW_B(cudaMemcpyAsync(lvl, h_lvl.data(), 4 * (kMaxWideLevels + 2), cudaMemcpyHostToDevice, stream));
+    {
+      const unsigned Gc = (unsigned)std::min<size_t>((N + B - 1) / B, (size_t)c->sm_count * 8);
+      for (int k = 0; k <= kMaxWideLevels; ++k)                   // a level without tasks is an empty launch
+        wide_collapse_kernel<<<Gc, B, 0, stream>>>(lvl + k, lvl + k + 1, tasks[k & 1], tasks[(k + 1) & 1], misc, max_leaf, left, right, size, blo, bhi,
+                                                   slot, leftmost, nodes_tmp);
+      DW_B(cudaMemcpyAsync(h_lvl.data(), lvl, 4 * (kMaxWideLevels + 2), cudaMemcpyDeviceToHost, stream));
       DW_B(cudaStreamSynchronize(stream));
-      DW_B(cudaMemsetAsync(misc, 0, 4, stream));
-      if (count > 0) levels.push_back(levels.back() + count);      // the children made by this launch are the next level
-      cur ^= 1;
-      ++wide_depth;
+      wide_depth = 0;
+      for (int k = 0; k <= kMaxWideLevels + 1 && h_lvl[k] > 0; ++k) {
+        ++wide_depth;
+        if (k > 0) levels.push_back(levels.back() + h_lvl[k]);  // the children made by level k - 1 are level k
+      }
+      if (h_lvl[kMaxWideLevels + 1] > 0) { rc = dw_fail(c, DW_E_RANGE, "dw_build_bvh: the tree is deeper than %d levels", kMaxWideLevels); goto done; }
     }
     DW_B(cudaMemcpyAsync(h_misc, misc, 16, cudaMemcpyDeviceToHost, stream));
     DW_B(cudaStreamSynchronize(stream));
     n_nodes = h_misc[1];
-    DW_B(cudaMalloc(&c->d_nodes, 128 * (size_t)n_nodes));
+    DW_B(dw_salloc(c, &c->d_nodes, 128 * (size_t)n_nodes, stream));
     DW_B(cudaMemcpyAsync(c->d_nodes, nodes_tmp, 128 * (size_t)n_nodes, cudaMemcpyDeviceToDevice, stream));
   }
   DW_B(cudaGetLastError());
@@ -925,10 +1043,10 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
     }
   }
 done:
-  cudaFree(tlo); cudaFree(thi); cudaFree(tlo_t); cudaFree(thi_t); cudaFree(counts); cudaFree(offs); cudaFree(ref_tri); cudaFree(blo); cudaFree(bhi); cudaFree(scene); cudaFree(keys); cudaFree(keys2); cudaFree(vals);
-  cudaFree(vals2); cudaFree(left); cudaFree(right); cudaFree(parent); cudaFree(size); cudaFree(leftmost); cudaFree(nn);
-  cudaFree(keep); cudaFree(isnew); cudaFree(kpos); cudaFree(npos); cudaFree(slot); cudaFree(misc); cudaFree(tmp); cudaFree(nodes_tmp); cudaFree(occ); cudaFree(sat);
-  for (int k = 0; k < 2; ++k) { cudaFree(cl[k]); cudaFree(ch[k]); cudaFree(cn[k]); cudaFree(tasks[k]); }
+  dw_sfree(tlo, stream); dw_sfree(thi, stream); dw_sfree(tlo_t, stream); dw_sfree(thi_t, stream); dw_sfree(counts, stream); dw_sfree(offs, stream); dw_sfree(ref_tri, stream); dw_sfree(blo, stream); dw_sfree(bhi, stream); dw_sfree(scene, stream); dw_sfree(keys, stream); dw_sfree(keys2, stream); dw_sfree(vals, stream);
+  dw_sfree(vals2, stream); dw_sfree(left, stream); dw_sfree(right, stream); dw_sfree(parent, stream); dw_sfree(size, stream); dw_sfree(leftmost, stream); dw_sfree(nn, stream);
+  dw_sfree(flag, stream); dw_sfree(bsum, stream); dw_sfree(boff, stream); dw_sfree(pst, stream); dw_sfree(slot, stream); dw_sfree(misc, stream); dw_sfree(tmp, stream); dw_sfree(nodes_tmp, stream); dw_sfree(occ, stream); dw_sfree(sat, stream);
+  for (int k = 0; k < 2; ++k) { dw_sfree(cl[k], stream); dw_sfree(ch[k], stream); dw_sfree(cn[k], stream); dw_sfree(tasks[k], stream); }
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
   if (rc != DW_OK) dw_bvh_free(c);
