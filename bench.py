@@ -220,6 +220,10 @@ def main():
     ap.add_argument("--sweep", action="store_true", help="with --config 4: also run BASELINE.json configs[4] as written (PTFE reflectivity 0.90 / 0.95 / "
                     "0.99, 10 batches of 1e7 photons each with photon_id_base = b * 1e7, only dw_set_surfaces between them) and report the wall "
                     "time of the sweep, the hit map totals and the arrival-time histogram per reflectivity in config.sweep")
+    ap.add_argument("--design-study", type=int, default=0, help="also time dw_design_study (ONE library call: emit, propagate, tally, LCE and "
+                    "t90) for this many point sources on a Z x R^2 grid of the config's liquid volume (the paper's LCE map has ~2500), "
+                    "--study-photons each; reported in config.design_study (SURVEY 8(f) f3, diagnostic)")
+    ap.add_argument("--study-photons", type=int, default=1_000_000, help="photons per source of --design-study (the paper: 1e6)")
     ap.add_argument("--no-counters", action="store_true", help="skip the run of the counting instantiation (roofline.implementation_counters)")
     ap.add_argument("--counter-sample", type=int, default=2_000_000, help="photons of the batch that the counting instantiation runs over")
     ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
@@ -355,10 +359,32 @@ def main():
                          achieved_gbs=44.0 * n / (ems * 1e-3) / 1e9, hbm_peak_gbs=peaks0["hbm_gbs"],
                          frac_of_hbm=44.0 * n / (ems * 1e-3) / 1e9 / peaks0["hbm_gbs"])
 
+    study_info = None
+    if args.design_study > 0 and world == 1 and args.config in (1, 2, 3):
+        g = geom
+        R, zl = (250.0, 495.0) if args.config == 1 else (1300.0, 2600.0)
+        nz = max(1, int(round(np.sqrt(args.design_study * 2))))         # twice as many heights as radii, as in the paper's maps
+        nr = max(1, -(-args.design_study // nz))
+        srcs = [_synth.source(_synth.SHAPE_POINT, (float(np.sqrt((j + 0.5) / nr) * (R - 20.0)), 0.0, float(10.0 + (i + 0.5) / nz * (zl - 20.0))))
+                for i in range(nz) for j in range(nr)][: args.design_study]
+        group = np.where(np.arange(g.n_channels) < g.n_channels // 2, 0, 1).astype(np.int32)
+        comp = (np.asarray(g.surface) + 1).astype(np.int32)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res = ctx.design_study(srcs, args.study_photons, c.seed, c.max_steps, group, 2, comp, int(comp.max()) + 1, n_bins=1000, dt=1.0,
+                               sources_per_batch=max(1, (1 << 25) // args.study_photons), device=dev)
+        dt = time.perf_counter() - t0
+        lce = res["lce"].sum(1)
+        study_info = dict(sources=len(srcs), photons_per_source=args.study_photons, seconds=dt, photons_per_s=len(srcs) * args.study_photons / dt,
+                          api="dw_design_study (one call)", lce_min=float(lce.min()), lce_max=float(lce.max()),
+                          t90_min_ns=float(np.nanmin(res["t90"])), t90_max_ns=float(np.nanmax(res["t90"])),
+                          absorbed_by_component=[int(v) for v in res["absorbed_by_component"]])
+
     sweep_info = None
     if args.sweep and args.config == 4 and world == 1 and not args.emit:
-        nb = 10
-        batches = [dw.DevicePhotons(c.make_photons(n, b * n), dev) for b in range(nb)]       # 10 x 440 MB resident; generation is not timed
+        nb, nbp = 10, 10_000_000                                                             # BASELINE.json: 1e8 photons in batches of 1e7
+        batches = [dw.DevicePhotons(c.make_photons(nbp, b * nbp), dev) for b in range(nb)]   # 10 x 440 MB resident; generation is not timed
+        out_b = dw.DeviceResults(nbp, ("flags", "channel", "t", "steps", "last_tri", "x", "y", "z"), dev)
         sweep_info, t_all = {}, 0.0
         for rho in (0.90, 0.95, 0.99):
             o4 = _synth.config(4, ptfe_reflectivity=rho).optics
@@ -367,7 +393,7 @@ def main():
             t0 = time.perf_counter()
             ctx.set_surfaces(o4.detect, o4.reflect_diffuse, o4.reflect_specular, o4.transmit)    # the only thing that changes: no BVH rebuild
             for b in range(nb):
-                ctx.propagate(batches[b], c.seed, c.max_steps, out, hs, flags=flags, stream=stream)
+                ctx.propagate(batches[b], c.seed, c.max_steps, out_b, hs, flags=flags, stream=stream)
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
             t_all += dt
@@ -376,12 +402,12 @@ def main():
             th = hh["time_hist"].astype(np.int64)
             cum = np.cumsum(th)
             nch = ctx.n_chan // 2
-            sweep_info[f"rho_{rho:.2f}"] = dict(seconds=dt, photons=n * nb, photons_per_s=n * nb / dt, detected=det, lce=det / (n * nb),
+            sweep_info[f"rho_{rho:.2f}"] = dict(seconds=dt, photons=nbp * nb, photons_per_s=nbp * nb / dt, detected=det, lce=det / (nbp * nb),
                                                 hits_bottom_array=int(hh["chan_count"][:nch].sum()), hits_top_array=int(hh["chan_count"][nch:].sum()),
                                                 max_hits_one_pmt=int(hh["chan_count"].max()), escaped=int(hh["fate_count"][3]),
                                                 arrival_hist_peak_bin_ns=int(th.argmax()), arrival_hist_overflow=int(th[-1]),
                                                 bin_holding_90_percent_ns=int(np.searchsorted(cum, 0.9 * cum[-1])),
-                                                steps_per_photon=int(hh["total_steps"][0]) / (n * nb))
+                                                steps_per_photon=int(hh["total_steps"][0]) / (nbp * nb))
         sweep_info["wall_seconds_3_reflectivities"] = t_all
         o4 = c.optics
         ctx.set_surfaces(o4.detect, o4.reflect_diffuse, o4.reflect_specular, o4.transmit)
@@ -436,8 +462,9 @@ def main():
     # T_roof = max(B_L2 / BW_L2, B_HBM / BW_HBM, F / P_FP32); each term as a fraction of the measured time
     frac_alu = achieved_lane / peak_lane
     frac_l2 = (tree_bytes / kernel_s / 1e9) / l2_gbs if l2_gbs else None
-    tree_in_l2 = (stats["node_bytes"] + stats["tri_bytes"]) < 100e6
-    hbm_bytes = state_bytes + (0 if tree_in_l2 else tree_bytes)
+    tree_total = float(stats["node_bytes"] + stats["tri_bytes"])
+    tree_in_l2 = tree_total < 100e6
+    hbm_bytes = state_bytes + tree_total                                         # the state once, and one compulsory pass over the tree
     frac_hbm = (hbm_bytes / kernel_s / 1e9) / peaks["hbm_gbs"]
     terms = dict(alu=frac_alu, l2=frac_l2 or 0.0, hbm=frac_hbm)
     binding = max(terms, key=terms.get)
@@ -510,7 +537,8 @@ def main():
                             **({"moved": args.move, "refit": refit_info} if args.move else {}),
                             **({"render": render_info} if render_info else {}),
                             **({"pipelined": pipelined} if pipelined else {}),
-                            **({"sweep": sweep_info} if sweep_info else {})),
+                            **({"sweep": sweep_info} if sweep_info else {}),
+                            **({"design_study": study_info} if study_info else {})),
                 photon_steps_per_s=total_steps / (total_ms * 1e-3),
                 steps_per_photon=total_steps / (n_all * args.steps),
                 fates={k: int(v) for k, v in zip(dw.FATE_NAMES, fate[:6])},
