@@ -353,6 +353,26 @@ int dw_design_study(dw_ctx* ctx, const dw_source* sources, int64_t n_sources, in
                     int32_t max_steps, const dw_tally_tables* tables, int64_t sources_per_batch, float quantile, float* lce_out,
                     float* t90_out, void* cuda_stream);
 
+/* dw_design_study for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the same
+ * loop and the same results (photon ids are s * photons_per_source + i, so the batching does not show), but the source table, the
+ * photon and result buffers of a batch and the queue head of the propagation launches lie in ONE file-scope device array of
+ * DW_STATIC_SCRATCH_BYTES that every GPU on which the library's module is loaded holds until the process exits.  The call makes no
+ * cudaMalloc / cudaFree / cudaMallocAsync and creates no stream or event; it issues one cudaMemcpyAsync (the sources), 8-byte
+ * cudaMemsetAsync's and kernel launches on the stream.  Limits, DW_E_RANGE with a message beyond them:
+ *   n_sources <= DW_STATIC_MAX_SOURCES,  photons_per_source <= DW_STATIC_MAX_PHOTONS (a batch is as many whole sources as fit that).
+ * sources: HOST [n_sources]; tables (ACCUMULATED: the caller zeroes) and lce_out / t90_out (may be NULL): DEVICE, the caller's.
+ * The array is shared by ALL contexts and calls on a device and keeps the last call's contents: the call zeroes the queue head
+ * before every launch and overwrites what it reads, but two calls that overlap on the GPU (different streams, or two contexts on
+ * one device) race on it -- keep them on one stream or order them with events.  The first call on a device looks the array up
+ * (cudaGetSymbolAddress with that device current, which loads the module); make one call before a capture starts.  Asynchronous
+ * like dw_emit_sources. */
+#define DW_STATIC_MAX_SOURCES 4096
+#define DW_STATIC_MAX_PHOTONS 262144
+#define DW_STATIC_SCRATCH_BYTES (256 + 64 * DW_STATIC_MAX_SOURCES + 60 * DW_STATIC_MAX_PHOTONS)   /* 15.25 MiB */
+int dw_design_study_static(dw_ctx* ctx, const dw_source* sources, int64_t n_sources, int64_t photons_per_source, uint64_t seed,
+                           int32_t max_steps, const dw_tally_tables* tables, float quantile, float* lce_out, float* t90_out,
+                           void* cuda_stream);
+
 
 /* Measured denominators for the roofline (SURVEY.md 8(d) "Peaks": the driver's peaks file holds HBM and
  * tensor numbers only).  Runs four short register-only / L2-resident kernels on the default stream and waits for them:

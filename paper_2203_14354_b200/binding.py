@@ -31,7 +31,8 @@ COUNTER_NAMES = ("node_visits", "tri_tests", "queries_traced", "queries_skipped"
 EXPORTS = ("dw_create", "dw_destroy", "dw_last_error", "dw_version", "dw_set_materials", "dw_set_surfaces",
            "dw_set_geometry", "dw_build_bvh", "dw_first_hit", "dw_propagate", "dw_propagate_host",
            "dw_debug_philox", "dw_last_launch", "dw_emit", "dw_set_films", "dw_tally", "dw_probe_peaks", "dw_refit_bvh", "dw_render",
-           "dw_tally_finish", "dw_emit_sources", "dw_design_study", "dw_propagate_counters")
+           "dw_tally_finish", "dw_emit_sources", "dw_design_study", "dw_propagate_counters", "dw_design_study_static")
+STATIC_MAX_SOURCES, STATIC_MAX_PHOTONS = 4096, 262144       # include/darwinopt.h DW_STATIC_MAX_*
 
 vp, i32, i64, u32, u64, f32 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_float
 
@@ -126,6 +127,7 @@ def load(build_if_missing: bool = True) -> C.CDLL:
     L.dw_tally_finish.argtypes = [vp, C.POINTER(TallyTables), i64, f32, vp, vp, vp]
     L.dw_emit_sources.argtypes = [vp, C.POINTER(Source), i64, i64, u64, C.POINTER(Photons), vp]
     L.dw_design_study.argtypes = [vp, C.POINTER(Source), i64, i64, u64, i32, C.POINTER(TallyTables), i64, f32, vp, vp, vp]
+    L.dw_design_study_static.argtypes = [vp, C.POINTER(Source), i64, i64, u64, i32, C.POINTER(TallyTables), f32, vp, vp, vp]
     L.dw_last_launch.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
     for name in EXPORTS:
         if name not in ("dw_last_error",):
@@ -287,6 +289,17 @@ class Context:
                                            _stream_ptr()))
         torch.cuda.synchronize()
         return acc.numpy()
+
+    def design_study_static(self, sources, photons_per_source, seed, max_steps, acc: "Tally", quantile=0.9, stream=None):
+        """dw_design_study_static: the same loop with every scratch buffer in the library's fixed device array, so the call allocates
+        nothing (include/darwinopt.h).  `acc` holds the caller's tables (zeroed by the caller) and receives lce / t90.  At most
+        STATIC_MAX_SOURCES sources of at most STATIC_MAX_PHOTONS photons each (DW_E_RANGE beyond).  Asynchronous on the stream."""
+        ns = len(sources)
+        if ns > acc.ns:
+            raise ValueError(f"{ns} sources, the tables hold {acc.ns}")
+        arr = (Source * ns)(*[_source(s) for s in sources])
+        self._check(self.L.dw_design_study_static(self.h, arr, ns, int(photons_per_source), int(seed), int(max_steps), C.byref(acc.c),
+                                                  float(quantile), _dp(acc.lce), _dp(acc.t90) if acc.nb > 0 else None, _stream_ptr(stream)))
 
     def probe_peaks(self) -> dict:
         """Measured issue rates and L2 read bandwidth of this device (include/darwinopt.h dw_probe_peaks)."""

@@ -9,7 +9,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "libdarwinopt.so"
-SOURCES = ["dw_api.cu", "dw_bvh.cu", "dw_kernels.cu", "dw_probe.cu"]
+SOURCES = ["dw_api.cu", "dw_bvh.cu", "dw_kernels.cu", "dw_probe.cu", "dw_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-O2", "--expt-relaxed-constexpr"]
 

@@ -457,6 +457,7 @@ static int check_source(dw_ctx* c, const char* who, const dw_source* src) {
     return dw_fail(c, DW_E_ARG, "%s: radius, sigma, tau must be >= 0, z0 <= z1, 0 <= f_singlet <= 1", who);
   return DW_OK;
 }
+int dw_check_source(dw_ctx* c, const char* who, const dw_source* src) { return check_source(c, who, src); }   // for dw_static.cu
 static int check_emit_out(dw_ctx* c, const char* who, const dw_photons* out) {
   if (out->n < 0) return dw_fail(c, DW_E_ARG, "%s: n < 0", who);
   const float* const arr[11] = {out->px, out->py, out->pz, out->kx, out->ky, out->kz, out->ex, out->ey, out->ez, out->wavelength, out->t0};

@@ -143,5 +143,11 @@ int dw_render_impl(dw_ctx* ctx, const dw_camera* cam, int32_t* tri, float* depth
 int dw_emit_impl(dw_ctx* ctx, const dw_source* src, uint64_t seed, const dw_photons* out, cudaStream_t stream);
 int dw_emit_sources_impl(dw_ctx* ctx, const dw_source* d_sources, int64_t photons_per_source, uint64_t seed, const dw_photons* out,
                          cudaStream_t stream);
+// The default propagation kernel over in->n <= 2^30 photons with the queue head in the caller's device memory (8 bytes, zeroed here
+// on the stream) instead of a stream-ordered allocation; no per-launch parameters, no histograms (dw_static.cu).
+int dw_propagate_head_impl(dw_ctx* ctx, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                           unsigned long long* head, cudaStream_t stream);
 int dw_debug_philox_impl(dw_ctx* ctx, uint64_t seed, uint64_t base, uint32_t step, uint32_t block, int64_t n,
                          uint32_t* out_raw, float* out_u, cudaStream_t stream);
+// implemented in dw_api.cu
+int dw_check_source(dw_ctx* ctx, const char* who, const dw_source* src);

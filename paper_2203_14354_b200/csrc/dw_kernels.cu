@@ -1532,6 +1532,43 @@ int dw_propagate_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t ma
   return DW_OK;
 }
 
+// launch_propagate for params == NULL, counters == NULL and no histograms, with the queue head given by the caller instead of
+// allocated on the stream (dw_design_study_static).  Same kernel, block size, shared memory and grid as the allocating path.
+int dw_propagate_head_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_results* out,
+                           unsigned long long* head, cudaStream_t stream) {
+  if (in->n <= 0) return DW_OK;
+  if (in->n > (int64_t(1) << 30) || !head) return dw_fail(c, DW_E_ARG, "dw_propagate_head_impl: at most 2^30 photons and a queue head");
+  PropArgs A{};
+  A.bvh = c->bvh; A.tab = c->tables; A.in = *in;
+  if (out) A.out = *out;
+  for (int r = 0; r < 10; ++r) {
+    A.keys[2 * r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
+    A.keys[2 * r + 1] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
+  }
+  A.seed = seed; A.max_steps = max_steps; A.flags = 0u;
+  A.th_phys = 8; A.th_leaf = 12;
+  A.counters = nullptr;
+  A.queue_head = head;
+  const int B = 128;
+  const bool films = c->tables.film != nullptr && c->tables.film_on != nullptr;
+  const bool flat = DW_FLAT_TABLES && c->tables.nl_mat == 1 && c->tables.nl_surf == 1;
+  const size_t smem = sizeof(int) * (size_t)warp_ints(flat && !films) * (B / 32);
+  void (*kern)(PropArgs) = films ? (flat ? propagate_pool_kernel<true, true, false> : propagate_pool_kernel<true, false, false>)
+                                 : (flat ? propagate_pool_kernel<false, true, false> : propagate_pool_kernel<false, false, false>);
+  int per_sm = 0;
+  DW_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, B, smem));
+  if (per_sm < 1) return dw_fail(c, DW_E_CUDA, "dw_design_study_static: kernel does not fit on an SM");
+  const int64_t warps_needed = (in->n + kSlots - 1) / kSlots;
+  const int64_t blocks_needed = (warps_needed + (B / 32) - 1) / (B / 32);
+  const int grid = (int)std::min<int64_t>((int64_t)c->sm_count * per_sm, std::max<int64_t>(blocks_needed, 1));
+  DW_CUDA(c, cudaMemsetAsync(head, 0, sizeof(unsigned long long), stream));
+  kern<<<grid, B, smem, stream>>>(A);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return dw_fail(c, DW_E_CUDA, "propagate kernel launch failed: %s", cudaGetErrorString(e));
+  c->last_grid = grid; c->last_block = B; c->last_smem = (int)smem; c->n_launches += 1;
+  return DW_OK;
+}
+
 int dw_propagate_counters_impl(dw_ctx* c, const dw_photons* in, uint64_t seed, int32_t max_steps, const dw_propagate_params* params,
                                uint64_t* host_out, int n_out) {
   if (in->n > (int64_t(1) << 30)) return dw_fail(c, DW_E_ARG, "dw_propagate_counters: at most 2^30 photons");
