@@ -521,6 +521,53 @@ __device__ __forceinline__ bool segment_is_free(const DwBvh& B, V3 x, V3 k, floa
   }
 }
 
+// L2 eviction priorities for the photon state (measured, off): a result word is stored when its photon ends, and the other seven
+// photons of its 32-byte sector end up to milliseconds later; the launch moves 1.18 GB through HBM where the state is 0.76 GB.
+// DW_OUT_HINT 1 / 2 / 3: result stores with L2::evict_last / .cg / .wt; DW_IN_HINT 1 / 2 / 3: input loads with L2::evict_first /
+// .cs / L2::evict_last.  None lowers the traffic (profiles/r02_experiments.md section 5d): evict_last stores 1.179 GB and 0.4 ms
+// slower, evict_first loads 2.74 GB (the sectors of a warp's id chunk are re-read between refills), evict_last loads 1.247 GB.
+#ifndef DW_OUT_HINT
+#define DW_OUT_HINT 0
+#endif
+#ifndef DW_IN_HINT
+#define DW_IN_HINT 0
+#endif
+template <class T> __device__ __forceinline__ void st_out(T* p, T v) {
+  static_assert(sizeof(T) == 4, "result words are 32 bits");
+#if DW_OUT_HINT == 1
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  unsigned bits;
+  memcpy(&bits, &v, 4);
+  asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(bits), "l"(pol) : "memory");
+#elif DW_OUT_HINT == 2
+  __stcg(p, v);
+#elif DW_OUT_HINT == 3
+  __stwt(p, v);
+#else
+  *p = v;
+#endif
+}
+__device__ __forceinline__ float ld_in(const float* p) {
+#if DW_IN_HINT == 1
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  float v;
+  asm volatile("ld.global.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+  return v;
+#elif DW_IN_HINT == 2
+  return __ldcs(p);
+#elif DW_IN_HINT == 3
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  float v;
+  asm volatile("ld.global.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(p), "l"(pol));
+  return v;
+#else
+  return *p;
+#endif
+}
+
 // ------------------------------------------------------------------------------------------------ propagation
 struct PropArgs {
   uint32_t keys[20];                // Philox round keys of `seed` (k0 + r W0, k1 + r W1), filled by the host: constant-bank operands
@@ -978,11 +1025,11 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       uint32_t step = 0, hist = 0;
       bool absorb_first = false;
       if (fresh) {
-        x = mk(A.in.px[pi], A.in.py[pi], A.in.pz[pi]);
-        k = mk(A.in.kx[pi], A.in.ky[pi], A.in.kz[pi]);
-        e = mk(A.in.ex[pi], A.in.ey[pi], A.in.ez[pi]);
-        lambda = A.in.wavelength[pi];
-        t = A.in.t0[pi];
+        x = mk(ld_in(A.in.px + pi), ld_in(A.in.py + pi), ld_in(A.in.pz + pi));
+        k = mk(ld_in(A.in.kx + pi), ld_in(A.in.ky + pi), ld_in(A.in.kz + pi));
+        e = mk(ld_in(A.in.ex + pi), ld_in(A.in.ey + pi), ld_in(A.in.ez + pi));
+        lambda = ld_in(A.in.wavelength + pi);
+        t = ld_in(A.in.t0 + pi);
       } else if (slot >= 0) {
         x = mk(poolf[W_X * kSlots + slot], poolf[W_Y * kSlots + slot], poolf[W_Z * kSlots + slot]);
         k = mk(poolf[W_KX * kSlots + slot], poolf[W_KY * kSlots + slot], poolf[W_KZ * kSlots + slot]);
@@ -1187,16 +1234,16 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
 
       // -------------------------------------------------------------- a10: outputs and reductions
       if (fate != 0xFFu) {
-        if (A.out.flags) A.out.flags[pi] = fate | hist;
-        if (A.out.channel) A.out.channel[pi] = channel;
-        if (A.out.t) A.out.t[pi] = t;
-        if (A.out.steps) A.out.steps[pi] = step;
-        if (A.out.last_tri) A.out.last_tri[pi] = last_tri;
-        if (A.out.x) A.out.x[pi] = x.x;
-        if (A.out.y) A.out.y[pi] = x.y;
-        if (A.out.z) A.out.z[pi] = x.z;
-        if (A.out.kx) { A.out.kx[pi] = k.x; A.out.ky[pi] = k.y; A.out.kz[pi] = k.z; }
-        if (A.out.ex) { A.out.ex[pi] = e.x; A.out.ey[pi] = e.y; A.out.ez[pi] = e.z; }
+        if (A.out.flags) st_out(A.out.flags + pi, fate | hist);
+        if (A.out.channel) st_out(A.out.channel + pi, channel);
+        if (A.out.t) st_out(A.out.t + pi, t);
+        if (A.out.steps) st_out(A.out.steps + pi, step);
+        if (A.out.last_tri) st_out(A.out.last_tri + pi, last_tri);
+        if (A.out.x) st_out(A.out.x + pi, x.x);
+        if (A.out.y) st_out(A.out.y + pi, x.y);
+        if (A.out.z) st_out(A.out.z + pi, x.z);
+        if (A.out.kx) { st_out(A.out.kx + pi, k.x); st_out(A.out.ky + pi, k.y); st_out(A.out.kz + pi, k.z); }
+        if (A.out.ex) { st_out(A.out.ex + pi, e.x); st_out(A.out.ey + pi, e.y); st_out(A.out.ez + pi, e.z); }
         atomicAdd(&s_fate[fate & 7u], 1u);
         atomicAdd(&s_steps, (unsigned long long)step);
         st[slot] = S_EMPTY;
