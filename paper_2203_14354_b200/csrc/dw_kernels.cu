@@ -899,6 +899,17 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 #ifndef DW_TRI_REPS
 #define DW_TRI_REPS 2
 #endif
+// Slots that must be ready for a physics phase before tracing lanes that find nothing queued leave the traversal loop for it.  The
+// pool of 64 slots never holds less than 32 ready slots when 8 lanes are idle, so 32 means "whenever th_phys lanes starve"; 16 lets
+// a warp in its tail do the same.  C2 42.46 -> 42.14 ms, C3 44.76 -> 44.46 (12 / 16 / 20 within 0.1 ms; profiles/r02_experiments.md 5e).
+#ifndef DW_TH_READY
+#define DW_TH_READY 16
+#endif
+// Ready slots from which a physics phase runs whatever the lanes are doing (a phase takes at most 32).  Phases with fewer slots cost
+// the same instructions: 28 / 24 / 20 / 16 measured 42.9 / 44.5 / 46.7 / 49.0 against 42.4 ms.
+#ifndef DW_TH_PHYS_FULL
+#define DW_TH_PHYS_FULL 32
+#endif
 #ifndef DW_NODE_REPS_MIN
 #define DW_NODE_REPS_MIN 16
 #endif
@@ -990,7 +1001,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
     const int nB = 32 - __popc(idle);
     if (nP + nE + nQ + nB == 0) break;
 
-    const bool do_phys = (nP + nE >= 32) || (nQ == 0 && (nB == 0 || nP + nE >= 8));
+    const bool do_phys = (nP + nE >= DW_TH_PHYS_FULL) || (nQ == 0 && (nB == 0 || nP + nE >= 8));
     if (do_phys) {
       // -------------------------------------------------------------- phase P: up to 32 slots, finished queries first
       const int nPc = min(nP, 32);
@@ -1301,7 +1312,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       if (prevAct >= 0) nReady += prevAct - nAct;           // queries that ended in the last iteration
       prevAct = nAct;
       if (nAct == 0) break;
-      if (32 - nAct >= th_fetch && (nQ_rem > 0 || nReady >= 32)) break;
+      if (32 - nAct >= th_fetch && (nQ_rem > 0 || nReady >= DW_TH_READY)) break;
       if (nI > 0 && nL < th_leaf) {
 #if DW_NODE_REPS > 1
         // several node visits per vote while most lanes are in internal nodes: the votes are a quarter of the traversal's instructions
