@@ -1049,6 +1049,7 @@ done:
   for (int k = 0; k < 2; ++k) { dw_sfree(cl[k], stream); dw_sfree(ch[k], stream); dw_sfree(cn[k], stream); dw_sfree(tasks[k], stream); }
   if (ev0) cudaEventDestroy(ev0);
   if (ev1) cudaEventDestroy(ev1);
+  cudaStreamSynchronize(stream);   // the frees above are complete when the call returns: the next build finds its memory in the pool
   if (rc != DW_OK) dw_bvh_free(c);
   return rc;
 }
