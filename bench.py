@@ -225,7 +225,9 @@ def main():
                     "--study-photons each; reported in config.design_study (SURVEY 8(f) f3, diagnostic)")
     ap.add_argument("--study-photons", type=int, default=1_000_000, help="photons per source of --design-study (the paper: 1e6)")
     ap.add_argument("--no-counters", action="store_true", help="skip the run of the counting instantiation (roofline.implementation_counters)")
-    ap.add_argument("--counter-sample", type=int, default=2_000_000, help="photons of the batch that the counting instantiation runs over")
+    ap.add_argument("--counter-sample", type=int, default=0,
+                    help="photons of the batch that the counting instantiation runs over (0 = the whole batch: a short sample is mostly the "
+                         "tail of its warps and under-reports the lanes per iteration)")
     ap.add_argument("--block", type=int, default=0, help="threads per block (0 = library default)")
     ap.add_argument("--blocks-per-sm", type=int, default=0, help="cap on resident blocks per SM (0 = occupancy limit)")
     args = ap.parse_args()
@@ -486,7 +488,7 @@ def main():
     # what the kernel actually does per photon-step: the counting instantiation, once over a sample, outside the timed region
     if not args.legacy and not args.literal and not args.no_counters:
         try:
-            ns = min(n, args.counter_sample)
+            ns = min(n, args.counter_sample) if args.counter_sample > 0 else n
             hs = dw.DeviceHists(ctx.n_chan, 0, 0.0, 1.0, dev)
             ps = dw.DevicePhotons(ph.slice(0, ns), dev)
             ctx.propagate(ps, c.seed, c.max_steps, None, hs, flags=flags, stream=stream)

@@ -874,8 +874,8 @@ __global__ void __launch_bounds__(128, 6) propagate_kernel(const __grid_constant
 #ifndef DW_POOL_SLOTS
 #define DW_POOL_SLOTS 64
 #endif
-constexpr int kSlots = DW_POOL_SLOTS;      // 33..64: lane l looks after slots l and l + 32 (the latter if it exists)
-static_assert(kSlots > 32 && kSlots <= 64, "pool size");
+constexpr int kSlots = DW_POOL_SLOTS;      // 33..96: lane l looks after slots l, l + 32 and l + 64 (those that exist)
+static_assert(kSlots > 32 && kSlots <= 96, "pool size");
 // The last two words exist only in the full layout: with flat tables and no films the wavelength is never read again and n1 is one
 // table load from the medium, so the lean layout (20 words) leaves them out.  With 8 shared stack entries a lean block takes 26 kB, six of
 // them fit the 164 kB shared-memory configuration instead of 196 kB, and L1 grows from ~60 to ~92 kB (profiles/r01_captures_9_to_12_c2.md).
@@ -907,6 +907,9 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 #endif
 // Ready slots from which a physics phase runs whatever the lanes are doing (a phase takes at most 32).  Phases with fewer slots cost
 // the same instructions: 28 / 24 / 20 / 16 measured 42.9 / 44.5 / 46.7 / 49.0 against 42.4 ms.
+#ifndef DW_REFILL_MIN
+#define DW_REFILL_MIN 0
+#endif
 #ifndef DW_TH_PHYS_FULL
 #define DW_TH_PHYS_FULL 32
 #endif
@@ -966,8 +969,10 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   int* const my_stack = wbase + warp_stack(kLean) + lane;
   constexpr int sstride = 32;
   const bool has2 = lane + 32 < kSlots;            // this lane also looks after slot lane + 32
+  const bool has3 = lane + 64 < kSlots;            // ... and slot lane + 64 (pools of more than 64 slots)
   st[lane] = S_EMPTY;
   if (has2) st[lane + 32] = S_EMPTY;
+  if (has3) st[lane + 64] = S_EMPTY;
   __syncthreads();
   int lstack[kStackLocal];
   const unsigned lt = (1u << lane) - 1u;
@@ -991,20 +996,26 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
   for (;;) {
     // ---------------------------------------------------------------- census of the warp's slots
     const int s0 = st[lane], s1 = has2 ? st[lane + 32] : -1;
+    int s2 = -1;
+    if constexpr (kSlots > 64) s2 = has3 ? st[lane + 64] : -1;
     const unsigned p0 = __ballot_sync(0xffffffffu, s0 == S_PHYS), p1 = __ballot_sync(0xffffffffu, s1 == S_PHYS);
     const unsigned e0 = __ballot_sync(0xffffffffu, s0 == S_EMPTY), e1 = __ballot_sync(0xffffffffu, s1 == S_EMPTY);
     const unsigned t0 = __ballot_sync(0xffffffffu, s0 == S_TRACE), t1 = __ballot_sync(0xffffffffu, s1 == S_TRACE);
+    unsigned p2 = 0, e2 = 0, t2 = 0;
+    if constexpr (kSlots > 64) {
+      p2 = __ballot_sync(0xffffffffu, s2 == S_PHYS); e2 = __ballot_sync(0xffffffffu, s2 == S_EMPTY); t2 = __ballot_sync(0xffffffffu, s2 == S_TRACE);
+    }
     const unsigned idle = __ballot_sync(0xffffffffu, my < 0);
-    const int nP = __popc(p0) + __popc(p1);
-    const int nE = exhausted ? 0 : __popc(e0) + __popc(e1);
-    const int nQ = __popc(t0) + __popc(t1);
+    const int nP = __popc(p0) + __popc(p1) + __popc(p2);
+    const int nE = exhausted ? 0 : __popc(e0) + __popc(e1) + __popc(e2);
+    const int nQ = __popc(t0) + __popc(t1) + __popc(t2);
     const int nB = 32 - __popc(idle);
     if (nP + nE + nQ + nB == 0) break;
 
     const bool do_phys = (nP + nE >= DW_TH_PHYS_FULL) || (nQ == 0 && (nB == 0 || nP + nE >= 8));
     if (do_phys) {
       // -------------------------------------------------------------- phase P: up to 32 slots, finished queries first
-      const int nPc = min(nP, 32);
+      const int nPc = min(nP, 32 - min(nE, DW_REFILL_MIN)); // finished queries first, but DW_REFILL_MIN lanes are kept for empty slots
       int take = min(nE, 32 - nPc);                         // empty slots to refill (a2)
       if (take > 0 && w_next == w_end) {                    // claim a new chunk of photon ids (one atomic per warp)
         unsigned long long base = 0;
@@ -1020,12 +1031,16 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
       if (s1 == S_PHYS) q[__popc(p0) + __popc(p1 & lt)] = lane + 32;
       if (s0 == S_EMPTY) q[nP + __popc(e0 & lt)] = lane;
       if (s1 == S_EMPTY) q[nP + __popc(e0) + __popc(e1 & lt)] = lane + 32;
+      if constexpr (kSlots > 64) {
+        if (s2 == S_PHYS) q[__popc(p0) + __popc(p1) + __popc(p2 & lt)] = lane + 64;
+        if (s2 == S_EMPTY) q[nP + __popc(e0) + __popc(e1) + __popc(e2 & lt)] = lane + 64;
+      }
       __syncwarp();
       int slot = -1;
       bool fresh = false;
       int64_t pi = 0;
       if (lane < nPc) slot = q[lane];
-      else if (lane < nPc + take) { slot = q[lane]; fresh = true; pi = w_next + (lane - nPc); }
+      else if (lane < nPc + take) { slot = q[nP + (lane - nPc)]; fresh = true; pi = w_next + (lane - nPc); }
       w_next += take;
       if (nPc + take == 0) continue;                        // nothing to do this round (queue just ran dry)
       CNT(C_PHASES, 1); CNT(C_LANES_PHYS, nPc); CNT(C_LANES_FRESH, take);
@@ -1283,6 +1298,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
     if (nQ > 0 && idle) {
       if (s0 == S_TRACE) q[__popc(t0 & lt)] = lane;
       if (s1 == S_TRACE) q[__popc(t0) + __popc(t1 & lt)] = lane + 32;
+      if constexpr (kSlots > 64) { if (s2 == S_TRACE) q[__popc(t0) + __popc(t1) + __popc(t2 & lt)] = lane + 64; }
       __syncwarp();
       const int r = __popc(idle & lt);
       if (my < 0 && r < nQ) {
