@@ -792,6 +792,65 @@ static int quantise_nodes(dw_ctx* c, int n_nodes, const float lo[3], const float
   return DW_OK;
 }
 
+#if DW_WIDE8
+// Experiment: the 4-wide tree re-made 8-wide on the host (dw_internal.cuh DW_WIDE8).  Replaces c->d_nodes; the refit state is void.
+static int widen8(dw_ctx* c, int n_nodes, cudaStream_t stream, int* n8_out) {
+  struct Child { float lo[3], hi[3]; int ref; };
+  std::vector<float4> h(8 * (size_t)n_nodes);
+  DW_CUDA(c, cudaStreamSynchronize(stream));
+  DW_CUDA(c, cudaMemcpy(h.data(), c->d_nodes, sizeof(float4) * h.size(), cudaMemcpyDeviceToHost));
+  auto kids = [&](int node, std::vector<Child>& out) {
+    const float* q = reinterpret_cast<const float*>(&h[8 * (size_t)node]);
+    for (int k = 0; k < 4; ++k) {
+      int ref; memcpy(&ref, q + 24 + k, 4);
+      if (ref == DW_REF_NONE) continue;
+      Child ch;
+      for (int a = 0; a < 3; ++a) { ch.lo[a] = q[4 * a + k]; ch.hi[a] = q[12 + 4 * a + k]; }
+      ch.ref = ref;
+      out.push_back(ch);
+    }
+  };
+  auto count4 = [&](int node) { std::vector<Child> t; kids(node, t); return (int)t.size(); };
+  auto area = [](const Child& ch) { const float x = ch.hi[0] - ch.lo[0], y = ch.hi[1] - ch.lo[1], z = ch.hi[2] - ch.lo[2]; return x * y + y * z + z * x; };
+  std::vector<int> from{0};                       // 8-wide node -> the 4-wide node it starts from
+  std::vector<float4> out;
+  for (size_t i = 0; i < from.size(); ++i) {
+    std::vector<Child> L;
+    kids(from[i], L);
+    for (;;) {                                    // pull up the children of the largest inner child that still fits
+      int best = -1;
+      for (int k = 0; k < (int)L.size(); ++k)
+        if (L[k].ref >= 0 && (int)L.size() - 1 + count4(L[k].ref) <= 8 && (best < 0 || area(L[k]) > area(L[best]))) best = k;
+      if (best < 0) break;
+      const int node = L[best].ref;
+      L.erase(L.begin() + best);
+      kids(node, L);
+    }
+    for (Child& ch : L)
+      if (ch.ref >= 0) { from.push_back(ch.ref); ch.ref = (int)from.size() - 1; }
+    float rec[64];
+    for (int half = 0; half < 2; ++half)
+      for (int k = 0; k < 4; ++k) {
+        const int j = 4 * half + k;
+        const bool on = j < (int)L.size();
+        float* q = rec + 32 * half;
+        for (int a = 0; a < 3; ++a) { q[4 * a + k] = on ? L[j].lo[a] : FLT_MAX; q[12 + 4 * a + k] = on ? L[j].hi[a] : -FLT_MAX; }
+        const int ref = on ? L[j].ref : DW_REF_NONE;
+        memcpy(q + 24 + k, &ref, 4);
+        q[28 + k] = 0.f;
+      }
+    for (int v = 0; v < 16; ++v) out.push_back(make_float4(rec[4 * v], rec[4 * v + 1], rec[4 * v + 2], rec[4 * v + 3]));
+  }
+  float4* d = nullptr;
+  DW_CUDA(c, cudaMalloc(&d, sizeof(float4) * out.size()));
+  DW_CUDA(c, cudaMemcpy(d, out.data(), sizeof(float4) * out.size(), cudaMemcpyHostToDevice));
+  cudaFree(c->d_nodes);
+  c->d_nodes = d;
+  *n8_out = (int)from.size();
+  return DW_OK;
+}
+#endif
+
 static int nodes_area(dw_ctx* c, int n_nodes, cudaStream_t stream, double* out) {
   int rc = DW_OK;
   double* d = nullptr;
@@ -1033,6 +1092,15 @@ int dw_bvh_build_impl(dw_ctx* c, const dw_build_params* params, dw_build_stats* 
       rc = nodes_area(c, n_nodes, stream, &r.build_area);
       if (rc != DW_OK) goto done;
     }
+#if DW_WIDE8
+    if (n > 0) {
+      int n8 = 0;
+      rc = widen8(c, n_nodes, stream, &n8);
+      if (rc != DW_OK) goto done;
+      n_nodes = n8;
+      c->bvh.nodes = c->d_nodes; c->bvh.n_nodes = n8;
+    }
+#endif
     if (stats) {
       stats->n_tri = nt; stats->n_refs = n; stats->split_div = split_used; stats->n_nodes = n_nodes; stats->node_bytes = 128ll * n_nodes; stats->tri_bytes = 48ll * n;
       stats->max_depth = wide_depth; stats->n_leaves = h_misc[2];

@@ -47,6 +47,13 @@ constexpr int kDwStackLocal = 84;
 #define DW_NODE_Q16 0
 #endif
 
+// Experiment (off): 8-wide nodes, 256 B = two 4-wide records (children 0-3 and 4-7), made on the host from the 4-wide tree by pulling
+// the children of the largest inner children up while at most 8 result (dw_bvh.cu widen8); a visit tests all eight boxes.  No refit.
+// Measured in profiles/r02_experiments.md section 5g.
+#ifndef DW_WIDE8
+#define DW_WIDE8 0
+#endif
+
 // Triangle record in leaf order, 48 B, read as three float4 (Moeller-Trumbore form):
 //   a = (v0.x, v0.y, v0.z, e1.x)  b = (e1.y, e1.z, e2.x, e2.y)
 //   c = (e2.z, as_float(caller id), as_float(code), as_float(channel))

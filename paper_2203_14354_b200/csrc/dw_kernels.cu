@@ -235,11 +235,44 @@ __device__ __forceinline__ void node_process(const DwBvh& bvh, const Ray& r, Tra
   if (h3 && next != r3) ts_push(s, r3, sstack, sstride, lstack);
   ts_goto(s, next, sstack, sstride, lstack);
 }
+#if DW_WIDE8 && !DW_NODE_Q16
+// One 8-wide node: both halves are tested, the nearest hit child is visited next, the others are pushed as they lose.
+__device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
+  const float4* p = bvh.nodes + 16 * (size_t)s.node;
+  int next = DW_REF_NONE;
+  float bn = INFINITY;
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    NodeRegs n;
+    n.rf = __ldg(p + 8 * h + 6);
+    const int r0 = __float_as_int(n.rf.x), r1 = __float_as_int(n.rf.y), r2 = __float_as_int(n.rf.z), r3 = __float_as_int(n.rf.w);
+    if (h == 1 && r0 == DW_REF_NONE) break;          // children are packed from the front: an empty first child of the second half ends it
+    ldg256(p + 8 * h, n.lx, n.ly); ldg256(p + 8 * h + 2, n.lz, n.hx); ldg256(p + 8 * h + 4, n.hy, n.hz);
+    float n0, n1, n2, n3;
+    const bool h0 = slab(r, s.best_t, bvh.eps_len, n.lx.x, n.ly.x, n.lz.x, n.hx.x, n.hy.x, n.hz.x, n0) && (r0 != DW_REF_NONE);
+    const bool h1 = slab(r, s.best_t, bvh.eps_len, n.lx.y, n.ly.y, n.lz.y, n.hx.y, n.hy.y, n.hz.y, n1) && (r1 != DW_REF_NONE);
+    const bool h2 = slab(r, s.best_t, bvh.eps_len, n.lx.z, n.ly.z, n.lz.z, n.hx.z, n.hy.z, n.hz.z, n2) && (r2 != DW_REF_NONE);
+    const bool h3 = slab(r, s.best_t, bvh.eps_len, n.lx.w, n.ly.w, n.lz.w, n.hx.w, n.hy.w, n.hz.w, n3) && (r3 != DW_REF_NONE);
+    const int prev = next;                             // the nearest of the first half loses if this half holds a nearer one
+    if (h0 && (next == DW_REF_NONE || n0 < bn)) { next = r0; bn = n0; }
+    if (h1 && (next == DW_REF_NONE || n1 < bn)) { next = r1; bn = n1; }
+    if (h2 && (next == DW_REF_NONE || n2 < bn)) { next = r2; bn = n2; }
+    if (h3 && (next == DW_REF_NONE || n3 < bn)) { next = r3; bn = n3; }
+    if (prev != DW_REF_NONE && next != prev) ts_push(s, prev, sstack, sstride, lstack);
+    if (h0 && next != r0) ts_push(s, r0, sstack, sstride, lstack);
+    if (h1 && next != r1) ts_push(s, r1, sstack, sstride, lstack);
+    if (h2 && next != r2) ts_push(s, r2, sstack, sstride, lstack);
+    if (h3 && next != r3) ts_push(s, r3, sstack, sstride, lstack);
+  }
+  ts_goto(s, next, sstack, sstride, lstack);
+}
+#else
 __device__ __forceinline__ void step_internal(const DwBvh& bvh, const Ray& r, TraceState& s, int* sstack, int sstride, int* lstack) {
   NodeRegs n;
   node_load(bvh, s.node, n);
   node_process(bvh, r, s, n, sstack, sstride, lstack);
 }
+#endif
 
 // One triangle of the current leaf (Moeller-Trumbore on the pre-packed record).  exclude: caller id to ignore.
 // medium >= 0: only triangles whose near side (the side the ray comes from) is `medium` count (DESIGN.md
