@@ -960,6 +960,13 @@ constexpr int warp_ints(bool lean) { return warp_stack(lean) + kStackShared * 32
 // inside the phase ran its later iterations for the few lanes still rejected: 9 of 32 lanes on average over the loop; one iteration
 // per phase costs more in slot traffic than it saves: profiles/r02_experiments.md.)  Draws are keyed by (photon, step, block 1 + j):
 // same results.  0: the loop of the first build.
+// DW_RAYL_COOP 1: the loop S6 for all lanes of a phase together, every lane of the warp drawing one candidate for one of the
+// scattering photons (up to four candidates per photon and round; results bit-identical).  Measured: 18.5 instead of 15.6 lanes per
+// instruction, the same number of instructions, 1.4 kB more code -> 0.95 instead of 0.33 stall cycles per instruction waiting for
+// instructions, 44.7 against 42.1 ms (profiles/r02_experiments.md section 5h).  Off.
+#ifndef DW_RAYL_COOP
+#define DW_RAYL_COOP 0
+#endif
 #ifndef DW_RAYL_REQUEUE
 #define DW_RAYL_REQUEUE 0
 #endif
@@ -1160,8 +1167,8 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
               if (absorb_first) {
                 fate = DW_FATE_BULK_ABSORBED;                         // S4 first branch
               } else {                                                // S4 second branch + S6
-#if DW_RAYL_REQUEUE
-                rj = 0;                                               // the loop runs below, one iteration per phase
+#if DW_RAYL_REQUEUE || DW_RAYL_COOP
+                rj = 0;                                               // the loop runs below, for all lanes of the phase together
                 --step;                                               // S9 counts the step when the loop ends
 #else
                 if (!rayleigh(k, e, [&](uint32_t b) { return DRAW_HOT(pid, step, b); })) fate = DW_FATE_NAN_ABORT;
@@ -1218,7 +1225,49 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
         }
         ++step;                                                       // S9 (every executed iteration counts, also the last: S13)
       }
-#if DW_RAYL_REQUEUE
+#if DW_RAYL_COOP
+      // S6 for all lanes of the phase together.  The rejection loop accepts two candidates in three, so run lane by lane it takes the
+      // warp four iterations at nine, three, one lanes.  Here every lane of the warp draws ONE candidate for one of the nR scattering
+      // photons: lane l serves the photon of rank l % nR with candidate number rj + l / nR (Philox block 1 + that number, as in the
+      // loop), and a photon takes its accepted candidate of lowest number: the same direction and polarisation as the loop's.
+#pragma unroll 1
+      for (;;) {
+        const unsigned rm = __ballot_sync(0xffffffffu, rj >= 0);
+        if (!rm) break;
+        const int nR = __popc(rm);
+        const int rank = __popc(rm & lt);
+        CNT(C_RAYL_ITER, 1); CNT(C_LANES_RAYL, nR);
+        __syncwarp();
+        if (rj >= 0) q[rank] = lane;
+        __syncwarp();
+        const int cand = (lane >= nR) + (lane >= 2 * nR) + (lane >= 3 * nR);   // lane / nR, at most four candidates per photon and round
+        const int src = q[min(lane - cand * nR, nR - 1)];             // the lane whose photon this lane draws for (lanes >= 4 nR: unused)
+        const uint32_t pi_r = __shfl_sync(0xffffffffu, (uint32_t)pi, src), step_r = __shfl_sync(0xffffffffu, step, src);
+        const int rj_r = __shfl_sync(0xffffffffu, rj, src);
+        const V3 e_r = mk(__shfl_sync(0xffffffffu, e.x, src), __shfl_sync(0xffffffffu, e.y, src), __shfl_sync(0xffffffffu, e.z, src));
+        const float4 r = DRAW_HOT(A.in.photon_id_base + (uint64_t)pi_r, step_r, 1u + (uint32_t)(rj_r + cand));
+        const float ct = 1.0f - 2.0f * r.x;
+        const float st_ = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+        float sp, cp;
+        sincospif(2.0f * r.y, &sp, &cp);
+        const V3 kn = mk(st_ * cp, st_ * sp, ct);
+        V3 er = fma3(-dot(e_r, kn), kn, e_r);
+        const float w = dot(er, er);
+        er = rsqrtf(w) * er;
+        const unsigned acc = __ballot_sync(0xffffffffu, r.z < w && lane < 4 * nR);
+        const unsigned stride = 1u | (nR < 32 ? 1u << nR : 0u) | (2 * nR < 32 ? 1u << (2 * nR) : 0u) | (3 * nR < 32 ? 1u << (3 * nR) : 0u);
+        const unsigned mine = stride << rank;                         // the lanes that drew for this lane's photon (lanes >= 32 drop out)
+        const int win = __ffs(acc & mine) - 1;
+        const int from = win >= 0 ? win : lane;
+        const V3 kw = mk(__shfl_sync(0xffffffffu, kn.x, from), __shfl_sync(0xffffffffu, kn.y, from), __shfl_sync(0xffffffffu, kn.z, from));
+        const V3 ew = mk(__shfl_sync(0xffffffffu, er.x, from), __shfl_sync(0xffffffffu, er.y, from), __shfl_sync(0xffffffffu, er.z, from));
+        if (rj >= 0) {
+          if (win >= 0) { k = kw; e = ew; ++step; rj = -1; }                                        // S9
+          else if (rj + __popc(mine) >= 4096) { fate = DW_FATE_NAN_ABORT; ++step; rj = -1; }        // the loop gives up (never observed)
+          else rj += __popc(mine);
+        }
+      }
+#elif DW_RAYL_REQUEUE
 #pragma unroll 1
       for (int it = 0; it < DW_RAYL_REQUEUE; ++it) {
         const unsigned rm = __ballot_sync(0xffffffffu, rj >= 0);
@@ -1239,7 +1288,7 @@ __global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_
           else ++rj;
         }
       }
-      if (slot >= 0 && rj >= 0) {
+      if (DW_RAYL_REQUEUE && slot >= 0 && rj >= 0) {
         // rejected: the slot waits for the next phase with the iteration number (position and time are those of the scatter point)
         poolf[W_X * kSlots + slot] = x.x; poolf[W_Y * kSlots + slot] = x.y; poolf[W_Z * kSlots + slot] = x.z;
         poolf[W_T * kSlots + slot] = t;
