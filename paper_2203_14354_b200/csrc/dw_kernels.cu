@@ -621,9 +621,13 @@ struct PropArgs {
 #ifndef DW_PHILOX_KEYS
 #define DW_PHILOX_KEYS 2
 #endif
+#ifndef DW_PHILOX_UNROLL
+#define DW_PHILOX_UNROLL 10
+#endif
+constexpr int kPhiloxUnroll = DW_PHILOX_UNROLL;   // rounds per loop iteration of the inlined generator (10: no loop)
 __device__ __forceinline__ float4 draw4_keys(const PropArgs& A, uint64_t pid, uint32_t step, uint32_t block) {
   uint4 c = make_uint4((uint32_t)pid, (uint32_t)(pid >> 32), step, block);
-#pragma unroll
+#pragma unroll(kPhiloxUnroll)
   for (int r = 0; r < 10; ++r) {
     uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
     uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
