@@ -522,6 +522,20 @@ def main():
         except Exception:
             pass
 
+    # what ncu measured for this kernel on this workload (issue slots, lanes per instruction, L1 / L2 throughput), beside the model
+    cap_file = ROOT / "profiles" / "capture_metrics.csv"
+    if cap_file.exists() and n == c.n_photons and not args.legacy:
+        try:
+            import csv
+            rows = [r for r in csv.DictReader(cap_file.open()) if r["config"] == f"C{args.config}"]
+            if rows:
+                cap = {r["metric"]: float(r["value"]) for r in rows}
+                cap["warp_instructions_per_photon_step"] = cap["smsp__inst_executed.sum"] / steps_per_launch if steps_per_launch else None
+                cap["source"] = "NOT measured in this run: one ncu --set full capture of the same kernel and workload, profiles/capture_metrics.md"
+                roofline["ncu_capture"] = cap
+        except Exception:
+            pass
+
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         cpu, _ = cpu_baseline(c, args.ref_sample)
