@@ -9,7 +9,7 @@
 
 #include "../../include/darwinopt.h"
 
-#define DW_VERSION 108
+#define DW_VERSION 109
 
 // ---------------------------------------------------------------------------------------------------------
 // Device-side views (plain structs passed by value to kernels)

@@ -463,7 +463,21 @@ __device__ __forceinline__ Cf csqrtf_(Cf a) {               // principal square 
   return cf(re, a.im < 0.f ? -im : im);
 }
 // Returns 0 reflected, 1 transmitted (crossed into the other medium), 2 absorbed in the film.  nh faces the photon.
-__device__ __noinline__ int film_event(float n1, float nf, float kf, float d_nm, float n3, float lambda, V3 nh, V3& k, V3& e, float u) {
+// The film event inline in the film-enabled instantiation (which keeps one block fewer per SM and 96 registers): C2 with silicon-film
+// cathodes 41.1 against 43.7 ms per 4e6 photons with the call; with films set and none switched on 21.2 either way (18.8 in the
+// film-free instantiation).  Six blocks at 80 registers lose both ways (inline 47.3, call 46.6): profiles/r02_experiments.md 5i.
+#ifndef DW_FILM_INLINE
+#define DW_FILM_INLINE 1
+#endif
+#if DW_FILM_INLINE
+#define DW_FILM_ATTR __forceinline__
+#else
+#define DW_FILM_ATTR __noinline__
+#endif
+#ifndef DW_FILM_BLOCKS_LESS
+#define DW_FILM_BLOCKS_LESS 1
+#endif
+__device__ DW_FILM_ATTR int film_event(float n1, float nf, float kf, float d_nm, float n3, float lambda, V3 nh, V3& k, V3& e, float u) {
   const float ci = -dot(k, nh);
   const V3 sv = cross(k, nh);
   const float si2 = dot(sv, sv), si = sqrtf(si2);
@@ -981,7 +995,7 @@ enum : int { C_NODE = 0, C_TRI, C_TRACED, C_SKIPPED, C_PHASES, C_LANES_PHYS, C_L
              C_Q_FRESH, C_N_FRESH, C_Q_SURF, C_N_SURF, C_H_SURF, C_Q_BULK, C_N_BULK, C_H_BULK, kCounters = 24 };
 
 template <bool kFilm, bool kFlat, bool kCount>
-__global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - 1 : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
+__global__ void __launch_bounds__(128, kFilm ? DW_POOL_MIN_BLOCKS - DW_FILM_BLOCKS_LESS : DW_POOL_MIN_BLOCKS) propagate_pool_kernel(const __grid_constant__ PropArgs A) {
   extern __shared__ int s_dyn[];
   __shared__ unsigned long long s_cnt[kCount ? kCounters : 1];
   if constexpr (kCount) { if (threadIdx.x < kCounters) s_cnt[threadIdx.x] = 0ull; }
