@@ -119,11 +119,26 @@ struct Ray {
   V3 inv, oi;  // fp32 nodes: 1/d (zero components pushed to +-1e30) and o * inv, so that a plane p is met at p * inv - oi;
                // 16-bit nodes: the same for a plane given as q steps of q_cs from q_lo: q * (q_cs / d) - (o - q_lo) / d
 };
+// 1 / det of the triangle test by MUFU as well: another 0.8 %, but the finer closed sphere then leaks 6 of 4e6 photons instead of 2
+// (budget 4: tests/test_gpu_parity.py test_leak_budget_second_seed_and_finer_sphere); the edge rules count on the rounded quotient.  Off.
+#ifndef DW_TRI_RCP_APPROX
+#define DW_TRI_RCP_APPROX 0
+#endif
+// 1 / d of the ray set-up by MUFU.RCP alone (C2 42.18 -> 41.67 ms, C3 44.44 -> 43.93; results unchanged on C0-C3, 86 GPU tests pass).
+#ifndef DW_RAY_RCP_APPROX
+#define DW_RAY_RCP_APPROX 1
+#endif
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ void ray_setup(Ray& r, V3 o, V3 d, const DwBvh& bvh) {
   const float tiny = 1e-30f;   // zero components become +-tiny so that 0 * inf never appears
   r.o = o; r.d = d;
+#if DW_RAY_RCP_APPROX   // one MUFU each (1 ulp; the slab test has a slack of 8 ulp): an IEEE division is 14 instructions with its slow path
+  const V3 inv = mk(rcp_approx(fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), rcp_approx(fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
+                    rcp_approx(fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
+#else
   const V3 inv = mk(1.0f / (fabsf(d.x) > tiny ? d.x : copysignf(tiny, d.x)), 1.0f / (fabsf(d.y) > tiny ? d.y : copysignf(tiny, d.y)),
                     1.0f / (fabsf(d.z) > tiny ? d.z : copysignf(tiny, d.z)));
+#endif
 #if DW_NODE_Q16
   r.inv = mk(bvh.q_cs.x * inv.x, bvh.q_cs.y * inv.y, bvh.q_cs.z * inv.z);
   r.oi = mk((o.x - bvh.q_lo.x) * inv.x, (o.y - bvh.q_lo.y) * inv.y, (o.z - bvh.q_lo.z) * inv.z);
@@ -304,7 +319,11 @@ __device__ __forceinline__ void tri_process(const Ray& r, TraceState& s, const T
   V3 pv = cross(r.d, e2);
   float det = dot(e1, pv);
   if (fabsf(det) >= 1e-30f) {
+#if DW_TRI_RCP_APPROX
+    float idet = rcp_approx(det);
+#else
     float idet = 1.0f / det;
+#endif
     V3 tv = mk(r.o.x - a.x, r.o.y - a.y, r.o.z - a.z);
     float u = dot(tv, pv) * idet;
     V3 qv = cross(tv, e1);
